@@ -1,0 +1,145 @@
+/*
+ * nb.h -- C ABI of the B200 cluster-pair short-range non-bonded library.
+ *
+ * The five working calls are the ones BASELINE.json's north_star lists
+ * (nb_init / nb_put_atoms / nb_search / nb_prune / nb_forces); they follow the paper's
+ * statement of the problem: positions go in and forces come out every step
+ * (PAPER.md L105), the pair list is built rarely and reused for many steps (L185, L193),
+ * pruning runs in rolling chunks between force computations (L193).
+ *
+ * Conventions
+ *  - Pointers marked [dev] are CUDA device pointers owned by the caller; the library
+ *    never frees them and never keeps them past the call.  Everything else is host memory.
+ *    [host] variants (suffix _host) take plain host pointers and do the copies themselves.
+ *  - Every call returns NB_OK or a negative NB_ERR_* code; nothing throws or exits.
+ *    nb_last_error() gives a message for the last failure on that context.
+ *  - All work is enqueued on the stream given in nb_params and returns without
+ *    synchronising, except nb_search (reads list sizes back to size buffers) and the
+ *    introspection / _host calls.
+ *  - Call order: nb_init -> nb_put_atoms -> nb_search -> { nb_put_atoms -> [nb_prune] ->
+ *    nb_forces }* -> nb_put_atoms -> nb_search ...; violations return NB_ERR_STATE.
+ *  - Units: nm, kJ/mol, e.  Rectangular periodic boxes only.  natoms, types, charges'
+ *    layout and exclusions are fixed for the lifetime of a context (only
+ *    positions change per step).
+ *  - Between searches the caller passes CONTINUOUS (not re-wrapped) coordinates; the
+ *    library applies the periodic image fixed for each atom at the last search.
+ *
+ * Cluster geometry: clusters of NB_CLUSTER_SIZE = 8 atoms, 8 clusters
+ * (2x2x2 cells of the search grid) per super-cluster, one joint j-cluster list per
+ * (super-cluster, periodic shift) with an 8-bit interaction mask per j-cluster.
+ */
+#ifndef NB_B200_H
+#define NB_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NB_CLUSTER_SIZE 8
+#define NB_SUPER_SIZE 8        /* clusters per super-cluster */
+#define NB_NSHIFT 27
+#define NB_SHIFT_CENTER 13     /* shift id = (sx+1) + 3*(sy+1) + 9*(sz+1), s in {-1,0,1}^3 */
+#define NB_MAX_TYPES 96
+
+typedef struct nb_ctx nb_ctx; /* opaque, owned by the library */
+
+enum { NB_OK = 0, NB_ERR_ARG = -1, NB_ERR_STATE = -2, NB_ERR_CUTOFF = -3, NB_ERR_BOX = -4,
+       NB_ERR_NOMEM = -5, NB_ERR_CUDA = -6, NB_ERR_OVERFLOW = -7 };
+enum { NB_COUL_EWALD = 0, NB_COUL_RF = 1 };
+enum { NB_MOD_NONE = 0, NB_MOD_POTSHIFT = 1 };
+
+typedef struct {
+    int32_t natoms, ntypes;          /* ntypes <= NB_MAX_TYPES */
+    const float* lj_c6c12;           /* host [ntypes*ntypes*2]: c6 = 4 eps sigma^6, c12 = 4 eps sigma^12; copied */
+    const int32_t* excl_off;         /* host CSR [natoms+1]; copied.  NULL = no exclusions */
+    const int32_t* excl_idx;         /* host [excl_off[natoms]]; symmetric, no self entries; copied */
+    float rc;                        /* interaction cut-off, nm (LJ and Coulomb; interact iff r^2 < rc^2) */
+    int32_t coulomb;                 /* NB_COUL_* */
+    float ewald_beta;                /* nm^-1; if <= 0 derived from ewald_rtol: erfc(beta*rc) = rtol.
+                                        (beta*rc)^2 must be <= 16 (range of the correction fit) */
+    float ewald_rtol;
+    float eps_rf;                    /* reaction-field dielectric; <= 0 or inf -> infinity (eps_r = 1) */
+    float epsfac;                    /* 1/(4 pi eps0); 0 -> 138.935458 kJ mol^-1 nm e^-2 */
+    int32_t lj_modifier;             /* NB_MOD_*: potential-shift changes energies only */
+    int32_t coul_modifier;           /* Ewald only; reaction-field always carries its own constant c_rf */
+    int32_t device;                  /* CUDA ordinal */
+    void* stream;                    /* cudaStream_t (NULL = legacy default stream) */
+} nb_params;
+
+/* Counters for the last calls; all device work they describe has completed when
+ * nb_get_stats returns (it synchronises the stream). */
+typedef struct {
+    int32_t cluster_size, nclusters, nsuper, nslots;
+    int32_t ncolumns_x, ncolumns_y;
+    int64_t n_sci_entries;           /* non-empty (super-cluster, shift) list elements */
+    int64_t n_joint_outer;           /* joint j entries with any outer mask bit */
+    int64_t n_pairs_outer;           /* listed cluster pairs (ci,cj,s): outer mask bits set */
+    int64_t n_pairs_inner;           /* cluster pairs with the inner mask bit set (after pruning) */
+    int64_t n_excl_masks;            /* joint entries carrying a non-trivial exclusion mask */
+    int64_t n_work_units;            /* list chunks scheduled by the force/prune kernels (L199-L201) */
+    int64_t slots_last_forces;       /* atom-pair slots evaluated by the last nb_forces = 64 * n_pairs_inner */
+    int64_t kernel_launches;         /* kernels launched by this context so far */
+    int64_t search_count, prune_count, force_count;
+    int32_t list_grow_retries;
+    float ewald_beta;
+} nb_stats;
+
+/* Creates a context.  Copies the LJ table and exclusions.  NB_ERR_ARG on bad sizes,
+ * an exclusion index out of range, rc <= 0, or (beta*rc)^2 > 16. */
+int nb_init(const nb_params* p, nb_ctx** out);
+
+/* (a1) Coordinate staging.  x [dev] natoms*3 fp32, q [dev] natoms,
+ * type [dev] natoms (0 <= type < ntypes), box host [3] (Lx,Ly,Lz > 0).  Copies them; if a
+ * grid exists and the box is unchanged, also refreshes the cluster-ordered (x,y,z,q) array. */
+int nb_put_atoms(nb_ctx*, const float* x, const float* q, const int32_t* type, const float box[3]);
+/* Same with host pointers (pageable or pinned); copies are enqueued on the stream. */
+int nb_put_atoms_host(nb_ctx*, const float* x, const float* q, const int32_t* type, const float box[3]);
+
+/* (a2)-(a5) Gridding into clusters (L129-L131), bounding-box pair search with interaction
+ * masks (L131-L133, L187), exclusion masks (L135), list splitting/sorting (L199-L201).
+ * Sets inner list := outer list.  NB_ERR_CUTOFF unless rc <= rlist_outer <= min(L)/2;
+ * NB_ERR_BOX for a non-positive box.  Synchronises (reads list sizes). */
+int nb_search(nb_ctx*, float rlist_outer);
+
+/* (a6) Dynamic pruning (L187-L193): recomputes the inner interaction mask of rolling part
+ * `part` of `nparts` of the outer list from the current coordinates: a cluster pair stays
+ * iff some atom pair is closer than rlist_inner.  Needs rc <= rlist_inner <= rlist_outer,
+ * 0 <= part < nparts; nparts = 1 prunes everything. */
+int nb_prune(nb_ctx*, float rlist_inner, int part, int nparts);
+
+/* (a7)-(a8) Forces over the inner list.  f [dev] natoms*3 fp32 in the caller's atom order,
+ * overwritten.  energies [dev] double[2] = {E_lj, E_coul} (kJ/mol) or NULL for the force-only
+ * kernel flavour (L139).  virial [dev] double[9] row-major, Xi = -1/2 sum_pairs d (x) F, or
+ * NULL; a non-NULL virial requires non-NULL energies. */
+int nb_forces(nb_ctx*, float* f, double* energies, double* virial);
+/* Same with host pointers; synchronises before returning. */
+int nb_forces_host(nb_ctx*, float* f, double* energies, double* virial);
+
+void nb_free(nb_ctx*);
+const char* nb_last_error(const nb_ctx*);
+
+/* ---- introspection: for parity tests and statistics only; these synchronise ---- */
+int nb_get_layout(nb_ctx*, int32_t* cluster_size, int32_t* nclusters, int32_t* nsuper, int32_t* nslots);
+/* atom_of_slot [dev] nslots (-1 = padding); xq [dev] nslots*4 (x,y,z,q as used by the kernels:
+ * wrapped at the last search, then moved by nb_put_atoms).  Either may be NULL. */
+int nb_get_slots(nb_ctx*, int32_t* atom_of_slot, float* xq);
+/* Number of listed cluster pairs (ci,cj,shift): which = 0 outer, 1 inner. */
+int nb_list_count(nb_ctx*, int which, int64_t* n);
+/* Dumps the list in its stored order (deterministic).  All arrays [dev] with n entries (n from
+ * nb_list_count); any may be NULL.  shift: 0..26 as defined by NB_SHIFT_CENTER, displacing the
+ * i-cluster: d = x_a + s L - x_b.  pairmask bit a*8+b = 1: atoms a of ci and b of cj interact
+ * (both real, not excluded, not the same atom, and b > a when ci == cj at zero shift).
+ * part: rolling part of the entry under the nparts of the last nb_prune (0 before any prune). */
+int nb_list_dump(nb_ctx*, int which, int32_t* ci, int32_t* cj, int32_t* shift, uint64_t* pairmask,
+                 int32_t* part);
+int nb_get_stats(nb_ctx*, nb_stats* out);
+/* Measures the device's FP32 FMA issue peak with a register-resident FFMA chain kernel
+ * (MEASURED_PEAKS.json has no FP32 entry).  Returns lane-FMA/s in *fma_per_s. */
+int nb_measure_fp32_peak(nb_ctx*, double* fma_per_s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NB_B200_H */

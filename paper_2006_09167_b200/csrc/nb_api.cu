@@ -1,0 +1,265 @@
+// nb_api.cu -- the C ABI of include/nb.h: argument checking, state machine, parameter
+// preparation and memory ownership.  All arithmetic of the method lives in the kernels of
+// nb_grid.cu / nb_list.cu / nb_prune.cu / nb_force.cu.  Links the CUDA runtime only.
+#include "nb_internal.h"
+
+#include <math.h>
+#include <stdarg.h>
+
+#include <new>
+
+int nb_fail(nb_ctx* c, int code, const char* fmt, ...)
+{
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof(c->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+static bool finite_pos(float v) { return v > 0.f && isfinite(v); }
+
+extern "C" int nb_init(const nb_params* p, nb_ctx** out)
+{
+    if (!p || !out) return NB_ERR_ARG;
+    *out = nullptr;
+    if (p->natoms <= 0 || p->ntypes <= 0 || p->ntypes > NB_MAX_TYPES || !p->lj_c6c12 || !finite_pos(p->rc)) return NB_ERR_ARG;
+    if (p->coulomb != NB_COUL_EWALD && p->coulomb != NB_COUL_RF) return NB_ERR_ARG;
+    if (p->excl_off && p->excl_off[p->natoms] > 0 && !p->excl_idx) return NB_ERR_ARG;
+    if (cudaSetDevice(p->device) != cudaSuccess) return NB_ERR_CUDA;
+    nb_ctx* c = new (std::nothrow) nb_ctx();
+    if (!c) return NB_ERR_NOMEM;
+    c->err[0] = 0;
+    memset(&c->st, 0, sizeof(c->st));
+    c->prm = *p;
+    c->prm.lj_c6c12 = nullptr; c->prm.excl_off = nullptr; c->prm.excl_idx = nullptr;
+    c->stream = (cudaStream_t)p->stream;
+    c->natoms = p->natoms;
+    c->ntypes = p->ntypes;
+    *out = c;   // returned even on failure below so that nb_last_error() can be read; nb_free() it
+
+    // ---- interaction constants (fp64 on the host, stored fp32) ----
+    const double rc = p->rc;
+    const double epsfac = p->epsfac != 0.f ? (double)p->epsfac : 138.935458;   // reading A2
+    double beta = 0.0;
+    if (p->coulomb == NB_COUL_EWALD) {
+        if (p->ewald_beta > 0.f) beta = p->ewald_beta;
+        else {
+            if (!(p->ewald_rtol > 0.f && p->ewald_rtol < 1.f)) return nb_fail(c, NB_ERR_ARG, "ewald_rtol must be in (0,1) when ewald_beta <= 0");
+            double lo = 0.0, hi = 1.0;   // reading A3: erfc(beta*rc) = rtol
+            while (erfc(hi * rc) > p->ewald_rtol) hi *= 2.0;
+            for (int it = 0; it < 200; it++) {
+                double mid = 0.5 * (lo + hi);
+                if (erfc(mid * rc) > p->ewald_rtol) lo = mid; else hi = mid;
+            }
+            beta = 0.5 * (lo + hi);
+        }
+        if (beta * rc * beta * rc > 16.0) return nb_fail(c, NB_ERR_ARG, "(beta*rc)^2 = %g exceeds 16, the range of the Ewald correction fit", beta * rc * beta * rc);
+    }
+    NbConst& K = c->kc;
+    memset(&K, 0, sizeof(K));
+    K.rc2 = p->rc * p->rc;
+    K.epsfac = (float)epsfac;
+    K.beta = (float)beta; K.beta2 = (float)(beta * beta); K.beta3 = (float)(beta * beta * beta);
+    K.ewald_shift = (p->coulomb == NB_COUL_EWALD && p->coul_modifier == NB_MOD_POTSHIFT) ? (float)(erfc(beta * rc) / rc) : 0.f;
+    double krf = (p->eps_rf <= 0.f || isinf(p->eps_rf)) ? 1.0 / (2.0 * rc * rc * rc)
+                                                         : ((double)p->eps_rf - 1.0) / ((2.0 * p->eps_rf + 1.0) * rc * rc * rc);   // reading A6
+    K.krf = (float)krf; K.two_krf = (float)(2.0 * krf); K.crf = (float)(1.0 / rc + krf * rc * rc);
+    K.lj_sh6 = p->lj_modifier == NB_MOD_POTSHIFT ? (float)pow(rc, -6.0) : 0.f;
+    K.lj_sh12 = p->lj_modifier == NB_MOD_POTSHIFT ? (float)pow(rc, -12.0) : 0.f;
+    K.ntypes1 = p->ntypes + 1;
+    c->beta = (float)beta;
+    c->st.ewald_beta = (float)beta;
+
+    cudaStream_t st = c->stream;
+    const int n = p->natoms, nt1 = p->ntypes + 1;
+    std::vector<float2> tab((size_t)nt1 * nt1, make_float2(0.f, 0.f));
+    for (int i = 0; i < p->ntypes; i++)
+        for (int j = 0; j < p->ntypes; j++) {
+            const float* e = p->lj_c6c12 + 2 * ((size_t)i * p->ntypes + j);
+            tab[(size_t)i * nt1 + j] = make_float2(6.f * e[0], 12.f * e[1]);
+        }
+    NB_CUDA(c, c->ljtab.ensure(tab.size(), st));
+    NB_CUDA(c, cudaMemcpyAsync(c->ljtab.p, tab.data(), tab.size() * sizeof(float2), cudaMemcpyHostToDevice, st));
+    std::vector<int32_t> zero_off;
+    const int32_t* eo = p->excl_off;
+    if (!eo) { zero_off.assign(n + 1, 0); eo = zero_off.data(); }
+    c->nexcl = eo[n];
+    if (eo[0] != 0 || c->nexcl < 0) return nb_fail(c, NB_ERR_ARG, "excl_off must start at 0 and be non-decreasing");
+    for (int i = 0; i < n; i++) {
+        if (eo[i + 1] < eo[i]) return nb_fail(c, NB_ERR_ARG, "excl_off must be non-decreasing");
+        for (int k = eo[i]; k < eo[i + 1]; k++)
+            if (p->excl_idx[k] < 0 || p->excl_idx[k] >= n || p->excl_idx[k] == i)
+                return nb_fail(c, NB_ERR_ARG, "exclusion %d of atom %d is out of range or a self entry", k, i);
+    }
+    NB_CUDA(c, c->excl_off.ensure(n + 1, st));
+    NB_CUDA(c, c->excl_idx.ensure(c->nexcl + 1, st));
+    NB_CUDA(c, cudaMemcpyAsync(c->excl_off.p, eo, sizeof(int32_t) * (n + 1), cudaMemcpyHostToDevice, st));
+    if (c->nexcl) NB_CUDA(c, cudaMemcpyAsync(c->excl_idx.p, p->excl_idx, sizeof(int32_t) * c->nexcl, cudaMemcpyHostToDevice, st));
+    NB_CUDA(c, c->x.ensure((size_t)3 * n, st));
+    NB_CUDA(c, c->q.ensure(n, st));
+    NB_CUDA(c, c->type.ensure(n, st));
+    NB_CUDA(c, cudaStreamSynchronize(st));   // host staging vectors go out of scope
+    return NB_OK;
+}
+
+static int put_atoms_common(nb_ctx* c, const float* x, const float* q, const int32_t* type, const float box[3], cudaMemcpyKind kind)
+{
+    if (!c) return NB_ERR_ARG;
+    if (!x || !q || !type || !box) return nb_fail(c, NB_ERR_ARG, "nb_put_atoms: null argument");
+    for (int k = 0; k < 3; k++)
+        if (!finite_pos(box[k])) return nb_fail(c, NB_ERR_BOX, "box[%d] = %g is not positive", k, box[k]);
+    cudaStream_t st = c->stream;
+    const int n = c->natoms;
+    NB_CUDA(c, cudaMemcpyAsync(c->x.p, x, sizeof(float) * 3 * n, kind, st));
+    NB_CUDA(c, cudaMemcpyAsync(c->q.p, q, sizeof(float) * n, kind, st));
+    NB_CUDA(c, cudaMemcpyAsync(c->type.p, type, sizeof(int32_t) * n, kind, st));
+    for (int k = 0; k < 3; k++) c->box[k] = box[k];
+    c->have_atoms = true;
+    c->atoms_since_search = true;
+    if (c->have_grid) {
+        if (box[0] != c->grid_box[0] || box[1] != c->grid_box[1] || box[2] != c->grid_box[2]) {
+            c->have_list = false;   // a new box needs a new search
+            c->have_grid = false;
+        } else {
+            return nbi_refresh_xq(c);
+        }
+    }
+    return NB_OK;
+}
+
+extern "C" int nb_put_atoms(nb_ctx* c, const float* x, const float* q, const int32_t* type, const float box[3])
+{
+    return put_atoms_common(c, x, q, type, box, cudaMemcpyDeviceToDevice);
+}
+
+extern "C" int nb_put_atoms_host(nb_ctx* c, const float* x, const float* q, const int32_t* type, const float box[3])
+{
+    return put_atoms_common(c, x, q, type, box, cudaMemcpyHostToDevice);
+}
+
+extern "C" int nb_search(nb_ctx* c, float rlist_outer)
+{
+    if (!c) return NB_ERR_ARG;
+    if (!c->have_atoms) return nb_fail(c, NB_ERR_STATE, "nb_search before nb_put_atoms");
+    const float minL = fminf(c->box[0], fminf(c->box[1], c->box[2]));
+    if (!(rlist_outer >= c->prm.rc) || !(rlist_outer <= 0.5f * minL))
+        return nb_fail(c, NB_ERR_CUTOFF, "rlist_outer = %g must satisfy rc = %g <= rlist_outer <= min(L)/2 = %g", rlist_outer, c->prm.rc, 0.5f * minL);
+    c->have_list = false;
+    return nbi_search(c, rlist_outer);
+}
+
+extern "C" int nb_prune(nb_ctx* c, float rlist_inner, int part, int nparts)
+{
+    if (!c) return NB_ERR_ARG;
+    if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "nb_prune without a valid list (call nb_search)");
+    if (nparts < 1 || part < 0 || part >= nparts) return nb_fail(c, NB_ERR_ARG, "nb_prune: part %d of %d", part, nparts);
+    if (!(rlist_inner >= c->prm.rc) || !(rlist_inner <= c->rlist_outer))
+        return nb_fail(c, NB_ERR_CUTOFF, "rlist_inner = %g must satisfy rc = %g <= rlist_inner <= rlist_outer = %g", rlist_inner, c->prm.rc, c->rlist_outer);
+    return nbi_prune(c, rlist_inner, part, nparts);
+}
+
+extern "C" int nb_forces(nb_ctx* c, float* f, double* energies, double* virial)
+{
+    if (!c) return NB_ERR_ARG;
+    if (!f) return nb_fail(c, NB_ERR_ARG, "nb_forces: f is null");
+    if (virial && !energies) return nb_fail(c, NB_ERR_ARG, "nb_forces: virial needs energies (same kernel flavour)");
+    if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "nb_forces without a valid list (call nb_search)");
+    return nbi_forces(c, f, energies, virial);
+}
+
+extern "C" int nb_forces_host(nb_ctx* c, float* f, double* energies, double* virial)
+{
+    if (!c) return NB_ERR_ARG;
+    if (!f) return nb_fail(c, NB_ERR_ARG, "nb_forces_host: f is null");
+    cudaStream_t st = c->stream;
+    NB_CUDA(c, c->stage_f.ensure((size_t)3 * c->natoms, st));
+    NB_CUDA(c, c->stage_ev.ensure(16, st));
+    int rc = nb_forces(c, c->stage_f.p, energies ? c->stage_ev.p : nullptr, virial ? c->stage_ev.p + 2 : nullptr);
+    if (rc != NB_OK) return rc;
+    NB_CUDA(c, cudaMemcpyAsync(f, c->stage_f.p, sizeof(float) * 3 * c->natoms, cudaMemcpyDeviceToHost, st));
+    if (energies) NB_CUDA(c, cudaMemcpyAsync(energies, c->stage_ev.p, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (virial) NB_CUDA(c, cudaMemcpyAsync(virial, c->stage_ev.p + 2, 9 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    NB_CUDA(c, cudaStreamSynchronize(st));
+    return NB_OK;
+}
+
+extern "C" void nb_free(nb_ctx* c)
+{
+    if (!c) return;
+    cudaStreamSynchronize(c->stream);
+    c->x.release(); c->q.release(); c->type.release();
+    c->stage_x.release(); c->stage_q.release(); c->stage_f.release(); c->stage_type.release(); c->stage_ev.release();
+    c->excl_off.release(); c->excl_idx.release(); c->ljtab.release();
+    c->col_count.release(); c->col_atom_off.release(); c->col_sc_off.release(); c->atom_col.release();
+    c->atom_rank.release(); c->col_atoms.release(); c->grid_totals.release(); c->image.release(); c->xw_atom.release();
+    c->xq.release(); c->type_slot.release(); c->atom_of_slot.release(); c->slot_of_atom.release();
+    c->bb_lo.release(); c->bb_hi.release(); c->sbb_lo.release(); c->sbb_hi.release(); c->f4.release();
+    c->ent_count.release(); c->ent_jbegin.release(); c->jl.release(); c->imask_outer.release();
+    c->plane_outer.release(); c->plane_inner.release(); c->batch_ent.release(); c->scan_tmp.release();
+    c->scan_blk.release(); c->excl_masks.release(); c->counters.release(); c->units_canon.release();
+    c->units_sorted.release(); c->fshift.release();
+    delete c;
+}
+
+extern "C" const char* nb_last_error(const nb_ctx* c) { return c ? c->err : "null context"; }
+
+extern "C" int nb_get_layout(nb_ctx* c, int32_t* cluster_size, int32_t* nclusters, int32_t* nsuper, int32_t* nslots)
+{
+    if (!c) return NB_ERR_ARG;
+    if (!c->have_grid) return nb_fail(c, NB_ERR_STATE, "no grid yet (call nb_search)");
+    if (cluster_size) *cluster_size = NB_C;
+    if (nclusters) *nclusters = c->nclusters;
+    if (nsuper) *nsuper = c->nsc;
+    if (nslots) *nslots = c->nslots;
+    return NB_OK;
+}
+
+extern "C" int nb_get_slots(nb_ctx* c, int32_t* atom_of_slot, float* xq)
+{
+    if (!c) return NB_ERR_ARG;
+    if (!c->have_grid) return nb_fail(c, NB_ERR_STATE, "no grid yet (call nb_search)");
+    if (atom_of_slot) NB_CUDA(c, cudaMemcpyAsync(atom_of_slot, c->atom_of_slot.p, sizeof(int32_t) * c->nslots, cudaMemcpyDeviceToDevice, c->stream));
+    if (xq) NB_CUDA(c, cudaMemcpyAsync(xq, c->xq.p, sizeof(float4) * c->nslots, cudaMemcpyDeviceToDevice, c->stream));
+    NB_CUDA(c, cudaStreamSynchronize(c->stream));
+    return NB_OK;
+}
+
+extern "C" int nb_list_count(nb_ctx* c, int which, int64_t* n)
+{
+    if (!c || !n) return NB_ERR_ARG;
+    if (which != 0 && which != 1) return nb_fail(c, NB_ERR_ARG, "which must be 0 (outer) or 1 (inner)");
+    if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "no list yet (call nb_search)");
+    return nbi_list_count(c, which, n);
+}
+
+extern "C" int nb_list_dump(nb_ctx* c, int which, int32_t* ci, int32_t* cj, int32_t* shift, uint64_t* pairmask, int32_t* part)
+{
+    if (!c) return NB_ERR_ARG;
+    if (which != 0 && which != 1) return nb_fail(c, NB_ERR_ARG, "which must be 0 (outer) or 1 (inner)");
+    if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "no list yet (call nb_search)");
+    return nbi_list_dump(c, which, ci, cj, shift, pairmask, part);
+}
+
+extern "C" int nb_get_stats(nb_ctx* c, nb_stats* out)
+{
+    if (!c || !out) return NB_ERR_ARG;
+    NB_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (c->have_list) {
+        int64_t n = 0;
+        int rc = nbi_list_count(c, 1, &n);
+        if (rc != NB_OK) return rc;
+        c->st.n_pairs_inner = n;
+        c->st.slots_last_forces = c->st.force_count ? n * 64 : 0;
+    }
+    *out = c->st;
+    return NB_OK;
+}
+
+extern "C" int nb_measure_fp32_peak(nb_ctx* c, double* fma_per_s)
+{
+    if (!c || !fma_per_s) return NB_ERR_ARG;
+    return nbi_measure_fp32_peak(c, fma_per_s);
+}

@@ -1,0 +1,352 @@
+// nb_grid.cu -- (a1) coordinate refresh and (a2) gridding + cluster sort.
+//
+// "The clusters and pair list are obtained during search using a regular grid in
+// x and y dimensions but binning the resulting z columns into cells with fixed number of
+// particles"; L131: super-clusters come from "a 2x2x2 cell grouping on the search grid".
+// The paper does this on the CPU; here it runs on the GPU (BASELINE.json north_star: one GPU,
+// no CPU fallback).  Readings A10/A11: column side ~ (64/rho)^(1/3); per column a
+// z-sort, 64-atom slabs, each split by y (2x32), x (2x16), z (2x8), ties by atom index; a
+// partly filled last slab fills its clusters in that order, real atoms first.
+#include "nb_internal.h"
+
+#include <math.h>
+
+namespace {
+
+__device__ __forceinline__ uint32_t float_orderable(float v)
+{
+    uint32_t u = __float_as_uint(v);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+
+// One thread per atom: wrap into the box (image fixed until the next search), column index,
+// rank inside the column (arrival order; the later sort makes the layout deterministic).
+__global__ void k_bin(int n, const float* __restrict__ x, const float* __restrict__ q, float3 box, int ncx,
+                      int ncy, float inv_cx, float inv_cy, char4* __restrict__ image,
+                      float4* __restrict__ xw_atom, int* __restrict__ atom_col, int* __restrict__ atom_rank,
+                      int* __restrict__ col_count)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float L[3] = {box.x, box.y, box.z};
+    float w[3];
+    int img[3];
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        float v = x[3 * i + k];
+        float kf = floorf(v / L[k]);
+        float t = __fmaf_rn(-kf, L[k], v);
+        if (t < 0.f) { kf -= 1.f; t = __fmaf_rn(-kf, L[k], v); }
+        else if (t >= L[k]) { kf += 1.f; t = __fmaf_rn(-kf, L[k], v); }
+        kf = fminf(fmaxf(kf, -127.f), 127.f);
+        w[k] = __fmaf_rn(-kf, L[k], v);
+        img[k] = (int)kf;
+    }
+    int cx = min(ncx - 1, max(0, (int)floorf(w[0] * inv_cx)));
+    int cy = min(ncy - 1, max(0, (int)floorf(w[1] * inv_cy)));
+    int col = cx * ncy + cy;
+    image[i] = make_char4((signed char)img[0], (signed char)img[1], (signed char)img[2], 0);
+    xw_atom[i] = make_float4(w[0], w[1], w[2], q[i]);
+    atom_col[i] = col;
+    atom_rank[i] = atomicAdd(&col_count[col], 1);
+}
+
+// Single block: exclusive scans over columns of the atom count and of the super-cluster count.
+__global__ void k_col_scan(int ncol, const int* __restrict__ col_count, int* __restrict__ col_atom_off,
+                           int* __restrict__ col_sc_off, int* __restrict__ totals)
+{
+    __shared__ int s_a[1024], s_s[1024];
+    __shared__ int carry_a, carry_s, maxc;
+    int t = threadIdx.x;
+    if (t == 0) { carry_a = 0; carry_s = 0; maxc = 0; }
+    __syncthreads();
+    for (int base = 0; base < ncol; base += 1024) {
+        int c = base + t;
+        int cnt = c < ncol ? col_count[c] : 0;
+        int nsc = (cnt + NB_SC_ATOMS - 1) / NB_SC_ATOMS;
+        s_a[t] = cnt;
+        s_s[t] = nsc;
+        atomicMax(&maxc, cnt);
+        __syncthreads();
+        for (int d = 1; d < 1024; d <<= 1) {
+            int va = t >= d ? s_a[t - d] : 0, vs = t >= d ? s_s[t - d] : 0;
+            __syncthreads();
+            s_a[t] += va;
+            s_s[t] += vs;
+            __syncthreads();
+        }
+        if (c < ncol) {
+            col_atom_off[c] = carry_a + s_a[t] - cnt;
+            col_sc_off[c] = carry_s + s_s[t] - nsc;
+        }
+        __syncthreads();
+        if (t == 1023) { carry_a += s_a[t]; carry_s += s_s[t]; }
+        __syncthreads();
+    }
+    if (t == 0) {
+        col_atom_off[ncol] = carry_a;
+        col_sc_off[ncol] = carry_s;
+        totals[0] = carry_s;
+        totals[1] = maxc;
+    }
+}
+
+__global__ void k_col_scatter(int n, const int* __restrict__ atom_col, const int* __restrict__ atom_rank,
+                              const int* __restrict__ col_atom_off, int* __restrict__ col_atoms)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    col_atoms[col_atom_off[atom_col[i]] + atom_rank[i]] = i;
+}
+
+struct SlabScratch {
+    float key[NB_SC_ATOMS];
+    int atom[NB_SC_ATOMS];
+    int atom2[NB_SC_ATOMS];
+};
+
+// Stable rank sort of the 64 entries of a slab inside segments of `seg` entries, by
+// (coordinate `comp`, atom index); invalid entries (atom == INT_MAX) sort last.
+__device__ __forceinline__ void slab_segment_sort(SlabScratch& s, const float4* __restrict__ xw_atom, int comp,
+                                                  int seg, int lane)
+{
+#pragma unroll
+    for (int h = 0; h < 2; h++) {
+        int e = lane + 32 * h;
+        int a = s.atom[e];
+        float4 v = a != INT_MAX ? xw_atom[a] : make_float4(INFINITY, INFINITY, INFINITY, 0.f);
+        s.key[e] = comp == 0 ? v.x : (comp == 1 ? v.y : v.z);
+    }
+    __syncwarp();
+#pragma unroll
+    for (int h = 0; h < 2; h++) {
+        int e = lane + 32 * h;
+        int s0 = (e / seg) * seg;
+        float k = s.key[e];
+        int a = s.atom[e];
+        int rank = 0;
+        for (int o = s0; o < s0 + seg; o++) {
+            float ko = s.key[o];
+            int ao = s.atom[o];
+            rank += (ko < k || (ko == k && (ao < a || (ao == a && o < e)))) ? 1 : 0;   // padding entries tie: keep order
+        }
+        s.atom2[s0 + rank] = a;
+    }
+    __syncwarp();
+#pragma unroll
+    for (int h = 0; h < 2; h++) s.atom[lane + 32 * h] = s.atom2[lane + 32 * h];
+    __syncwarp();
+}
+
+// One block per grid column: bitonic z-sort of the column in shared memory, then one warp per
+// 64-atom slab does the 2x2x2 sub-sorts and writes the cluster-ordered arrays and bounding boxes.
+__global__ void __launch_bounds__(256)
+k_col_layout(int ncy, const int* __restrict__ col_atom_off, const int* __restrict__ col_sc_off,
+             const int* __restrict__ col_atoms, const float4* __restrict__ xw_atom,
+             const int* __restrict__ type, int pad_type, int np2_max, float4* __restrict__ xq,
+             int* __restrict__ type_slot, int* __restrict__ atom_of_slot, int* __restrict__ slot_of_atom,
+             float4* __restrict__ bb_lo, float4* __restrict__ bb_hi, float4* __restrict__ sbb_lo,
+             float4* __restrict__ sbb_hi)
+{
+    extern __shared__ unsigned long long s_keys[];
+    __shared__ SlabScratch s_slab[8];
+    int col = blockIdx.x;
+    int a0 = col_atom_off[col], n = col_atom_off[col + 1] - a0;
+    if (n == 0) return;
+    int np2 = 1;
+    while (np2 < n) np2 <<= 1;
+    for (int i = threadIdx.x; i < np2; i += blockDim.x) {
+        unsigned long long k = ~0ull;
+        if (i < n) {
+            int a = col_atoms[a0 + i];
+            k = ((unsigned long long)float_orderable(xw_atom[a].z) << 32) | (unsigned)a;
+        }
+        s_keys[i] = k;
+    }
+    __syncthreads();
+    for (int k = 2; k <= np2; k <<= 1) {
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int i = threadIdx.x; i < np2; i += blockDim.x) {
+                int p = i ^ j;
+                if (p > i) {
+                    unsigned long long u = s_keys[i], v = s_keys[p];
+                    bool up = (i & k) == 0;
+                    if ((u > v) == up) { s_keys[i] = v; s_keys[p] = u; }
+                }
+            }
+            __syncthreads();
+        }
+    }
+    int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    int nslab = (n + NB_SC_ATOMS - 1) / NB_SC_ATOMS;
+    int sc0 = col_sc_off[col];
+    SlabScratch& s = s_slab[warp];
+    for (int slab = warp; slab < nslab; slab += 8) {
+#pragma unroll
+        for (int h = 0; h < 2; h++) {
+            int e = lane + 32 * h, idx = slab * NB_SC_ATOMS + e;
+            s.atom[e] = idx < n ? (int)(unsigned)(s_keys[idx] & 0xffffffffull) : INT_MAX;
+        }
+        __syncwarp();
+        slab_segment_sort(s, xw_atom, 1, 64, lane);   // y: 2 x 32
+        slab_segment_sort(s, xw_atom, 0, 32, lane);   // x: 2 x 16
+        slab_segment_sort(s, xw_atom, 2, 16, lane);   // z: 2 x 8 -> clusters of 8
+        int sc = sc0 + slab;
+        float slo[3] = {1e30f, 1e30f, 1e30f}, shi[3] = {-1e30f, -1e30f, -1e30f};
+#pragma unroll
+        for (int h = 0; h < 2; h++) {
+            int e = lane + 32 * h;
+            int slot = sc * NB_SC_ATOMS + e;
+            int a = s.atom[e];
+            bool real = a != INT_MAX;
+            float4 v;
+            if (real) {
+                v = xw_atom[a];
+                slot_of_atom[a] = slot;
+            } else {
+                // padding: far away, distinct per (slot, column); zero charge, zero-LJ type
+                int cx = col / ncy, cy = col % ncy;
+                v = make_float4(1.0e4f + 61.803f * (float)e, 1.0e4f + 61.803f * (float)cy,
+                                -1.0e4f - 61.803f * (float)cx, 0.f);
+            }
+            xq[slot] = v;
+            type_slot[slot] = real ? type[a] : pad_type;
+            atom_of_slot[slot] = real ? a : -1;
+            float lo[3] = {real ? v.x : 1e30f, real ? v.y : 1e30f, real ? v.z : 1e30f};
+            float hi[3] = {real ? v.x : -1e30f, real ? v.y : -1e30f, real ? v.z : -1e30f};
+            int cnt = real ? 1 : 0;
+#pragma unroll
+            for (int d = 1; d < 8; d <<= 1) {
+#pragma unroll
+                for (int k = 0; k < 3; k++) {
+                    lo[k] = fminf(lo[k], __shfl_xor_sync(0xffffffffu, lo[k], d));
+                    hi[k] = fmaxf(hi[k], __shfl_xor_sync(0xffffffffu, hi[k], d));
+                }
+                cnt += __shfl_xor_sync(0xffffffffu, cnt, d);
+            }
+            if ((lane & 7) == 0) {
+                int cl = sc * NB_SUPER_SIZE + (e >> 3);
+                bb_lo[cl] = make_float4(lo[0], lo[1], lo[2], (float)cnt);
+                bb_hi[cl] = make_float4(hi[0], hi[1], hi[2], 0.f);
+            }
+#pragma unroll
+            for (int k = 0; k < 3; k++) { slo[k] = fminf(slo[k], lo[k]); shi[k] = fmaxf(shi[k], hi[k]); }
+        }
+#pragma unroll
+        for (int d = 8; d < 32; d <<= 1) {
+#pragma unroll
+            for (int k = 0; k < 3; k++) {
+                slo[k] = fminf(slo[k], __shfl_xor_sync(0xffffffffu, slo[k], d));
+                shi[k] = fmaxf(shi[k], __shfl_xor_sync(0xffffffffu, shi[k], d));
+            }
+        }
+        if (lane == 0) {
+            sbb_lo[sc] = make_float4(slo[0], slo[1], slo[2], (float)col);
+            sbb_hi[sc] = make_float4(shi[0], shi[1], shi[2], 0.f);
+        }
+        __syncwarp();
+    }
+}
+
+// (a1) refresh of the cluster-ordered coordinates from caller-order x with the stored image.
+__global__ void k_refresh_xq(int n, const float* __restrict__ x, const float* __restrict__ q,
+                             const char4* __restrict__ image, const int* __restrict__ slot_of_atom, float3 box,
+                             float4* __restrict__ xq)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    char4 im = image[i];
+    float4 v;
+    v.x = __fmaf_rn(-(float)im.x, box.x, x[3 * i]);
+    v.y = __fmaf_rn(-(float)im.y, box.y, x[3 * i + 1]);
+    v.z = __fmaf_rn(-(float)im.z, box.z, x[3 * i + 2]);
+    v.w = q[i];
+    xq[slot_of_atom[i]] = v;
+}
+
+}  // namespace
+
+int nbi_refresh_xq(nb_ctx* c)
+{
+    int n = c->natoms;
+    k_refresh_xq<<<(n + 255) / 256, 256, 0, c->stream>>>(n, c->x.p, c->q.p, c->image.p, c->slot_of_atom.p,
+                                                         make_float3(c->box[0], c->box[1], c->box[2]), c->xq.p);
+    NB_LAUNCH_CHECK(c);
+    return NB_OK;
+}
+
+int nbi_grid(nb_ctx* c)
+{
+    const int n = c->natoms;
+    cudaStream_t st = c->stream;
+    const float* L = c->box;
+    // A10: column side ~ (64/rho)^(1/3) so that a super-cluster is roughly cubic.
+    double vol = (double)L[0] * L[1] * L[2];
+    double side = cbrt(NB_SC_ATOMS * vol / (double)n);
+    c->ncx = (int)fmax(1.0, floor(L[0] / side + 0.5));
+    c->ncy = (int)fmax(1.0, floor(L[1] / side + 0.5));
+    c->ncol = c->ncx * c->ncy;
+    c->inv_cx = (float)(c->ncx / (double)L[0]);
+    c->inv_cy = (float)(c->ncy / (double)L[1]);
+    NB_CUDA(c, c->col_count.ensure(c->ncol + 1, st));
+    NB_CUDA(c, c->col_atom_off.ensure(c->ncol + 1, st));
+    NB_CUDA(c, c->col_sc_off.ensure(c->ncol + 1, st));
+    NB_CUDA(c, c->atom_col.ensure(n, st));
+    NB_CUDA(c, c->atom_rank.ensure(n, st));
+    NB_CUDA(c, c->col_atoms.ensure(n, st));
+    NB_CUDA(c, c->image.ensure(n, st));
+    NB_CUDA(c, c->xw_atom.ensure(n, st));
+    NB_CUDA(c, c->slot_of_atom.ensure(n, st));
+    NB_CUDA(c, c->grid_totals.ensure(4, st));
+    NB_CUDA(c, cudaMemsetAsync(c->col_count.p, 0, sizeof(int) * (c->ncol + 1), st));
+    float3 box = make_float3(L[0], L[1], L[2]);
+    k_bin<<<(n + 255) / 256, 256, 0, st>>>(n, c->x.p, c->q.p, box, c->ncx, c->ncy, c->inv_cx, c->inv_cy,
+                                           c->image.p, c->xw_atom.p, c->atom_col.p, c->atom_rank.p,
+                                           c->col_count.p);
+    NB_LAUNCH_CHECK(c);
+    k_col_scan<<<1, 1024, 0, st>>>(c->ncol, c->col_count.p, c->col_atom_off.p, c->col_sc_off.p,
+                                   c->grid_totals.p);
+    NB_LAUNCH_CHECK(c);
+    k_col_scatter<<<(n + 255) / 256, 256, 0, st>>>(n, c->atom_col.p, c->atom_rank.p, c->col_atom_off.p,
+                                                   c->col_atoms.p);
+    NB_LAUNCH_CHECK(c);
+    int tot[2];
+    NB_CUDA(c, cudaMemcpyAsync(tot, c->grid_totals.p, sizeof(tot), cudaMemcpyDeviceToHost, st));
+    NB_CUDA(c, cudaStreamSynchronize(st));
+    c->nsc = tot[0];
+    c->max_col_count = tot[1];
+    c->nclusters = c->nsc * NB_SUPER_SIZE;
+    c->nslots = c->nsc * NB_SC_ATOMS;
+    int np2 = 1;
+    while (np2 < c->max_col_count) np2 <<= 1;
+    size_t smem = (size_t)np2 * sizeof(unsigned long long);
+    if (smem > 200 * 1024)
+        return nb_fail(c, NB_ERR_OVERFLOW, "grid column holds %d atoms; the in-shared-memory z-sort takes at most 25600",
+                       c->max_col_count);
+    NB_CUDA(c, c->xq.ensure(c->nslots, st));
+    NB_CUDA(c, c->type_slot.ensure(c->nslots, st));
+    NB_CUDA(c, c->atom_of_slot.ensure(c->nslots, st));
+    NB_CUDA(c, c->bb_lo.ensure(c->nclusters, st));
+    NB_CUDA(c, c->bb_hi.ensure(c->nclusters, st));
+    NB_CUDA(c, c->sbb_lo.ensure(c->nsc, st));
+    NB_CUDA(c, c->sbb_hi.ensure(c->nsc, st));
+    NB_CUDA(c, c->f4.ensure(c->nslots, st));
+    NB_CUDA(c, cudaMemsetAsync(c->f4.p, 0, sizeof(float4) * c->nslots, st));
+    NB_CUDA(c, cudaFuncSetAttribute(k_col_layout, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_col_layout<<<c->ncol, 256, smem, st>>>(c->ncy, c->col_atom_off.p, c->col_sc_off.p, c->col_atoms.p,
+                                             c->xw_atom.p, c->type.p, c->ntypes, np2, c->xq.p, c->type_slot.p,
+                                             c->atom_of_slot.p, c->slot_of_atom.p, c->bb_lo.p, c->bb_hi.p,
+                                             c->sbb_lo.p, c->sbb_hi.p);
+    NB_LAUNCH_CHECK(c);
+    c->grid_box[0] = L[0];
+    c->grid_box[1] = L[1];
+    c->grid_box[2] = L[2];
+    c->have_grid = true;
+    c->st.ncolumns_x = c->ncx;
+    c->st.ncolumns_y = c->ncy;
+    c->st.nsuper = c->nsc;
+    c->st.nclusters = c->nclusters;
+    c->st.nslots = c->nslots;
+    c->st.cluster_size = NB_C;
+    return NB_OK;
+}

@@ -1,0 +1,172 @@
+// nb_internal.h -- context and device data layout of the B200 cluster-pair library.
+// Not part of the public ABI (include/nb.h is).  Nothing here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <vector>
+
+#include "../../include/nb.h"
+
+#define NB_C NB_CLUSTER_SIZE          // atoms per cluster
+#define NB_SC_ATOMS 64                // atoms per super-cluster (8 clusters x 8 atoms)
+#define NB_NHALF 14                   // zero shift + 13 shifts with s >lex 0
+#define NB_BATCH 32                   // joint j entries per mask word (one ballot)
+#define NB_PAD_TYPE_ROW 1             // LJ table carries one extra all-zero type for padding atoms
+
+// One growable device array.
+template <typename T>
+struct DevBuf {
+    T* p = nullptr;
+    size_t cap = 0;
+    cudaError_t ensure(size_t n, cudaStream_t st, bool keep = false)
+    {
+        if (n <= cap) return cudaSuccess;
+        size_t ncap = n + n / 4 + 64;
+        T* np_ = nullptr;
+        cudaError_t e = cudaMalloc((void**)&np_, ncap * sizeof(T));
+        if (e != cudaSuccess) return e;
+        if (p) {
+            if (keep && cap) {
+                e = cudaMemcpyAsync(np_, p, cap * sizeof(T), cudaMemcpyDeviceToDevice, st);
+                if (e != cudaSuccess) return e;
+            }
+            cudaStreamSynchronize(st);
+            cudaFree(p);
+        }
+        p = np_;
+        cap = ncap;
+        return cudaSuccess;
+    }
+    void release()
+    {
+        if (p) cudaFree(p);
+        p = nullptr;
+        cap = 0;
+    }
+};
+
+// Parameters every kernel needs, passed by value.
+struct NbConst {
+    float box[3];
+    float rc2;            // rc^2
+    float epsfac;
+    float beta, beta2, beta3;
+    float ewald_shift;    // erfc(beta rc)/rc if potential-shift else 0
+    float two_krf, krf, crf;
+    float lj_sh6, lj_sh12;  // rc^-6, rc^-12 if potential-shift else 0
+    int ntypes1;          // ntypes + 1 (row length of the padded LJ table)
+};
+
+struct nb_ctx {
+    nb_params prm;
+    cudaStream_t stream = nullptr;
+    char err[512];
+    int natoms = 0, ntypes = 0;
+    NbConst kc;
+    float beta = 0.f;
+
+    // --- state machine ---
+    bool have_atoms = false, have_grid = false, have_list = false, atoms_since_search = false;
+    float box[3] = {0, 0, 0};
+    float grid_box[3] = {0, 0, 0};
+    float rlist_outer = 0.f;
+    int last_nparts = 1;
+
+    // --- caller-order copies (a1) ---
+    DevBuf<float> x, q;
+    DevBuf<int32_t> type;
+    DevBuf<float> stage_x, stage_q, stage_f;   // staging for the _host entry points
+    DevBuf<int32_t> stage_type;
+    DevBuf<double> stage_ev;
+
+    // --- topology ---
+    DevBuf<int32_t> excl_off, excl_idx;
+    int64_t nexcl = 0;
+    DevBuf<float2> ljtab;        // [(ntypes+1)^2] (6*c6, 12*c12); last row/column zero
+
+    // --- grid (a2) ---
+    int ncx = 0, ncy = 0, ncol = 0;
+    float inv_cx = 0.f, inv_cy = 0.f;          // columns per nm
+    DevBuf<int32_t> col_count, col_atom_off, col_sc_off, atom_col, atom_rank, col_atoms;
+    DevBuf<int32_t> grid_totals;               // [4]: nsc, max column count, ...
+    DevBuf<char4> image;                       // periodic image fixed at the last search
+    DevBuf<float4> xw_atom;                    // wrapped (x,y,z,q) in caller order, search scratch
+    int nsc = 0, nslots = 0, nclusters = 0, max_col_count = 0;
+    DevBuf<float4> xq;                         // [nslots] x,y,z,q   (cluster order)
+    DevBuf<int32_t> type_slot, atom_of_slot, slot_of_atom;
+    DevBuf<float4> bb_lo, bb_hi;               // per cluster; lo.w = number of real atoms
+    DevBuf<float4> sbb_lo, sbb_hi;             // per super-cluster
+    DevBuf<float4> f4;                         // [nslots] force accumulator (x,y,z,unused), kept zero between calls
+
+    // --- pair list (a3, a4) ---
+    int nent = 0;                              // nsc * NB_NHALF (super-cluster, shift) slots, some empty
+    DevBuf<int32_t> ent_count;                 // [nent] joint entries per slot
+    DevBuf<int32_t> ent_jbegin;                // [nent+1] first j slot (multiple of NB_BATCH)
+    std::vector<int32_t> h_ent_count, h_ent_jbegin;
+    int64_t njslots = 0, nbatch = 0;
+    DevBuf<int2> jl;                           // [njslots] {cj, exclusion mask ref (0 = none)}
+    DevBuf<uint8_t> imask_outer;               // [njslots] 8-bit interaction mask
+    DevBuf<uint32_t> plane_outer, plane_inner; // [nbatch*8] bit-planes of the masks, word = (batch, i-cluster)
+    DevBuf<int32_t> batch_ent;                 // [nbatch] owning (super-cluster, shift) slot
+    DevBuf<int32_t> scan_tmp, scan_blk;        // scratch for device scans
+    DevBuf<unsigned long long> excl_masks;     // [(nmask+1)*8*2] {interact, count} per (ref, i-cluster)
+    int64_t nmask = 0;
+    DevBuf<long long> counters;                // device counters (list statistics)
+
+    // --- work units (a5) ---
+    std::vector<int4> h_units;
+    DevBuf<int4> units_canon, units_sorted;    // {entry slot, batch begin, batch end, sci}
+    int nunits = 0;
+    DevBuf<double> fshift;                     // [27*3] per-shift i-force sums (virial)
+
+    nb_stats st;
+};
+
+// Half-set of shifts: index 0 is the zero shift, 1..13 are the shifts with s >lex 0 in
+// (sx,sy,sz) order (reading A14).  Decoded with nb_shift_vec().
+__host__ __device__ inline int nb_half_shift_id(int h)
+{
+    // ids = (sx+1) + 3*(sy+1) + 9*(sz+1)
+    const int ids[NB_NHALF] = {13, /* sx=+1: all (sy,sz) */ 2, 5, 8, 11, 14, 17, 20, 23, 26,
+                               /* sx=0, sy=+1 */ 7, 16, 25, /* sx=sy=0, sz=+1 */ 22};
+    return ids[h];
+}
+__host__ __device__ inline void nb_shift_vec(int id, int& sx, int& sy, int& sz)
+{
+    sx = id % 3 - 1;
+    sy = (id / 3) % 3 - 1;
+    sz = id / 9 - 1;
+}
+
+int nb_fail(nb_ctx* c, int code, const char* fmt, ...);
+
+#define NB_CUDA(c, expr)                                                                              \
+    do {                                                                                              \
+        cudaError_t e__ = (expr);                                                                     \
+        if (e__ != cudaSuccess)                                                                       \
+            return nb_fail((c), e__ == cudaErrorMemoryAllocation ? NB_ERR_NOMEM : NB_ERR_CUDA,        \
+                           "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__); \
+    } while (0)
+
+#define NB_LAUNCH_CHECK(c)                                                                            \
+    do {                                                                                              \
+        (c)->st.kernel_launches++;                                                                    \
+        NB_CUDA((c), cudaGetLastError());                                                             \
+    } while (0)
+
+// Stage implementations (one translation unit each).
+int nbi_grid(nb_ctx* c);                                   // (a2) nb_grid.cu
+int nbi_refresh_xq(nb_ctx* c);                             // (a1) nb_grid.cu
+int nbi_search(nb_ctx* c, float rlist);                    // (a3)-(a5) nb_list.cu
+int nbi_prune(nb_ctx* c, float rlist_inner, int part, int nparts);   // (a6) nb_prune.cu
+int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial);   // (a7)-(a8) nb_force.cu
+int nbi_list_count(nb_ctx* c, int which, int64_t* n);      // nb_list.cu
+int nbi_list_dump(nb_ctx* c, int which, int32_t* ci, int32_t* cj, int32_t* shift, uint64_t* pairmask,
+                  int32_t* part);
+int nbi_measure_fp32_peak(nb_ctx* c, double* fma_per_s);   // nb_force.cu
+int nbi_exclusive_scan(nb_ctx* c, const int32_t* in, int32_t* out, int64_t n, int32_t* total_dev);  // nb_list.cu

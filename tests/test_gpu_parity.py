@@ -1,0 +1,301 @@
+"""GPU parity tests (run on the B200 box with -m gpu): the CUDA path, driven through the C ABI,
+against the fp64 oracle on the same seeded inputs.  Tolerances are BASELINE.json's: lists and
+masks bit-exact as sets, relative RMS force error <= 1e-5, relative energy error <= 1e-5;
+virial: same bound on the Frobenius norm."""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2006_09167_b200 import workloads as W
+from tests import listcheck as LC
+from tests.gpu_util import Driver, oracle_forces, rel_rms
+
+pytestmark = pytest.mark.gpu
+
+TOL_F = 1e-5
+TOL_E = 1e-5
+
+
+@pytest.fixture(scope="module")
+def small_rect():
+    # rectangular box, two super-cluster columns per axis at most, rc close to L/2 in x
+    return W.small_water(150, 2.0, seed=21, rc=0.8, rlist_outer=0.9, rlist_inner=0.84, box_scale=(1.0, 1.1, 1.25))
+
+
+def check_layout(d, w):
+    lay = d.ctx.get_layout()
+    aos, xq = d.slots()
+    assert lay["cluster_size"] == 8 and lay["nslots"] == lay["nsuper"] * 64 == lay["nclusters"] * 8 == aos.size
+    real = aos[aos >= 0]
+    assert real.size == w.natoms and np.array_equal(np.sort(real), np.arange(w.natoms))   # T13: each atom once
+    # slot coordinates are the atom's coordinates up to whole box vectors; charges match
+    dx = xq[aos >= 0, :3].astype(np.float64) - w.x[real].astype(np.float64)
+    k = np.rint(dx / w.box)
+    assert np.abs(dx - k * w.box).max() < 2e-6
+    assert np.array_equal(xq[aos >= 0, 3], w.q[real])
+    # wrapped into the box (up to rounding)
+    assert (xq[aos >= 0, :3] > -1e-5).all() and (xq[aos >= 0, :3] < w.box + 1e-5).all()
+    # within a cluster real atoms come first; within a super-cluster partly-filled clusters come last
+    v = (aos >= 0).reshape(-1, 8)
+    assert (np.diff(v.astype(int), axis=1) <= 0).all()
+    cnt = v.sum(axis=1).reshape(-1, 8)
+    assert (np.diff(cnt, axis=1) <= 0).all()
+    # padding is small: fewer than 64 slots per grid column
+    st = d.ctx.get_stats()
+    assert (aos < 0).sum() < 64 * st["ncolumns_x"] * st["ncolumns_y"]
+    # super-clusters of a column are z-ordered slabs: find columns by xy cell and compare z ranges
+    z = np.where(aos >= 0, xq[:, 2], np.nan).reshape(-1, 64)
+    zmin, zmax = np.nanmin(z, axis=1), np.nanmax(z, axis=1)
+    same_col_next = cnt.sum(axis=1)[:-1] == 64   # a full slab is followed by a slab of the same column or a new column
+    cx = np.floor(np.nanmean(np.where(aos >= 0, xq[:, 0], np.nan).reshape(-1, 64), axis=1) * st["ncolumns_x"] / w.box[0])
+    cy = np.floor(np.nanmean(np.where(aos >= 0, xq[:, 1], np.nan).reshape(-1, 64), axis=1) * st["ncolumns_y"] / w.box[1])
+    samecol = (cx[1:] == cx[:-1]) & (cy[1:] == cy[:-1]) & same_col_next
+    assert (zmax[:-1][samecol] <= zmin[1:][samecol]).all()
+    return aos, xq
+
+
+def check_lists(d, w, rl_outer, rl_inner, c_range=None):
+    aos, xq = d.slots()
+    kw = {} if c_range is None else dict(c_begin=c_range[0], c_end=c_range[1])
+    ref = O.lists(aos, xq, w.box, rl_outer, rl_inner, w.excl_off, w.excl_idx, **kw)
+
+    def sel(ci, cj):
+        if c_range is None:
+            return np.ones(ci.shape, bool)
+        return ((ci >= c_range[0]) & (ci < c_range[1])) | ((cj >= c_range[0]) & (cj < c_range[1]))
+
+    for which, rkeys in ((0, ref.keys("outer")), (1, ref.keys("inner"))):
+        ci, cj, s, pm, part = d.dump(which)
+        assert ci.size == d.ctx.list_count(which)
+        ci2, cj2, s2, pm2 = LC.canonicalise(ci, cj, s, pm)
+        assert np.array_equal(ci2, ci) and np.array_equal(cj2, cj)   # the library stores the canonical half
+        keys = LC.triple_keys(ci2, cj2, s2)
+        assert np.unique(keys).size == keys.size, "duplicate cluster pair in the list"
+        m = sel(ci2, cj2)
+        got = np.sort(keys[m])
+        want = np.sort(rkeys)
+        assert got.size == want.size and np.array_equal(got, want), (which, got.size, want.size)
+        # pair masks, bit-exact
+        order_g = np.argsort(keys[m])
+        rk = ref.keys("outer") if which == 0 else ref.keys("inner")
+        rmask = ref.pairmask if which == 0 else ref.pairmask[ref.inner]
+        order_r = np.argsort(rk)
+        assert np.array_equal(pm2[m][order_g], rmask[order_r])
+    return ref
+
+
+def test_config0_layout_lists_forces(cfg0):
+    w = cfg0
+    d = Driver(w)
+    d.put()
+    d.ctx.search(w.rlist_outer)
+    check_layout(d, w)
+    # before any prune the inner list is the outer list
+    assert d.ctx.list_count(0) == d.ctx.list_count(1)
+    f_outer = d.forces()
+    d.ctx.prune(w.rlist_inner)
+    ref_l = check_lists(d, w, w.rlist_outer, w.rlist_inner)
+    aos, xq = d.slots()
+    # layout-independent completeness: every atom pair within rlist_inner is in a listed inner pair
+    ci, cj, s, _, _ = d.dump(1)
+    miss, n = LC.coverage_missing(aos, xq, w.box, w.rlist_inner - 1e-6, ci, cj, s)
+    assert miss == 0 and n > 50000
+    assert 0.4 < ref_l.inner.mean() < 0.95
+    ref = oracle_forces(w)
+    f = d.forces()
+    assert rel_rms(f, ref.f) <= TOL_F
+    assert rel_rms(f_outer, ref.f) <= TOL_F           # T10: pruning does not change the forces
+    assert rel_rms(f, f_outer) < 2e-6
+    frms = np.sqrt((ref.f**2).sum(1).mean())
+    assert np.linalg.norm(f.sum(0)) / (w.natoms * frms) < 1e-6   # T6 on the GPU
+    f2, e, vir = d.forces(energy=True, virial=True)
+    assert rel_rms(f2, ref.f) <= TOL_F
+    assert abs(e.sum() - ref.energy) / abs(ref.energy) <= TOL_E
+    assert abs(e[0] - ref.e_lj) <= TOL_E * abs(ref.energy) and abs(e[1] - ref.e_coul) <= TOL_E * abs(ref.energy)
+    assert np.linalg.norm(vir - ref.virial) / np.linalg.norm(ref.virial) <= TOL_E
+    # image brute force agrees too (T5 through the GPU)
+    img = oracle_forces(w, method="images")
+    assert rel_rms(f, img.f) <= TOL_F
+    st = d.ctx.get_stats()
+    assert st["n_pairs_inner"] == ref_l.inner.sum() and st["n_pairs_outer"] == ref_l.inner.size
+    assert st["slots_last_forces"] == 64 * st["n_pairs_inner"]
+    # mean number of set interaction-mask bits per joint entry: the paper's "approximately four of eight" (L135)
+    assert 2.5 < st["n_pairs_outer"] / st["n_joint_outer"] < 6.5
+
+
+@pytest.mark.parametrize("coulomb", ["ewald", "rf"])
+def test_small_rectangular_box(coulomb):
+    w = W.small_water(150, 2.0, seed=21, rc=0.8, rlist_outer=0.9, rlist_inner=0.84,
+                      box_scale=(1.0, 1.1, 1.25), coulomb=coulomb)
+    d = Driver(w)
+    d.put()
+    d.ctx.search(w.rlist_outer)
+    check_layout(d, w)
+    d.ctx.prune(w.rlist_inner)
+    check_lists(d, w, w.rlist_outer, w.rlist_inner)
+    ref = oracle_forces(w)
+    f, e, vir = d.forces(energy=True, virial=True)
+    assert rel_rms(f, ref.f) <= TOL_F
+    assert abs(e.sum() - ref.energy) / abs(ref.energy) <= TOL_E
+    assert np.linalg.norm(vir - ref.virial) / np.linalg.norm(ref.virial) <= TOL_E
+    assert rel_rms(d.forces(), ref.f) <= TOL_F
+
+
+def test_modifiers_none_and_finite_eps_rf(small_rect):
+    w = small_rect
+    from paper_2006_09167_b200 import nb
+    d = Driver(w, lj_modifier=nb.NB_MOD_NONE, coul_modifier=nb.NB_MOD_NONE)
+    d.put()
+    d.ctx.search(w.rlist_outer)
+    ref = oracle_forces(w, lj_shift=False, coul_shift=False)
+    f, e = d.forces(energy=True)
+    assert rel_rms(f, ref.f) <= TOL_F and abs(e.sum() - ref.energy) / abs(ref.energy) <= TOL_E
+    d2 = Driver(w, coulomb="rf", eps_rf=78.0)
+    d2.put()
+    d2.ctx.search(w.rlist_outer)
+    p = O.Params(rc=w.rc, ntypes=w.ntypes, coulomb="rf", eps_rf=78.0)
+    ref2 = O.forces(w.x, w.q, w.type, w.box, w.lj_c6c12, w.excl_off, w.excl_idx, p)
+    f, e = d2.forces(energy=True)
+    assert rel_rms(f, ref2.f) <= TOL_F and abs(e.sum() - ref2.energy) / abs(ref2.energy) <= TOL_E
+
+
+def test_exclusion_extremes(small_rect):
+    """T15 on the GPU: no exclusions, and a topology where everything within a molecule-sized
+    group of 24 atoms is excluded (dense masks)."""
+    w = small_rect
+    n = w.natoms
+    import copy
+    w0 = copy.copy(w)
+    w0.excl_off, w0.excl_idx = np.zeros(n + 1, np.int32), np.zeros(0, np.int32)
+    d = Driver(w0)
+    d.put()
+    d.ctx.search(w.rlist_outer)
+    d.ctx.prune(w.rlist_outer)
+    check_lists(d, w0, w.rlist_outer, w.rlist_outer)
+    ref = oracle_forces(w0)
+    f, e = d.forces(energy=True)
+    assert rel_rms(f, ref.f) <= TOL_F and abs(e.sum() - ref.energy) / abs(ref.energy) <= TOL_E
+    grp = np.arange(n) // 24
+    idx = [np.setdiff1d(np.nonzero(grp == grp[i])[0], [i]) for i in range(n)]
+    w1 = copy.copy(w)
+    w1.excl_off = np.concatenate([[0], np.cumsum([len(v) for v in idx])]).astype(np.int32)
+    w1.excl_idx = np.concatenate(idx).astype(np.int32)
+    d = Driver(w1)
+    d.put()
+    d.ctx.search(w.rlist_outer)
+    d.ctx.prune(w.rlist_outer)
+    check_lists(d, w1, w.rlist_outer, w.rlist_outer)
+    ref = oracle_forces(w1)
+    f, e = d.forces(energy=True)
+    assert rel_rms(f, ref.f) <= TOL_F and abs(e.sum() - ref.energy) / abs(ref.energy) <= TOL_E
+
+
+def test_translation_and_broken_molecules(cfg0):
+    """T7 on the GPU: whole-box translation and per-atom box-vector shifts leave f, E unchanged."""
+    w = cfg0
+    ref = oracle_forces(w)
+    rng = np.random.default_rng(9)
+    xs = [np.mod(w.x.astype(np.float64) + rng.uniform(-3, 3, 3), w.box).astype(np.float32),
+          (w.x + rng.integers(-2, 3, size=w.x.shape) * w.box).astype(np.float32)]
+    for x in xs:
+        d = Driver(w)
+        d.put(x)
+        d.ctx.search(w.rlist_outer)
+        f, e = d.forces(energy=True)
+        r = oracle_forces(w, x=x)
+        assert rel_rms(f, r.f) <= TOL_F
+        assert abs(e.sum() - ref.energy) / abs(ref.energy) <= 2 * TOL_E
+
+
+def test_config1_parity_and_rolling_prune(cfg1):
+    w = cfg1
+    d = Driver(w)
+    d.put()
+    d.ctx.search(w.rlist_outer)
+    check_layout(d, w)
+    ref = oracle_forces(w, method="cells")
+    # full-size list parity on a sample of clusters (the oracle's all-pairs bb loop is O(n^2))
+    ncl = d.ctx.get_layout()["nclusters"]
+    d.ctx.prune(w.rlist_inner)
+    for c0 in (0, ncl // 2 + 3, ncl - 24):
+        check_lists(d, w, w.rlist_outer, w.rlist_inner, c_range=(c0, c0 + 24))
+    f, e, vir = d.forces(energy=True, virial=True)
+    assert rel_rms(f, ref.f) <= TOL_F
+    assert abs(e.sum() - ref.energy) / abs(ref.energy) <= TOL_E
+    assert np.linalg.norm(vir - ref.virial) / np.linalg.norm(ref.virial) <= TOL_E
+    st = d.ctx.get_stats()
+    assert 3.5 < st["n_pairs_outer"] / st["n_joint_outer"] < 5.5      # P:L135 "approximately four of eight"
+    inner_full = st["n_pairs_inner"]
+    assert 0.5 < inner_full / st["n_pairs_outer"] < 0.8
+    # T11: pruning the k parts one after the other at fixed x == one full prune
+    full = d.dump(1)
+    d.ctx.search(w.rlist_outer)
+    for p in range(w.nparts):
+        d.ctx.prune(w.rlist_inner, p, w.nparts)
+    rolled = d.dump(1)
+    for a, b in zip(full[:4], rolled[:4]):
+        assert np.array_equal(a, b)
+    assert set(np.unique(rolled[4]).tolist()) == set(range(w.nparts))
+    # rolling over moving atoms (motion recipe): forces stay equal to the all-pairs oracle
+    for t in (1, 2, 50, 99):
+        x = w.positions_at(t)
+        d.put(x)
+        before = d.dump(1)
+        part = t % w.nparts
+        d.ctx.prune(w.rlist_inner, part, w.nparts)
+        after = d.dump(1)
+        # only entries of the pruned part may change
+        kb = LC.triple_keys(before[0], before[1], before[2])[before[4] != part]
+        ka = LC.triple_keys(after[0], after[1], after[2])[after[4] != part]
+        assert np.array_equal(kb, ka)
+        r = oracle_forces(w, x=x, method="cells")
+        assert rel_rms(d.forces(), r.f) <= TOL_F
+    # determinism (T16): same inputs, same dump
+    d.put()
+    d.ctx.search(w.rlist_outer)
+    d.ctx.prune(w.rlist_inner)
+    again = d.dump(1)
+    for a, b in zip(full[:4], again[:4]):
+        assert np.array_equal(a, b)
+
+
+def test_host_entry_points(cfg0):
+    w = cfg0
+    d = Driver(w)
+    d.ctx.put_atoms_host(w.x, w.q, w.type, w.box)
+    d.ctx.search(w.rlist_outer)
+    f = np.zeros((w.natoms, 3), np.float32)
+    e = np.zeros(2)
+    v = np.zeros(9)
+    d.ctx.forces_host(f, e, v)
+    ref = oracle_forces(w)
+    assert rel_rms(f.astype(np.float64), ref.f) <= TOL_F
+    assert abs(e.sum() - ref.energy) / abs(ref.energy) <= TOL_E
+
+
+def test_error_codes(cfg0):
+    from paper_2006_09167_b200 import nb
+    w = cfg0
+    d = Driver(w)
+    with pytest.raises(nb.NbError) as ei:
+        d.ctx.search(w.rlist_outer)
+    assert ei.value.code == -2   # NB_ERR_STATE: no atoms yet
+    d.put()
+    with pytest.raises(nb.NbError) as ei:
+        d.ctx.search(0.5)        # below rc
+    assert ei.value.code == -3
+    with pytest.raises(nb.NbError) as ei:
+        d.ctx.search(1.0)        # above L/2
+    assert ei.value.code == -3
+    with pytest.raises(nb.NbError) as ei:
+        d.ctx.forces(d.f)
+    assert ei.value.code == -2
+    d.ctx.search(w.rlist_outer)
+    with pytest.raises(nb.NbError) as ei:
+        d.ctx.prune(0.95)        # above rlist_outer
+    assert ei.value.code == -3
+    with pytest.raises(nb.NbError) as ei:
+        d.ctx.prune(w.rlist_inner, 2, 2)
+    assert ei.value.code == -1
+    with pytest.raises(nb.NbError):
+        nb.Context(10, np.zeros((1, 1, 2), np.float32), None, None, rc=-1.0)
