@@ -1,0 +1,407 @@
+#!/usr/bin/env python
+"""bench.py -- the cluster-pair short-range non-bonded step on B200 (BASELINE.json metric:
+"non-bonded pair interactions/s and force-step us at 1 B200; % FP32 peak").
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--coulomb ewald|rf]
+  python bench.py --impl reference ...      # the fp64 CPU oracle, as it stands, on the host cores
+
+One "step" is one MD step of the whole hot path on the synthetic water box, in the paper's
+schedule: every step stages new coordinates
+(nb_put_atoms) and computes forces (nb_forces); every nstlist-th step first rebuilds the grid and
+the outer pair list (nb_search) and prunes it fully; every other step prunes one rolling part of
+the outer list (nb_prune) before the forces.  So K = nstlist steps contain every row of SURVEY 8(a)
+in the proportions the method prescribes.  `value` = effective pair interactions (non-excluded
+atom pairs with r < rc, the paper's "effective" throughput, L167-L173) per second.
+
+N > 1 (torchrun): the path does not shard ("replicas only"): every rank runs an
+independent replica on its own GPU, no data-path collective; value = sum over ranks / max time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "effective non-bonded pair interactions/s (cluster-pair step: put_atoms+search/prune+forces)"
+UNIT = "pairs/s"
+# Algorithmic FP32 work of the force kernel per atom-pair slot (DESIGN.md "Roofline of the force
+# kernel"): FFMA = 2 flop, FADD/FMUL/compare/select = 1, MUFU = 1.
+FLOP_PER_SLOT = {"ewald": 60.0, "rf": 37.0}
+N_SM, FP32_LANES_PER_SM = 148, 128   # B200_PROFILING.md: 148 SMs; 128 FP32 lanes/SM (4 SMSP x 32)
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[k] (default 2: ~96k atoms)")
+    ap.add_argument("--coulomb", default="ewald", choices=["ewald", "rf"], help="config 2 only")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-flush", action="store_true", help="do not flush L2 between timed steps")
+    return ap.parse_args()
+
+
+def load_workload(args):
+    from paper_2006_09167_b200 import workloads
+    if args.config == 2:
+        return workloads.config2(args.coulomb)
+    return workloads.by_index(args.config)
+
+
+def workload_config(w, args, extra=None):
+    cfg = {"workload": f"BASELINE.json configs[{args.config}] {w.name}: {w.natoms} atoms, box "
+                       f"{float(w.box[0]):.4f}x{float(w.box[1]):.4f}x{float(w.box[2]):.4f} nm, {w.coulomb} rc={w.rc}, "
+                       f"rlist_outer={w.rlist_outer}, rlist_inner={w.rlist_inner}, nstlist={w.nstlist}, "
+                       f"rolling prune in {w.nparts} parts",
+           "natoms": w.natoms, "nstlist": w.nstlist, "nparts": w.nparts,
+           "parallelism": "replicas only (one independent box per GPU)"}
+    if extra:
+        cfg.update(extra)
+    return cfg
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.stop_flag = index, [], set(), False
+        self.max_mhz = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:   # NVML missing: report no clocks rather than fail the bench
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap"}
+        while not self.stop_flag:
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.02)
+
+    def result(self):
+        self.stop_flag = True
+        if self.nv is None or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": []}
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
+
+
+class Replica:
+    """One box on one GPU, driven through the Python binding of the C ABI."""
+
+    def __init__(self, w, device_index, flush):
+        import numpy as np
+        import torch
+        from paper_2006_09167_b200 import nb
+        self.torch, self.np, self.w = torch, np, w
+        self.dev = torch.device("cuda", device_index)
+        torch.cuda.set_device(self.dev)
+        self.ctx = nb.context_for(w, device=device_index)
+        nframes = w.nstlist
+        # coordinates of the motion recipe for one list lifetime, resident in HBM / pinned on the host
+        frames = np.stack([w.positions_at(t) for t in range(nframes)])
+        self.x_dev = torch.from_numpy(frames).to(self.dev)
+        self.x_host = torch.from_numpy(frames).pin_memory()
+        self.q_dev = torch.from_numpy(w.q).to(self.dev)
+        self.t_dev = torch.from_numpy(w.type).to(self.dev)
+        self.q_host = torch.from_numpy(w.q).pin_memory()
+        self.t_host = torch.from_numpy(w.type).pin_memory()
+        self.f_dev = torch.zeros((w.natoms, 3), dtype=torch.float32, device=self.dev)
+        self.e_dev = torch.zeros(2, dtype=torch.float64, device=self.dev)
+        self.v_dev = torch.zeros(9, dtype=torch.float64, device=self.dev)
+        self.f_host = torch.zeros((w.natoms, 3), dtype=torch.float32).pin_memory()
+        self.e_host = torch.zeros(2, dtype=torch.float64).pin_memory()
+        self.v_host = torch.zeros(9, dtype=torch.float64).pin_memory()
+        # L2 flush buffer: 256 MiB > 126 MB L2, written between timed steps (outside the events)
+        self.flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device=self.dev) if flush else None
+        self.pairs_at_frame = None
+        self.slots_at_frame = None
+
+    def step_device(self, t):
+        """Inputs already in HBM (the `value` leg)."""
+        w, c = self.w, self.ctx
+        fr = t % w.nstlist
+        c.put_atoms(self.x_dev[fr], self.q_dev, self.t_dev, w.box)
+        if fr == 0:
+            c.search(w.rlist_outer)
+            c.prune(w.rlist_inner, 0, 1)           # first use of a fresh list: full prune
+            c.forces(self.f_dev, self.e_dev, self.v_dev)   # energies + virial once per list lifetime
+        else:
+            c.prune(w.rlist_inner, fr % w.nparts, w.nparts)   # rolling part (L193)
+            c.forces(self.f_dev, None, None)
+
+    def step_host(self, t):
+        """Host buffers in, host buffers out (the `e2e` leg): copies inside the timed region."""
+        w, c = self.w, self.ctx
+        fr = t % w.nstlist
+        c.put_atoms_host(self.x_host[fr].numpy(), self.q_host.numpy(), self.t_host.numpy(), w.box)
+        if fr == 0:
+            c.search(w.rlist_outer)
+            c.prune(w.rlist_inner, 0, 1)
+            c.forces_host(self.f_host.numpy(), self.e_host.numpy(), self.v_host.numpy())
+        else:
+            c.prune(w.rlist_inner, fr % w.nparts, w.nparts)
+            c.forces_host(self.f_host.numpy(), None, None)
+
+    def flush(self):
+        if self.flush_buf is not None:
+            self.flush_buf.fill_(1)
+
+    def count_pass(self):
+        """Untimed pass over one list lifetime that records, per frame, the effective pair count and
+        the atom-pair slots the force kernel evaluates (both counted by the library's own kernels)."""
+        w = self.w
+        self.pairs_at_frame, self.slots_at_frame = [], []
+        for t in range(w.nstlist):
+            self.step_device(t)
+            n_int, _ = self.ctx.count_pairs()
+            self.pairs_at_frame.append(n_int)
+            self.slots_at_frame.append(64 * self.ctx.list_count(1))
+
+    def timed(self, step_fn, t0, nsteps):
+        """Times nsteps steps starting at schedule position t0 with one CUDA-event pair per step on
+        the stream the library launches on; returns (total ms, effective pairs, slots)."""
+        torch = self.torch
+        stream = torch.cuda.current_stream(self.dev)
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(nsteps)]
+        pairs = slots = 0
+        for i in range(nsteps):
+            self.flush()
+            ev[i][0].record(stream)
+            step_fn(t0 + i)
+            ev[i][1].record(stream)
+            fr = (t0 + i) % self.w.nstlist
+            pairs += self.pairs_at_frame[fr]
+            slots += self.slots_at_frame[fr]
+        torch.cuda.synchronize(self.dev)
+        return sum(a.elapsed_time(b) for a, b in ev), pairs, slots
+
+
+def cpu_baseline(w, budget_s=12.0):
+    """The oracle as it stands (fp64, linked cells, OpenMP over the host cores), timed on the same
+    workload: whole force+energy evaluations until ~budget_s of CPU work is spent."""
+    from oracle import oracle as O
+    beta = O.beta_from_rtol(w.rc, w.ewald_rtol) if w.coulomb == "ewald" else 0.0
+    p = O.Params(rc=w.rc, ntypes=w.ntypes, coulomb=w.coulomb, beta=beta)
+    reps, spent, npairs = 0, 0.0, 0
+    while reps < 2 or (spent < budget_s and reps < 50):
+        t0 = time.perf_counter()
+        r = O.forces(w.x, w.q, w.type, w.box, w.lj_c6c12, w.excl_off, w.excl_idx, p, method="cells")
+        spent += time.perf_counter() - t0
+        npairs += r.npairs
+        reps += 1
+    return {"value": npairs / spent, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+            "sample": f"{reps} full force+energy+virial evaluations of the same {w.natoms}-atom box by "
+                      f"oracle_forces_cells (fp64, linked cells), {spent:.1f} s of wall time",
+            "ms_per_eval": 1e3 * spent / reps}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same metric/unit.  Each step is one oracle
+    force evaluation of a water box made by the same recipe at the same density, sized so that the
+    whole --steps/--warmup run ends within a few minutes (a bounded sample of the workload)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from oracle import oracle as O
+    from paper_2006_09167_b200 import workloads
+    full = load_workload(args)
+    nsteps = args.steps + args.warmup
+    budget = 150.0
+    run = dict(rc=full.rc, rlist_outer=full.rlist_outer, rlist_inner=full.rlist_inner, nstlist=full.nstlist,
+               nparts=full.nparts, coulomb=full.coulomb)
+
+    def make(nside):
+        L = (nside ** 3 / workloads.MOLECULES_PER_NM3) ** (1.0 / 3.0)
+        return workloads._lattice_water(f"sample_{nside}", workloads.SEED_BASE + 100 + nside, nside, 0, L, **run)
+
+    def evaluate(w):
+        beta = O.beta_from_rtol(w.rc, w.ewald_rtol) if w.coulomb == "ewald" else 0.0
+        p = O.Params(rc=w.rc, ntypes=w.ntypes, coulomb=w.coulomb, beta=beta)
+        t0 = time.perf_counter()
+        r = O.forces(w.x, w.q, w.type, w.box, w.lj_c6c12, w.excl_off, w.excl_idx, p, method="cells")
+        return time.perf_counter() - t0, r.npairs
+
+    min_side = int(3.0 * full.rc * workloads.MOLECULES_PER_NM3 ** (1.0 / 3.0)) + 2   # >= 3 cells of rc per axis
+    probe = make(min_side)
+    evaluate(probe)
+    dt, _ = evaluate(probe)
+    per_mol = dt / min_side ** 3
+    nside = min_side
+    full_side = round((full.natoms / 3) ** (1.0 / 3.0))
+    while nside + 1 <= full_side and per_mol * (nside + 1) ** 3 * nsteps <= budget:
+        nside += 1
+    w = probe if nside == min_side else make(nside)
+    for _ in range(args.warmup):
+        evaluate(w)
+    spent, npairs = 0.0, 0
+    for _ in range(args.steps):
+        dt, n = evaluate(w)
+        spent += dt
+        npairs += n
+    value = npairs / spent
+    sample = (f"each step = one oracle_forces_cells evaluation (fp64, force+energy+virial) of a {w.natoms}-atom "
+              f"water box, same recipe/density/cut-offs as the workload ({full.natoms} atoms)")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * spent / max(args.steps, 1),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(full, args, {"reference_sample_atoms": w.natoms}),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def run_b200(args):
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the non-bonded path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dev = torch.device("cuda", local_rank)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def max_over_ranks(v):
+        if world == 1:
+            return v
+        t = torch.tensor([v], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def sum_over_ranks(v):
+        if world == 1:
+            return v
+        t = torch.tensor([v], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return float(t.item())
+
+    w = load_workload(args)
+    rep = Replica(w, local_rank, flush=not args.no_flush)
+    ctx = rep.ctx
+    fma_peak = ctx.measure_fp32_peak()          # lane-FMA/s of a register-resident FFMA chain, this GPU, now
+    rep.count_pass()                            # untimed: per-frame pair and slot counts (also warms everything up)
+    W = max(args.warmup, 3)
+    K = args.steps
+
+    # ---------------- device-resident leg: `value` ----------------
+    for i in range(W):
+        rep.step_device(i)
+    ctx.timing_enable(True)
+    ctx.timing_read(reset=True)
+    launches0 = ctx.get_stats()["kernel_launches"]
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    ms, pairs, slots = rep.timed(rep.step_device, W, K)
+    barrier()
+    clocks = sampler.result()
+    stages = ctx.timing_read(reset=True)
+    ctx.timing_enable(False)
+    launches = ctx.get_stats()["kernel_launches"] - launches0 - 1   # get_stats itself launches one counting kernel
+    ms_max = max_over_ranks(ms)
+    pairs_all = sum_over_ranks(float(pairs))
+    value = pairs_all / (ms_max * 1e-3)
+
+    # ---------------- host-buffer leg: `e2e` ----------------
+    e2e = None
+    if not args.no_e2e:
+        for i in range(W):
+            rep.step_host(i)
+        barrier()
+        ms_h, pairs_h, _ = rep.timed(rep.step_host, W, K)
+        barrier()
+        ms_h_max = max_over_ranks(ms_h)
+        n = w.natoms
+        n_energy_steps = sum(1 for i in range(W, W + K) if i % w.nstlist == 0)
+        e2e = {"value": sum_over_ranks(float(pairs_h)) / (ms_h_max * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": n * (12 + 4 + 4),
+               "d2h_bytes_per_step": n * 12 + (11 * 8 * n_energy_steps) / max(K, 1),
+               "ms_per_step": ms_h_max / max(K, 1)}
+
+    # ---------------- roofline of the dominant kernel (force kernel, FP32 ALU bound) ----------------
+    f_ms, f_n = stages["force"]
+    sm_max = clocks["sm_max_mhz"] or 1965
+    peak_tflops = N_SM * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    flop_slot = FLOP_PER_SLOT[w.coulomb]
+    slots_per_launch = slots / max(K, 1)
+    force_us = 1e3 * f_ms / max(f_n, 1)
+    achieved = flop_slot * slots_per_launch / (force_us * 1e-6) / 1e12 if f_n else 0.0
+    roofline = {"bound": "alu", "kernel": "k_force (a7)", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+                "frac": achieved / peak_tflops, "traffic": None,
+                "peak_source": f"derived: {N_SM} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x {sm_max} MHz (clocks.max.sm); "
+                               "MEASURED_PEAKS.json has no FP32 entry",
+                "measured_ffma_chain_tflops": 2 * fma_peak / 1e12,
+                "frac_of_measured_ffma_chain": achieved / (2 * fma_peak / 1e12),
+                "flop_per_slot": flop_slot, "slots_per_launch": slots_per_launch, "kernel_us": force_us}
+
+    if rank == 0:
+        st = ctx.get_stats()
+        per_stage_us = {k: (1e3 * v[0] / v[1] if v[1] else None) for k, v in stages.items()}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+                "ms_per_step": ms_max / max(K, 1), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32", "data": "synthetic",
+                "config": workload_config(w, args, {"l2": "flushed between timed steps (256 MiB fill)" if not args.no_flush
+                                                    else "not flushed"}),
+                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+                "raw_pairs_per_s_per_gpu": slots / (ms * 1e-3),
+                "work_efficiency": pairs / max(slots, 1),
+                "stage_us": per_stage_us,
+                "stage_share_of_step": {k: v[0] / ms for k, v in stages.items()},
+                "list": {k: st[k] for k in ("nsuper", "n_sci_entries", "n_joint_outer", "n_pairs_outer", "n_pairs_inner",
+                                            "n_excl_masks", "n_work_units")}}
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(w)
+        print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_b200(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

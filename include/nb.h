@@ -138,6 +138,28 @@ int nb_get_stats(nb_ctx*, nb_stats* out);
 /* Measures the device's FP32 FMA issue peak with a register-resident FFMA chain kernel
  * (MEASURED_PEAKS.json has no FP32 entry).  Returns lane-FMA/s in *fma_per_s. */
 int nb_measure_fp32_peak(nb_ctx*, double* fma_per_s);
+/* Counts, over the current inner list and coordinates, the atom pairs with r^2 < rc^2 that
+ * interact (*n_interacting: the paper's "effective" pair count) and those
+ * that are force-field exclusions (*n_excluded; they contribute only the Ewald/RF correction).
+ * Host outputs; either may be NULL.  Synchronises. */
+int nb_count_pairs(nb_ctx*, int64_t* n_interacting, int64_t* n_excluded);
+
+/* Per-stage device timing with CUDA events on the context's stream ("CUDA events
+ * on the caller's stream").  Stage ids index the arrays of nb_timing_read. */
+enum { NB_T_PUT = 0,      /* (a1) nb_put_atoms: copies + cluster-order refresh */
+       NB_T_GRID = 1,     /* (a2) gridding + cluster sort */
+       NB_T_SEARCH = 2,   /* (a3)+(a5) pair search count/fill passes, unit table upload */
+       NB_T_MASKS = 3,    /* (a4) exclusion masks (+ list statistics) */
+       NB_T_PRUNE = 4,    /* (a6) prune kernel */
+       NB_T_FORCE = 5,    /* (a7) force kernel alone */
+       NB_T_REDUCE = 6,   /* (a8) gather to caller order, virial/energy finalisation */
+       NB_T_NKINDS = 7 };
+/* on != 0: record an event pair around every stage from now on.  Off by default. */
+int nb_timing_enable(nb_ctx*, int on);
+/* Synchronises the stream, then returns the accumulated milliseconds and number of timed
+ * intervals per stage (host arrays of NB_T_NKINDS; either may be NULL); reset != 0 zeroes
+ * the accumulators afterwards. */
+int nb_timing_read(nb_ctx*, double* ms, int64_t* count, int reset);
 
 #ifdef __cplusplus
 }

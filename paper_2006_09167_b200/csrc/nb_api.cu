@@ -113,6 +113,7 @@ static int put_atoms_common(nb_ctx* c, const float* x, const float* q, const int
         if (!finite_pos(box[k])) return nb_fail(c, NB_ERR_BOX, "box[%d] = %g is not positive", k, box[k]);
     cudaStream_t st = c->stream;
     const int n = c->natoms;
+    NbStageTimer tm(c, NB_T_PUT);
     NB_CUDA(c, cudaMemcpyAsync(c->x.p, x, sizeof(float) * 3 * n, kind, st));
     NB_CUDA(c, cudaMemcpyAsync(c->q.p, q, sizeof(float) * n, kind, st));
     NB_CUDA(c, cudaMemcpyAsync(c->type.p, type, sizeof(int32_t) * n, kind, st));
@@ -190,6 +191,8 @@ extern "C" void nb_free(nb_ctx* c)
 {
     if (!c) return;
     cudaStreamSynchronize(c->stream);
+    for (auto& r : c->tim_open) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
+    for (auto e : c->tim_pool) cudaEventDestroy(e);
     c->x.release(); c->q.release(); c->type.release();
     c->stage_x.release(); c->stage_q.release(); c->stage_f.release(); c->stage_type.release(); c->stage_ev.release();
     c->excl_off.release(); c->excl_idx.release(); c->ljtab.release();
@@ -262,4 +265,39 @@ extern "C" int nb_measure_fp32_peak(nb_ctx* c, double* fma_per_s)
 {
     if (!c || !fma_per_s) return NB_ERR_ARG;
     return nbi_measure_fp32_peak(c, fma_per_s);
+}
+
+extern "C" int nb_count_pairs(nb_ctx* c, int64_t* n_interacting, int64_t* n_excluded)
+{
+    if (!c) return NB_ERR_ARG;
+    if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "no list yet (call nb_search)");
+    return nbi_count_pairs(c, n_interacting, n_excluded);
+}
+
+extern "C" int nb_timing_enable(nb_ctx* c, int on)
+{
+    if (!c) return NB_ERR_ARG;
+    c->timing = on != 0;
+    return NB_OK;
+}
+
+extern "C" int nb_timing_read(nb_ctx* c, double* ms, int64_t* count, int reset)
+{
+    if (!c) return NB_ERR_ARG;
+    NB_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (auto& r : c->tim_open) {
+        float t = 0.f;
+        NB_CUDA(c, cudaEventElapsedTime(&t, r.e0, r.e1));
+        c->tim_ms[r.kind] += t;
+        c->tim_n[r.kind]++;
+        c->tim_pool.push_back(r.e0);
+        c->tim_pool.push_back(r.e1);
+    }
+    c->tim_open.clear();
+    for (int k = 0; k < NB_T_NKINDS; k++) {
+        if (ms) ms[k] = c->tim_ms[k];
+        if (count) count[k] = c->tim_n[k];
+        if (reset) { c->tim_ms[k] = 0.0; c->tim_n[k] = 0; }
+    }
+    return NB_OK;
 }

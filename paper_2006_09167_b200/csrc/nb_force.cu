@@ -318,6 +318,61 @@ __global__ void __launch_bounds__(256) k_fp32_peak(float* out, int iters, float 
     out[blockIdx.x * blockDim.x + threadIdx.x] = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
 }
 
+// Counts atom pairs with r^2 < rc^2 over the inner list: interacting ("effective" pairs,
+// PAPER.md L167-L173) and excluded-but-counted.  Same block/warp/lane mapping as the prune kernel.
+__global__ void __launch_bounds__(256) k_count_pairs(ForceArgs A, unsigned long long* __restrict__ out)
+{
+    const int4 u = A.units[blockIdx.x];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7;
+    const int sci = u.w, h = u.x - sci * NB_NHALF, ci = sci * 8 + warp;
+    int sx, sy, sz;
+    nb_shift_vec(nb_half_shift_id(h), sx, sy, sz);
+    float xi[8], yi[8], zi[8];
+#pragma unroll
+    for (int a = 0; a < 8; a++) {
+        const float4 v = A.xq[ci * 8 + a];
+        xi[a] = fmaf((float)sx, A.kc.box[0], v.x);
+        yi[a] = fmaf((float)sy, A.kc.box[1], v.y);
+        zi[a] = fmaf((float)sz, A.kc.box[2], v.z);
+    }
+    unsigned n_int = 0, n_exc = 0;
+    for (int b = u.y; b < u.z; b++) {
+        unsigned bits = A.plane[(size_t)b * 8 + warp];
+        while (bits) {
+            int my = -1;
+#pragma unroll
+            for (int t = 0; t < 4; t++) {
+                const int p = bits ? __ffs(bits) - 1 : -1;
+                bits &= bits - 1;
+                if (t == g) my = p;
+            }
+            if (my < 0) continue;
+            const int2 ce = A.jl[(size_t)b * 32 + my];
+            const float4 xj = A.xq[ce.x * 8 + k];
+            const ulonglong2 mm = *reinterpret_cast<const ulonglong2*>(&A.masks[((size_t)ce.y * 8 + warp) * 2]);
+            const unsigned cbyte = (unsigned)(mm.y >> (8 * k)) & 0xffu, mbyte = (unsigned)(mm.x >> (8 * k)) & cbyte;
+#pragma unroll
+            for (int a = 0; a < 8; a++) {
+                const float dx = xi[a] - xj.x, dy = yi[a] - xj.y, dz = zi[a] - xj.z;
+                const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                if (r2 < A.kc.rc2) {
+                    n_int += (mbyte >> a) & 1u;
+                    n_exc += ((cbyte & ~mbyte) >> a) & 1u;
+                }
+            }
+        }
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        n_int += __shfl_xor_sync(0xffffffffu, n_int, d);
+        n_exc += __shfl_xor_sync(0xffffffffu, n_exc, d);
+    }
+    if (lane == 0) {
+        if (n_int) atomicAdd(&out[0], (unsigned long long)n_int);
+        if (n_exc) atomicAdd(&out[1], (unsigned long long)n_exc);
+    }
+}
+
 template <int COUL, bool ENERGY>
 int launch_force(nb_ctx* c, const ForceArgs& A)
 {
@@ -358,6 +413,7 @@ int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial)
     }
     int rc = NB_OK;
     if (c->nunits > 0) {
+        NbStageTimer tm(c, NB_T_FORCE);
         if (c->prm.coulomb == NB_COUL_EWALD)
             rc = energy ? launch_force<NB_COUL_EWALD, true>(c, A) : launch_force<NB_COUL_EWALD, false>(c, A);
         else
@@ -366,6 +422,7 @@ int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial)
     }
     double* xf = c->fshift.p + NB_NSHIFT * 3;
     const int nb = (c->nslots + 255) / 256;
+    NbStageTimer tm(c, NB_T_REDUCE);
     if (virial)
         k_gather<true><<<nb, 256, 0, st>>>(c->nslots, c->f4.p, c->atom_of_slot.p, c->xq.p, f, xf);
     else
@@ -403,5 +460,31 @@ int nbi_measure_fp32_peak(nb_ctx* c, double* fma_per_s)
     cudaEventDestroy(e1);
     out.release();
     *fma_per_s = (double)grid * 256 * iters * 64.0 / (best * 1e-3);
+    return NB_OK;
+}
+
+int nbi_count_pairs(nb_ctx* c, int64_t* n_interacting, int64_t* n_excluded)
+{
+    cudaStream_t st = c->stream;
+    ForceArgs A;
+    memset(&A, 0, sizeof(A));
+    A.units = c->units_canon.p;
+    A.jl = c->jl.p;
+    A.plane = c->plane_inner.p;
+    A.xq = c->xq.p;
+    A.masks = c->excl_masks.p;
+    A.kc = c->kc;
+    for (int k = 0; k < 3; k++) A.kc.box[k] = c->box[k];
+    NB_CUDA(c, c->counters.ensure(8, st));
+    NB_CUDA(c, cudaMemsetAsync(c->counters.p, 0, 8 * sizeof(long long), st));
+    if (c->nunits > 0) {
+        k_count_pairs<<<c->nunits, 256, 0, st>>>(A, (unsigned long long*)c->counters.p);
+        NB_LAUNCH_CHECK(c);
+    }
+    long long v[2] = {0, 0};
+    NB_CUDA(c, cudaMemcpyAsync(v, c->counters.p, sizeof(v), cudaMemcpyDeviceToHost, st));
+    NB_CUDA(c, cudaStreamSynchronize(st));
+    if (n_interacting) *n_interacting = v[0];
+    if (n_excluded) *n_excluded = v[1];
     return NB_OK;
 }

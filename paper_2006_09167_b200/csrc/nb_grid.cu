@@ -280,6 +280,7 @@ int nbi_grid(nb_ctx* c)
     const int n = c->natoms;
     cudaStream_t st = c->stream;
     const float* L = c->box;
+    NbStageTimer tm(c, NB_T_GRID);
     // A10: column side ~ (64/rho)^(1/3) so that a super-cluster is roughly cubic.
     double vol = (double)L[0] * L[1] * L[2];
     double side = cbrt(NB_SC_ATOMS * vol / (double)n);

@@ -124,7 +124,43 @@ struct nb_ctx {
     int nunits = 0;
     DevBuf<double> fshift;                     // [27*3] per-shift i-force sums (virial)
 
+    // --- per-stage device timing (nb_timing_enable / nb_timing_read) ---
+    bool timing = false;
+    struct TimRec { int kind; cudaEvent_t e0, e1; };
+    std::vector<TimRec> tim_open;              // recorded, not yet read
+    std::vector<cudaEvent_t> tim_pool;         // recycled events
+    double tim_ms[NB_T_NKINDS] = {0};
+    int64_t tim_n[NB_T_NKINDS] = {0};
+
     nb_stats st;
+};
+
+// RAII stage timer: CUDA events on the context's stream around the launches of one stage.
+// Costs nothing unless nb_timing_enable(ctx, 1) was called.
+struct NbStageTimer {
+    nb_ctx* c;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int kind;
+    static cudaEvent_t get(nb_ctx* c)
+    {
+        if (!c->tim_pool.empty()) { cudaEvent_t e = c->tim_pool.back(); c->tim_pool.pop_back(); return e; }
+        cudaEvent_t e = nullptr;
+        cudaEventCreate(&e);
+        return e;
+    }
+    NbStageTimer(nb_ctx* c_, int kind_) : c(c_), kind(kind_)
+    {
+        if (!c->timing) return;
+        e0 = get(c);
+        e1 = get(c);
+        cudaEventRecord(e0, c->stream);
+    }
+    ~NbStageTimer()
+    {
+        if (!e0) return;
+        cudaEventRecord(e1, c->stream);
+        c->tim_open.push_back({kind, e0, e1});
+    }
 };
 
 // Half-set of shifts: index 0 is the zero shift, 1..13 are the shifts with s >lex 0 in
@@ -169,4 +205,5 @@ int nbi_list_count(nb_ctx* c, int which, int64_t* n);      // nb_list.cu
 int nbi_list_dump(nb_ctx* c, int which, int32_t* ci, int32_t* cj, int32_t* shift, uint64_t* pairmask,
                   int32_t* part);
 int nbi_measure_fp32_peak(nb_ctx* c, double* fma_per_s);   // nb_force.cu
+int nbi_count_pairs(nb_ctx* c, int64_t* n_interacting, int64_t* n_excluded);   // nb_force.cu
 int nbi_exclusive_scan(nb_ctx* c, const int32_t* in, int32_t* out, int64_t n, int32_t* total_dev);  // nb_list.cu

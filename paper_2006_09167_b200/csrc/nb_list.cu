@@ -422,6 +422,8 @@ int nbi_search(nb_ctx* c, float rlist)
     int rc = nbi_grid(c);
     if (rc != NB_OK) return rc;
     const int nsc = c->nsc;
+    NbStageTimer* tm = new NbStageTimer(c, NB_T_SEARCH);
+    struct TmGuard { NbStageTimer*& t; ~TmGuard() { delete t; } } tm_guard{tm};
     c->nent = nsc * NB_NHALF;
     NB_CUDA(c, c->ent_count.ensure(c->nent + 1, st));
     NB_CUDA(c, c->ent_jbegin.ensure(c->nent + 1, st));
@@ -512,6 +514,8 @@ int nbi_search(nb_ctx* c, float rlist)
     }
 
     // (a4) exclusion masks
+    delete tm;
+    tm = new NbStageTimer(c, NB_T_MASKS);
     ExclArgs E;
     E.natoms = c->natoms; E.excl_off = c->excl_off.p; E.excl_idx = c->excl_idx.p; E.slot_of_atom = c->slot_of_atom.p;
     E.ent_count = c->ent_count.p; E.ent_jbegin = c->ent_jbegin.p; E.jl = c->jl.p; E.imask = c->imask_outer.p;

@@ -90,6 +90,7 @@ int nbi_prune(nb_ctx* c, float rlist_inner, int part, int nparts)
     A.xq = c->xq.p;
     for (int k = 0; k < 3; k++) A.box[k] = c->box[k];
     A.rl2 = rlist_inner * rlist_inner;
+    NbStageTimer tm(c, NB_T_PRUNE);
     k_prune<<<u1 - u0, 256, 0, c->stream>>>(A);
     NB_LAUNCH_CHECK(c);
     return NB_OK;

@@ -23,7 +23,9 @@ NB_SHIFT_CENTER = 13
 
 EXPORTS = ["nb_init", "nb_put_atoms", "nb_put_atoms_host", "nb_search", "nb_prune", "nb_forces",
            "nb_forces_host", "nb_free", "nb_last_error", "nb_get_layout", "nb_get_slots", "nb_list_count",
-           "nb_list_dump", "nb_get_stats", "nb_measure_fp32_peak"]
+           "nb_list_dump", "nb_get_stats", "nb_measure_fp32_peak", "nb_count_pairs", "nb_timing_enable",
+           "nb_timing_read"]
+NB_T_NAMES = ["put", "grid", "search", "masks", "prune", "force", "reduce"]
 
 
 class nb_params(C.Structure):
@@ -181,6 +183,23 @@ class Context:
         v = C.c_double()
         self._check(lib().nb_measure_fp32_peak(self._h, C.byref(v)))
         return v.value
+
+
+    def count_pairs(self):
+        """(interacting, excluded) atom pairs with r < rc over the inner list."""
+        a, b = C.c_int64(), C.c_int64()
+        self._check(lib().nb_count_pairs(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
+
+    def timing_enable(self, on=True):
+        self._check(lib().nb_timing_enable(self._h, C.c_int(int(on))))
+
+    def timing_read(self, reset=True):
+        """{stage: (milliseconds, intervals)} accumulated since the last reset."""
+        ms = (C.c_double * len(NB_T_NAMES))()
+        cnt = (C.c_int64 * len(NB_T_NAMES))()
+        self._check(lib().nb_timing_read(self._h, ms, cnt, C.c_int(int(reset))))
+        return {k: (ms[i], cnt[i]) for i, k in enumerate(NB_T_NAMES)}
 
 
 def shift_vectors(shift_id):

@@ -299,3 +299,30 @@ def test_error_codes(cfg0):
     assert ei.value.code == -1
     with pytest.raises(nb.NbError):
         nb.Context(10, np.zeros((1, 1, 2), np.float32), None, None, rc=-1.0)
+
+
+def test_pair_count_and_stage_timing(cfg0):
+    """nb_count_pairs equals the oracle's count of pairs within rc (a handful of pairs may sit within
+    fp32 rounding of rc); nb_timing_* reports one interval per stage call."""
+    w = cfg0
+    d = Driver(w)
+    d.ctx.timing_enable(True)
+    d.put()
+    d.ctx.search(w.rlist_outer)
+    d.put()
+    d.ctx.prune(w.rlist_inner)
+    ref = oracle_forces(w)
+    n_int, n_exc = d.ctx.count_pairs()
+    assert abs(n_int - ref.npairs) <= 2 and ref.npairs > 90000
+    assert abs(n_exc - ref.npairs_excl) <= 0 and n_exc == 3 * (w.natoms // 3)
+    d.forces()
+    d.forces(energy=True, virial=True)
+    t = d.ctx.timing_read()
+    assert t["put"][1] == 2 and t["grid"][1] == 1 and t["search"][1] == 1 and t["masks"][1] == 1
+    assert t["prune"][1] == 1 and t["force"][1] == 2 and t["reduce"][1] == 2
+    assert all(v[0] > 0 for v in t.values())
+    t2 = d.ctx.timing_read()
+    assert all(v == (0.0, 0) for v in t2.values())
+    d.ctx.timing_enable(False)
+    d.forces()
+    assert d.ctx.timing_read()["force"][1] == 0
