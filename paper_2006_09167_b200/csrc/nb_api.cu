@@ -201,7 +201,7 @@ extern "C" void nb_free(nb_ctx* c)
     c->xq.release(); c->type_slot.release(); c->atom_of_slot.release(); c->slot_of_atom.release();
     c->bb_lo.release(); c->bb_hi.release(); c->sbb_lo.release(); c->sbb_hi.release(); c->f4.release();
     c->ent_count.release(); c->ent_jbegin.release(); c->jl.release(); c->imask_outer.release();
-    c->plane_outer.release(); c->plane_inner.release(); c->batch_ent.release(); c->scan_tmp.release();
+    c->plane_outer.release(); c->plane_inner.release(); c->plane_excl.release(); c->batch_ent.release(); c->scan_tmp.release();
     c->scan_blk.release(); c->excl_masks.release(); c->counters.release(); c->units_canon.release();
     c->units_sorted.release(); c->fshift.release();
     delete c;

@@ -25,6 +25,7 @@ struct ForceArgs {
     const int4* units;
     const int2* jl;
     const uint32_t* plane;
+    const uint32_t* plane_excl;
     const float4* xq;
     const int* type_slot;
     const float2* ljtab;
@@ -41,46 +42,53 @@ __device__ __forceinline__ void red_add_v4(float4* addr, float x, float y, float
                  : "memory");
 }
 
-// beta^3 h(z), h = P5/Q5 (ewald_corr_coeffs.h); z = beta^2 r^2.
-__device__ __forceinline__ float ewald_bh(float z, float beta3)
+// Single-instruction MUFU forms: the arguments are clamped away from zero/denormals by the
+// caller (r^2 >= 1e-6, Q(z) >= 1), so the denormal fix-up code of rsqrtf()/__fdividef() is dead weight.
+__device__ __forceinline__ float rsqrt_fast(float x)
 {
-    float p = NB_EWC_P5;
-    p = fmaf(p, z, NB_EWC_P4);
-    p = fmaf(p, z, NB_EWC_P3);
-    p = fmaf(p, z, NB_EWC_P2);
-    p = fmaf(p, z, NB_EWC_P1);
-    p = fmaf(p, z, NB_EWC_P0);
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rcp_fast(float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// beta^3 h(z), h = P5/Q5 (ewald_corr_coeffs.h); z = beta^2 r^2; ewp[k] = beta^3 P_k.
+__device__ __forceinline__ float ewald_bh(float z, const float (&ewp)[6])
+{
+    float p = ewp[5];
+    p = fmaf(p, z, ewp[4]);
+    p = fmaf(p, z, ewp[3]);
+    p = fmaf(p, z, ewp[2]);
+    p = fmaf(p, z, ewp[1]);
+    p = fmaf(p, z, ewp[0]);
     float q = NB_EWC_Q5;
     q = fmaf(q, z, NB_EWC_Q4);
     q = fmaf(q, z, NB_EWC_Q3);
     q = fmaf(q, z, NB_EWC_Q2);
     q = fmaf(q, z, NB_EWC_Q1);
     q = fmaf(q, z, NB_EWC_Q0);
-    return __fdividef(p * beta3, q);
+    return p * rcp_fast(q);
 }
 
 struct IAtoms {
     float x[8], y[8], z[8], q[8];
-    int t[8];
+    int t[8];   // byte offset of the i atom's row in the shared LJ table
 };
 
-// One step: this lane's j atom against the 8 i atoms.
+// One step: this lane's j atom (xj, byte offset tjb of its LJ column) against the 8 i atoms.
+// MASKED: cbyte/mbyte carry the lane's 8 "counted"/"interacts" bits (reading A4: an excluded pair
+// keeps the Ewald/RF correction, loses LJ and the 1/r part).
 template <int COUL, bool ENERGY, bool MASKED>
-__device__ __forceinline__ void pair_step(const ForceArgs& A, const float2* __restrict__ s_lj, const IAtoms& I,
-                                          float (&fi)[24], float& elj, float& ecoul, int2 ce, bool valid, int warp,
-                                          int k)
+__device__ __forceinline__ void pair_step(const NbConst& K, const char* __restrict__ s_ljb, const IAtoms& I,
+                                          float (&fi)[24], float& elj, float& ecoul, const float4 xj, const int tjb,
+                                          unsigned cbyte, unsigned mbyte, float& fjx, float& fjy, float& fjz)
 {
-    const NbConst& K = A.kc;
-    const int cj = ce.x;
-    const float4 xj = A.xq[cj * 8 + k];
-    const int tj = A.type_slot[cj * 8 + k];
-    unsigned mbyte = 0xffu, cbyte = 0xffu;
-    if (MASKED) {
-        const ulonglong2 mm = *reinterpret_cast<const ulonglong2*>(&A.masks[((size_t)ce.y * 8 + warp) * 2]);
-        cbyte = valid ? (unsigned)(mm.y >> (8 * k)) & 0xffu : 0u;
-        mbyte = (unsigned)(mm.x >> (8 * k)) & cbyte;
-    }
-    float fjx = 0.f, fjy = 0.f, fjz = 0.f;
+    fjx = 0.f; fjy = 0.f; fjz = 0.f;
 #pragma unroll
     for (int a = 0; a < 8; a++) {
         const float dx = I.x[a] - xj.x, dy = I.y[a] - xj.y, dz = I.z[a] - xj.z;
@@ -88,9 +96,9 @@ __device__ __forceinline__ void pair_step(const ForceArgs& A, const float2* __re
         bool within = r2 < K.rc2;                            // A7: strict
         if (MASKED) within = within && ((cbyte >> a) & 1u);
         r2 = fmaxf(r2, 1e-6f);                               // keeps masked / padding pairs finite
-        const float rinv = rsqrtf(r2);
+        const float rinv = rsqrt_fast(r2);
         const float rinv2 = rinv * rinv;
-        const float2 c = s_lj[I.t[a] + tj];                  // (6 c6, 12 c12)
+        const float2 c = *reinterpret_cast<const float2*>(s_ljb + (I.t[a] + tjb));   // (6 c6, 12 c12)
         const float rinv6 = rinv2 * rinv2 * rinv2;
         const float flj = (c.y * rinv6 - c.x) * rinv6;
         const float qq = I.q[a] * xj.w;                      // epsfac folded into the i charge
@@ -102,7 +110,7 @@ __device__ __forceinline__ void pair_step(const ForceArgs& A, const float2* __re
         }
         float fs, bh = 0.f;
         if (COUL == NB_COUL_EWALD) {
-            bh = ewald_bh(K.beta2 * r2, K.beta3);
+            bh = ewald_bh(K.beta2 * r2, K.ewp);
             fs = fmaf(rinv2, t1, -qq * bh);                  // F/r = (F_lj r + A m/r)/r^2 - A beta^3 h
         } else {
             fs = fmaf(rinv2, t1, -qq * K.two_krf);           // F/r = ... - 2 A k_rf
@@ -128,15 +136,16 @@ __device__ __forceinline__ void pair_step(const ForceArgs& A, const float2* __re
             ecoul += within ? vc : 0.f;
         }
     }
-    if (valid) red_add_v4(&A.f4[cj * 8 + k], fjx, fjy, fjz);
 }
 
 template <int COUL, bool ENERGY>
 __global__ void __launch_bounds__(256, 2) k_force(ForceArgs A)
 {
     extern __shared__ float2 s_lj[];
-    __shared__ int2 s_q[8][40];
+    __shared__ int2 s_q[8][40];   // per-warp queue of cluster pairs without a mask for this i-cluster
+    __shared__ int2 s_m[8][40];   // per-warp queue of cluster pairs with a non-trivial mask (and the unit's tail)
     const NbConst& K = A.kc;
+    const char* s_ljb = reinterpret_cast<const char*>(s_lj);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7;
     for (int i = threadIdx.x; i < K.ntypes1 * K.ntypes1; i += blockDim.x) s_lj[i] = A.ljtab[i];
     const int4 u = A.units[blockIdx.x];
@@ -152,7 +161,7 @@ __global__ void __launch_bounds__(256, 2) k_force(ForceArgs A)
         I.y[a] = fmaf((float)sy, K.box[1], v.y);
         I.z[a] = fmaf((float)sz, K.box[2], v.z);
         I.q[a] = K.epsfac * v.w;
-        I.t[a] = A.type_slot[ci * 8 + a] * K.ntypes1;
+        I.t[a] = A.type_slot[ci * 8 + a] * K.ntypes1 * 8;
     }
     float fi[24];
 #pragma unroll
@@ -161,42 +170,93 @@ __global__ void __launch_bounds__(256, 2) k_force(ForceArgs A)
     __syncthreads();
 
     int2* q = s_q[warp];
-    int nq = 0;
+    int2* m = s_m[warp];
+    int nq = 0, mq = 0;
+    const unsigned lt = (1u << lane) - 1u;
     unsigned bits = A.plane[(size_t)u.y * 8 + warp];
+    unsigned ebits = A.plane_excl[(size_t)u.y * 8 + warp] & bits;
     int2 ent = ((bits >> lane) & 1u) ? A.jl[(size_t)u.y * 32 + lane] : make_int2(0, 0);
     for (int b = u.y; b < u.z; b++) {
-        unsigned bits_n = 0;
+        const bool last = b + 1 == u.z;
+        unsigned bits_n = 0, ebits_n = 0;
         int2 ent_n = make_int2(0, 0);
-        if (b + 1 < u.z) {   // prefetch the next batch of the joint list
+        if (!last) {   // prefetch the next batch of the joint list
             bits_n = A.plane[(size_t)(b + 1) * 8 + warp];
+            ebits_n = A.plane_excl[(size_t)(b + 1) * 8 + warp] & bits_n;
             if ((bits_n >> lane) & 1u) ent_n = A.jl[(size_t)(b + 1) * 32 + lane];
         }
-        // compact the entries whose mask bit is set into the warp's queue
-        if ((bits >> lane) & 1u) q[nq + __popc(bits & ((1u << lane) - 1u))] = ent;
-        nq += __popc(bits);
+        // compact the entries whose mask bit is set into the warp's two queues
+        const unsigned nbits = bits & ~ebits;
+        if ((nbits >> lane) & 1u) q[nq + __popc(nbits & lt)] = ent;
+        if ((ebits >> lane) & 1u) m[mq + __popc(ebits & lt)] = ent;
+        nq += __popc(nbits);
+        mq += __popc(ebits);
         __syncwarp();
+        // full unmasked steps; the j data of the next step is loaded before this step's arithmetic
         int done = 0;
-        for (; nq - done >= 4; done += 4) {
-            const int2 ce = q[done + g];
-            if (__any_sync(0xffffffffu, ce.y != 0))
-                pair_step<COUL, ENERGY, true>(A, s_lj, I, fi, elj, ecoul, ce, true, warp, k);
-            else
-                pair_step<COUL, ENERGY, false>(A, s_lj, I, fi, elj, ecoul, ce, true, warp, k);
+        if (nq >= 4) {
+            int cj = q[g].x;
+            float4 xj = A.xq[cj * 8 + k];
+            int tjb = A.type_slot[cj * 8 + k] * 8;
+            while (true) {
+                done += 4;
+                const bool more = nq - done >= 4;
+                int cj_n = cj;
+                float4 xj_n = xj;
+                int tjb_n = tjb;
+                if (more) {
+                    cj_n = q[done + g].x;
+                    xj_n = A.xq[cj_n * 8 + k];
+                    tjb_n = A.type_slot[cj_n * 8 + k] * 8;
+                }
+                float fjx, fjy, fjz;
+                pair_step<COUL, ENERGY, false>(K, s_ljb, I, fi, elj, ecoul, xj, tjb, 0xffu, 0xffu, fjx, fjy, fjz);
+                red_add_v4(&A.f4[cj * 8 + k], fjx, fjy, fjz);
+                if (!more) break;
+                cj = cj_n;
+                xj = xj_n;
+                tjb = tjb_n;
+            }
         }
         const int rem = nq - done;
         int2 t = make_int2(0, 0);
         if (lane < rem) t = q[done + lane];
         __syncwarp();
-        if (lane < rem) q[lane] = t;
+        if (last) {   // the unit's tail goes through the masked queue (partly filled step allowed there)
+            if (lane < rem) m[mq + lane] = t;
+            mq += rem;
+            nq = 0;
+        } else {
+            if (lane < rem) q[lane] = t;
+            nq = rem;
+        }
         __syncwarp();
-        nq = rem;
+        int md = 0;
+        while (mq - md >= 4 || (last && mq - md > 0)) {
+            const bool valid = g < mq - md;
+            const int2 ce = valid ? m[md + g] : make_int2(ci, 0);
+            const float4 xj = A.xq[ce.x * 8 + k];
+            const int tjb = A.type_slot[ce.x * 8 + k] * 8;
+            const ulonglong2 mm = *reinterpret_cast<const ulonglong2*>(&A.masks[((size_t)ce.y * 8 + warp) * 2]);
+            const unsigned cbyte = valid ? (unsigned)(mm.y >> (8 * k)) & 0xffu : 0u;
+            const unsigned mbyte = (unsigned)(mm.x >> (8 * k)) & cbyte;
+            float fjx, fjy, fjz;
+            pair_step<COUL, ENERGY, true>(K, s_ljb, I, fi, elj, ecoul, xj, tjb, cbyte, mbyte, fjx, fjy, fjz);
+            if (valid) red_add_v4(&A.f4[ce.x * 8 + k], fjx, fjy, fjz);
+            md += 4;
+        }
+        if (!last) {
+            const int mrem = mq - md;
+            int2 tm = make_int2(0, 0);
+            if (lane < mrem) tm = m[md + lane];
+            __syncwarp();
+            if (lane < mrem) m[lane] = tm;
+            __syncwarp();
+            mq = mrem;
+        }
         bits = bits_n;
+        ebits = ebits_n;
         ent = ent_n;
-    }
-    if (nq > 0) {   // last, partly filled step: idle groups are masked off
-        const bool valid = g < nq;
-        const int2 ce = valid ? q[g] : make_int2(ci, 0);
-        pair_step<COUL, ENERGY, true>(A, s_lj, I, fi, elj, ecoul, ce, valid, warp, k);
     }
 
     if (ENERGY) {
@@ -396,6 +456,7 @@ int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial)
     A.units = c->units_sorted.p;
     A.jl = c->jl.p;
     A.plane = c->plane_inner.p;
+    A.plane_excl = c->plane_excl.p;
     A.xq = c->xq.p;
     A.type_slot = c->type_slot.p;
     A.ljtab = c->ljtab.p;
@@ -403,6 +464,10 @@ int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial)
     A.f4 = c->f4.p;
     A.kc = c->kc;
     for (int k = 0; k < 3; k++) A.kc.box[k] = c->box[k];
+    {
+        const float P[6] = {NB_EWC_P0, NB_EWC_P1, NB_EWC_P2, NB_EWC_P3, NB_EWC_P4, NB_EWC_P5};
+        for (int k = 0; k < 6; k++) A.kc.ewp[k] = (float)((double)c->kc.beta3 * (double)P[k]);
+    }
     NB_CUDA(c, c->fshift.ensure(NB_NSHIFT * 3 + 9, st));
     A.fshift = c->fshift.p;
     A.energies = energies;

@@ -60,6 +60,7 @@ struct NbConst {
     float two_krf, krf, crf;
     float lj_sh6, lj_sh12;  // rc^-6, rc^-12 if potential-shift else 0
     int ntypes1;          // ntypes + 1 (row length of the padded LJ table)
+    float ewp[6];         // beta^3 * P_k of the Ewald correction fit (numerator carries beta^3)
 };
 
 struct nb_ctx {
@@ -112,6 +113,7 @@ struct nb_ctx {
     DevBuf<int2> jl;                           // [njslots] {cj, exclusion mask ref (0 = none)}
     DevBuf<uint8_t> imask_outer;               // [njslots] 8-bit interaction mask
     DevBuf<uint32_t> plane_outer, plane_inner; // [nbatch*8] bit-planes of the masks, word = (batch, i-cluster)
+    DevBuf<uint32_t> plane_excl;               // [nbatch*8] bit set: the entry's exclusion mask is non-trivial for this i-cluster
     DevBuf<int32_t> batch_ent;                 // [nbatch] owning (super-cluster, shift) slot
     DevBuf<int32_t> scan_tmp, scan_blk;        // scratch for device scans
     DevBuf<unsigned long long> excl_masks;     // [(nmask+1)*8*2] {interact, count} per (ref, i-cluster)

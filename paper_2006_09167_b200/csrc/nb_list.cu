@@ -287,6 +287,31 @@ __global__ void k_excl_assign(int2* __restrict__ jl, const int* __restrict__ pre
     }
 }
 
+// One warp per batch of 32 joint entries: word (batch, w) of plane_excl has bit e set iff entry e
+// carries a mask whose row for i-cluster w is not all-ones (a force-field exclusion, a self pair
+// or the lower triangle of a diagonal cluster pair).  The force kernel routes exactly those
+// (entry, i-cluster) pairs through its masked instantiation.
+__global__ void k_excl_planes(const int2* __restrict__ jl, const unsigned long long* __restrict__ masks,
+                              uint32_t* __restrict__ plane_excl, long long nbatch)
+{
+    long long b = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    int lane = threadIdx.x & 31;
+    if (b >= nbatch) return;
+    const int ref = jl[b * 32 + lane].y;
+    unsigned mine = 0;
+#pragma unroll
+    for (int w = 0; w < 8; w++) {
+        bool nt = false;
+        if (ref != 0) {
+            const unsigned long long* m = &masks[((size_t)ref * 8 + w) * 2];
+            nt = (m[0] & m[1]) != ~0ull;
+        }
+        unsigned word = __ballot_sync(0xffffffffu, nt);
+        if (lane == w) mine = word;
+    }
+    if (lane < 8) plane_excl[b * 8 + lane] = mine;
+}
+
 // ---------------------------------------------------------------- introspection
 __global__ void k_count_bits(const uint32_t* __restrict__ plane, long long nwords, long long* __restrict__ out)
 {
@@ -489,6 +514,7 @@ int nbi_search(nb_ctx* c, float rlist)
     NB_CUDA(c, c->imask_outer.ensure(std::max<int64_t>(c->njslots, 1), st));
     NB_CUDA(c, c->plane_outer.ensure(std::max<int64_t>(c->nbatch * 8, 1), st));
     NB_CUDA(c, c->plane_inner.ensure(std::max<int64_t>(c->nbatch * 8, 1), st));
+    NB_CUDA(c, c->plane_excl.ensure(std::max<int64_t>(c->nbatch * 8, 1), st));
     NB_CUDA(c, c->batch_ent.ensure(std::max<int64_t>(c->nbatch, 1) * 2, st));
     NB_CUDA(c, c->units_canon.ensure(std::max(c->nunits, 1), st));
     NB_CUDA(c, c->units_sorted.ensure(std::max(c->nunits, 1), st));
@@ -546,6 +572,8 @@ int nbi_search(nb_ctx* c, float rlist)
             k_excl<1><<<(c->natoms + 127) / 128, 128, 0, st>>>(E);
             NB_LAUNCH_CHECK(c);
         }
+        k_excl_planes<<<(unsigned)((c->nbatch * 32 + 255) / 256), 256, 0, st>>>(c->jl.p, c->excl_masks.p, c->plane_excl.p, c->nbatch);
+        NB_LAUNCH_CHECK(c);
     } else {
         std::vector<unsigned long long> ones(16, ~0ull);
         NB_CUDA(c, cudaMemcpyAsync(c->excl_masks.p, ones.data(), 16 * sizeof(unsigned long long), cudaMemcpyHostToDevice, st));
