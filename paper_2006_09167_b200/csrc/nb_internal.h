@@ -16,6 +16,7 @@
 #define NB_SC_ATOMS 64                // atoms per super-cluster (8 clusters x 8 atoms)
 #define NB_NHALF 14                   // zero shift + 13 shifts with s >lex 0
 #define NB_BATCH 32                   // joint j entries per mask word (one ballot)
+#define NB_MAX_UNIT_BATCHES 16        // a work unit spans at most this many batches of one list element
 #define NB_PAD_TYPE_ROW 1             // LJ table carries one extra all-zero type for padding atoms
 
 // One growable device array.

@@ -487,7 +487,7 @@ int nbi_search(nb_ctx* c, float rlist)
     int nsm = 148;
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, c->prm.device);
     int64_t target = (int64_t)16 * nsm;
-    int ub = (int)std::min<int64_t>(16, std::max<int64_t>(1, c->nbatch / target));
+    int ub = (int)std::min<int64_t>(NB_MAX_UNIT_BATCHES, std::max<int64_t>(1, c->nbatch / target));
     c->h_units.clear();
     std::vector<int32_t> h_batch_ent(c->nbatch), h_batch_unit(c->nbatch);
     for (int e = 0; e < c->nent; e++) {

@@ -10,7 +10,10 @@
 // is the contiguous range [p*nu/k, (p+1)*nu/k) of the canonically ordered work units.
 // Block = 8 warps = the 8 i-clusters of one super-cluster (one work unit); warp w owns the
 // bit-plane w of the unit's mask words, so no cross-warp combination is needed.  Lanes own
-// j atoms: 4 j-clusters x 8 atoms per step, the 8 i-atoms live in registers.
+// j atoms: 4 j-clusters x 8 atoms per step, the 8 i-atoms live in registers.  The set bits of
+// the outer plane words are compacted into a per-warp queue (as in the force kernel), so every
+// step but the unit's last is full, and the j coordinates of the next step are loaded before
+// the current step's arithmetic.
 #include "nb_internal.h"
 
 namespace {
@@ -25,8 +28,27 @@ struct PruneArgs {
     float rl2;   // fl32(rlist_inner^2), reading A12
 };
 
+// 8 exact (A12) distance checks of this lane's j atom; DIAG keeps only pairs b > a.
+template <bool DIAG>
+__device__ __forceinline__ bool prune_checks(const float (&xi)[8], const float (&yi)[8], const float (&zi)[8],
+                                             const float4 xj, float rl2, bool diag, int k)
+{
+    bool found = false;
+#pragma unroll
+    for (int a = 0; a < 8; a++) {
+        const float dx = __fsub_rn(xi[a], xj.x), dy = __fsub_rn(yi[a], xj.y), dz = __fsub_rn(zi[a], xj.z);
+        const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+        bool ok = d2 < rl2;
+        if (DIAG) ok = ok && (!diag || k > a);   // zero-shift diagonal: only b > a are pairs
+        found = found || ok;
+    }
+    return found;
+}
+
 __global__ void __launch_bounds__(256) k_prune(PruneArgs A)
 {
+    __shared__ int2 s_q[8][40];                          // {cj, unit-local joint slot}
+    __shared__ unsigned s_res[8][NB_MAX_UNIT_BATCHES];   // inner mask words of this warp's plane
     const int4 u = A.units[blockIdx.x];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7;
     const int sci = u.w, h = u.x - sci * NB_NHALF, ci = sci * 8 + warp;
@@ -40,37 +62,67 @@ __global__ void __launch_bounds__(256) k_prune(PruneArgs A)
         yi[a] = __fmaf_rn((float)sy, A.box[1], v.y);
         zi[a] = __fmaf_rn((float)sz, A.box[2], v.z);
     }
+    int2* q = s_q[warp];
+    unsigned* res = s_res[warp];
+    if (lane < NB_MAX_UNIT_BATCHES) res[lane] = 0u;
+    const unsigned lt = (1u << lane) - 1u;
+    int nq = 0;
+    unsigned bits = A.plane_outer[(size_t)u.y * 8 + warp];
+    int cje = ((bits >> lane) & 1u) ? A.jl[(size_t)u.y * 32 + lane].x : 0;
+    __syncwarp();
     for (int b = u.y; b < u.z; b++) {
-        unsigned bits = A.plane_outer[(size_t)b * 8 + warp];
-        unsigned result = 0;
-        while (bits) {
-            int p[4];
-#pragma unroll
-            for (int t = 0; t < 4; t++) {
-                p[t] = bits ? __ffs(bits) - 1 : -1;
-                bits &= bits - 1;
-            }
-            const int my = g == 0 ? p[0] : (g == 1 ? p[1] : (g == 2 ? p[2] : p[3]));
-            const bool valid = my >= 0;
-            const int cj = valid ? A.jl[(size_t)b * 32 + my].x : ci;
-            const float4 xj = A.xq[cj * 8 + k];
-            const bool diag = cj == ci && h == 0;
-            bool found = false;
-#pragma unroll
-            for (int a = 0; a < 8; a++) {
-                const float dx = __fsub_rn(xi[a], xj.x), dy = __fsub_rn(yi[a], xj.y), dz = __fsub_rn(zi[a], xj.z);
-                const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-                bool ok = d2 < A.rl2;
-                if (diag) ok = ok && (k > a);   // zero-shift diagonal: only b > a are pairs
-                found = found || ok;
-            }
-            const unsigned gm = __ballot_sync(0xffffffffu, found && valid);
-#pragma unroll
-            for (int t = 0; t < 4; t++)
-                if (p[t] >= 0 && ((gm >> (8 * t)) & 0xffu)) result |= 1u << p[t];
+        const bool last = b + 1 == u.z;
+        unsigned bits_n = 0;
+        int cje_n = 0;
+        if (!last) {
+            bits_n = A.plane_outer[(size_t)(b + 1) * 8 + warp];
+            if ((bits_n >> lane) & 1u) cje_n = A.jl[(size_t)(b + 1) * 32 + lane].x;
         }
-        if (lane == 0) A.plane_inner[(size_t)b * 8 + warp] = result;
+        if ((bits >> lane) & 1u) q[nq + __popc(bits & lt)] = make_int2(cje, (b - u.y) * 32 + lane);
+        nq += __popc(bits);
+        __syncwarp();
+        int done = 0;
+        const int need = last ? 1 : 4;   // the unit's last batch also runs the partly filled step
+        if (nq >= need) {
+            bool valid = g < nq;
+            int2 ce = valid ? q[g] : make_int2(ci, 0);
+            float4 xj = A.xq[ce.x * 8 + k];
+            while (true) {
+                done += 4;
+                const bool more = nq - done >= need;
+                bool valid_n = false;
+                int2 ce_n = ce;
+                float4 xj_n = xj;
+                if (more) {
+                    valid_n = done + g < nq;
+                    ce_n = valid_n ? q[done + g] : make_int2(ci, 0);
+                    xj_n = A.xq[ce_n.x * 8 + k];
+                }
+                const bool diag = ce.x == ci && h == 0;
+                bool found;
+                if (__any_sync(0xffffffffu, diag)) found = prune_checks<true>(xi, yi, zi, xj, A.rl2, diag, k);
+                else found = prune_checks<false>(xi, yi, zi, xj, A.rl2, false, k);
+                const unsigned gm = __ballot_sync(0xffffffffu, found && valid);
+                if (k == 0 && ((gm >> (8 * g)) & 0xffu)) atomicOr(&res[ce.y >> 5], 1u << (ce.y & 31));
+                if (!more) break;
+                valid = valid_n;
+                ce = ce_n;
+                xj = xj_n;
+            }
+            done = min(done, nq);
+        }
+        const int rem = nq - done;
+        int2 t = make_int2(0, 0);
+        if (lane < rem) t = q[done + lane];
+        __syncwarp();
+        if (lane < rem) q[lane] = t;
+        __syncwarp();
+        nq = rem;
+        bits = bits_n;
+        cje = cje_n;
     }
+    __syncwarp();
+    if (lane < u.z - u.y) A.plane_inner[(size_t)(u.y + lane) * 8 + warp] = res[lane];
 }
 
 }  // namespace
