@@ -71,6 +71,7 @@ extern "C" int nb_init(const nb_params* p, nb_ctx** out)
     K.lj_sh12 = p->lj_modifier == NB_MOD_POTSHIFT ? (float)pow(rc, -12.0) : 0.f;
     K.ntypes1 = p->ntypes + 1;
     c->beta = (float)beta;
+    c->beta_d = beta;
     c->st.ewald_beta = (float)beta;
 
     cudaStream_t st = c->stream;
@@ -203,7 +204,8 @@ extern "C" void nb_free(nb_ctx* c)
     c->ent_count.release(); c->ent_jbegin.release(); c->jl.release(); c->imask_outer.release();
     c->plane_outer.release(); c->plane_inner.release(); c->plane_excl.release(); c->batch_ent.release(); c->scan_tmp.release();
     c->scan_blk.release(); c->excl_masks.release(); c->counters.release(); c->units_canon.release();
-    c->units_sorted.release(); c->fshift.release();
+    c->units_sorted.release(); c->fshift.release(); c->unit_order.release();
+    c->il_off.release(); c->ilm_off.release(); c->il_cnt.release(); c->il.release(); c->ilm.release();
     delete c;
 }
 

@@ -22,14 +22,19 @@
 namespace {
 
 struct ForceArgs {
-    const int4* units;
+    const int4* units;          // canonical work units {entry slot, batch begin, batch end, sci}
+    const int* unit_order;      // launch order (longest first) -> canonical unit index; nullptr = identity
     const int2* jl;
     const uint32_t* plane;
-    const uint32_t* plane_excl;
     const float4* xq;
     const int* type_slot;
     const float2* ljtab;
     const unsigned long long* masks;
+    const int* il_off;          // compact inner list, see nb_internal.h
+    const int* ilm_off;
+    const int2* il_cnt;
+    const int* il;
+    const int2* ilm;
     float4* f4;
     double* fshift;     // [27*3]
     double* energies;   // [2]
@@ -57,83 +62,104 @@ __device__ __forceinline__ float rcp_fast(float x)
     return y;
 }
 
-// beta^3 h(z), h = P5/Q5 (ewald_corr_coeffs.h); z = beta^2 r^2; ewp[k] = beta^3 P_k.
-__device__ __forceinline__ float ewald_bh(float z, const float (&ewp)[6])
+// Packed FP32x2 arithmetic (sm_100 FFMA2/FMUL2/FADD2): one issue slot per two pair evaluations.
+// The FP32 pipe rate in flop/s is the same as for scalar FFMA (measured), but the kernel is
+// issue-bound in scalar form, so halving the issue slots of the
+// FP32-pipe work is what moves it towards the FP32 roofline.
+__device__ __forceinline__ float2 f2(float a, float b) { return make_float2(a, b); }
+__device__ __forceinline__ float2 f2(float a) { return make_float2(a, a); }
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
+
+// beta^3 h(z) for two pairs, as P5(r^2)/Q5(r^2) with beta folded into the coefficients.
+__device__ __forceinline__ float2 ewald_bh2(float2 r2, const NbConst& K)
 {
-    float p = ewp[5];
-    p = fmaf(p, z, ewp[4]);
-    p = fmaf(p, z, ewp[3]);
-    p = fmaf(p, z, ewp[2]);
-    p = fmaf(p, z, ewp[1]);
-    p = fmaf(p, z, ewp[0]);
-    float q = NB_EWC_Q5;
-    q = fmaf(q, z, NB_EWC_Q4);
-    q = fmaf(q, z, NB_EWC_Q3);
-    q = fmaf(q, z, NB_EWC_Q2);
-    q = fmaf(q, z, NB_EWC_Q1);
-    q = fmaf(q, z, NB_EWC_Q0);
-    return p * rcp_fast(q);
+    float2 p = fma2(K.ewp2[5], r2, K.ewp2[4]);
+    float2 q = fma2(K.ewq2[5], r2, K.ewq2[4]);
+    p = fma2(p, r2, K.ewp2[3]);
+    q = fma2(q, r2, K.ewq2[3]);
+    p = fma2(p, r2, K.ewp2[2]);
+    q = fma2(q, r2, K.ewq2[2]);
+    p = fma2(p, r2, K.ewp2[1]);
+    q = fma2(q, r2, K.ewq2[1]);
+    p = fma2(p, r2, K.ewp2[0]);
+    q = fma2(q, r2, K.ewq2[0]);
+    return mul2(p, f2(rcp_fast(q.x), rcp_fast(q.y)));
 }
 
+// The 8 i atoms of the warp's cluster as 4 packed pairs (atoms 2p, 2p+1); charges carry epsfac.
 struct IAtoms {
-    float x[8], y[8], z[8], q[8];
-    int t[8];   // byte offset of the i atom's row in the shared LJ table
+    float2 x[4], y[4], z[4], q[4];
 };
 
-// One step: this lane's j atom (xj, byte offset tjb of its LJ column) against the 8 i atoms.
+// One step: this lane's j atom (xj; ljj points at the lane's j-type column of the warp's paired LJ
+// table, stride `ljs` float4 between i-atom pairs) against the 8 i atoms, two at a time.
 // MASKED: cbyte/mbyte carry the lane's 8 "counted"/"interacts" bits (reading A4: an excluded pair
 // keeps the Ewald/RF correction, loses LJ and the 1/r part).
+// Returns the NEGATED j force in (fjx, fjy, fjz) pairs (sum the halves and negate).
 template <int COUL, bool ENERGY, bool MASKED>
-__device__ __forceinline__ void pair_step(const NbConst& K, const char* __restrict__ s_ljb, const IAtoms& I,
-                                          float (&fi)[24], float& elj, float& ecoul, const float4 xj, const int tjb,
-                                          unsigned cbyte, unsigned mbyte, float& fjx, float& fjy, float& fjz)
+__device__ __forceinline__ void pair_step(const NbConst& K, const float4* __restrict__ ljj, const int ljs, const IAtoms& I,
+                                          float2 (&fix)[4], float2 (&fiy)[4], float2 (&fiz)[4], float& elj, float& ecoul,
+                                          const float4 xj, unsigned cbyte, unsigned mbyte, float2& fjx, float2& fjy,
+                                          float2& fjz)
 {
-    fjx = 0.f; fjy = 0.f; fjz = 0.f;
+    const float2 nxj = f2(-xj.x), nyj = f2(-xj.y), nzj = f2(-xj.z), qj = f2(xj.w);
+    fjx = f2(0.f); fjy = f2(0.f); fjz = f2(0.f);
 #pragma unroll
-    for (int a = 0; a < 8; a++) {
-        const float dx = I.x[a] - xj.x, dy = I.y[a] - xj.y, dz = I.z[a] - xj.z;
-        float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-        bool within = r2 < K.rc2;                            // A7: strict
-        if (MASKED) within = within && ((cbyte >> a) & 1u);
-        r2 = fmaxf(r2, 1e-6f);                               // keeps masked / padding pairs finite
-        const float rinv = rsqrt_fast(r2);
-        const float rinv2 = rinv * rinv;
-        const float2 c = *reinterpret_cast<const float2*>(s_ljb + (I.t[a] + tjb));   // (6 c6, 12 c12)
-        const float rinv6 = rinv2 * rinv2 * rinv2;
-        const float flj = (c.y * rinv6 - c.x) * rinv6;
-        const float qq = I.q[a] * xj.w;                      // epsfac folded into the i charge
-        float t1 = fmaf(qq, rinv, flj);                      // (F_lj + A/r) r
-        float mf = 1.f;
+    for (int p = 0; p < 4; p++) {
+        const float2 dx = add2(I.x[p], nxj), dy = add2(I.y[p], nyj), dz = add2(I.z[p], nzj);
+        const float2 r2u = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+        bool w0 = r2u.x < K.rc2, w1 = r2u.y < K.rc2;        // A7: strict
         if (MASKED) {
-            mf = ((mbyte >> a) & 1u) ? 1.f : 0.f;            // excluded pair: only the correction term
-            t1 *= mf;
+            w0 = w0 && ((cbyte >> (2 * p)) & 1u);
+            w1 = w1 && ((cbyte >> (2 * p + 1)) & 1u);
         }
-        float fs, bh = 0.f;
+        const float2 r2 = f2(fmaxf(r2u.x, 1e-6f), fmaxf(r2u.y, 1e-6f));   // keeps masked / padding pairs finite
+        const float2 rinv = f2(rsqrt_fast(r2.x), rsqrt_fast(r2.y));
+        const float2 rinv2 = mul2(rinv, rinv);
+        const float4 c = ljj[p * ljs];                        // (-6 c6_a, -6 c6_b, 12 c12_a, 12 c12_b)
+        const float2 nc6 = f2(c.x, c.y), c12 = f2(c.z, c.w);
+        const float2 rinv6 = mul2(mul2(rinv2, rinv2), rinv2);
+        const float2 flj = mul2(fma2(c12, rinv6, nc6), rinv6);
+        const float2 qq = mul2(I.q[p], qj);                   // epsfac folded into the i charge
+        float2 t1 = fma2(qq, rinv, flj);                      // (F_lj + A/r) r
+        float2 mf = f2(1.f);
+        if (MASKED) {
+            mf = f2(((mbyte >> (2 * p)) & 1u) ? 1.f : 0.f, ((mbyte >> (2 * p + 1)) & 1u) ? 1.f : 0.f);
+            t1 = mul2(t1, mf);                                // excluded pair: only the correction term
+        }
+        float2 fs, bh = f2(0.f);
         if (COUL == NB_COUL_EWALD) {
-            bh = ewald_bh(K.beta2 * r2, K.ewp);
-            fs = fmaf(rinv2, t1, -qq * bh);                  // F/r = (F_lj r + A m/r)/r^2 - A beta^3 h
+            bh = ewald_bh2(r2, K);
+            fs = fma2(rinv2, t1, neg2(mul2(qq, bh)));         // F/r = (F_lj r + A m/r)/r^2 - A beta^3 h
         } else {
-            fs = fmaf(rinv2, t1, -qq * K.two_krf);           // F/r = ... - 2 A k_rf
+            fs = fma2(rinv2, t1, neg2(mul2(qq, f2(K.two_krf))));   // F/r = ... - 2 A k_rf
         }
-        fs = within ? fs : 0.f;
-        fi[3 * a + 0] = fmaf(fs, dx, fi[3 * a + 0]);
-        fi[3 * a + 1] = fmaf(fs, dy, fi[3 * a + 1]);
-        fi[3 * a + 2] = fmaf(fs, dz, fi[3 * a + 2]);
-        fjx = fmaf(-fs, dx, fjx);
-        fjy = fmaf(-fs, dy, fjy);
-        fjz = fmaf(-fs, dz, fjz);
+        fs = f2(w0 ? fs.x : 0.f, w1 ? fs.y : 0.f);
+        fix[p] = fma2(fs, dx, fix[p]);
+        fiy[p] = fma2(fs, dy, fiy[p]);
+        fiz[p] = fma2(fs, dz, fiz[p]);
+        fjx = fma2(fs, dx, fjx);
+        fjy = fma2(fs, dy, fjy);
+        fjz = fma2(fs, dz, fjz);
         if (ENERGY) {
-            const float vlj = c.y * (1.f / 12.f) * (rinv6 * rinv6 - K.lj_sh12) - c.x * (1.f / 6.f) * (rinv6 - K.lj_sh6);
-            float vc;
+            // V_lj = c12 (r^-12 - rc^-12) - c6 (r^-6 - rc^-6), table holds (-6 c6, 12 c12)
+            const float2 a12 = fma2(rinv6, rinv6, f2(-K.lj_sh12)), a6 = add2(rinv6, f2(-K.lj_sh6));
+            const float2 vlj = fma2(mul2(c12, f2(1.f / 12.f)), a12, mul2(mul2(nc6, f2(1.f / 6.f)), a6));
+            float2 vc;
             if (COUL == NB_COUL_EWALD) {
                 // beta e(z) = r^2 beta^3 h(z) + beta (2/sqrt(pi)) exp(-z)
-                const float be = fmaf(r2, bh, K.beta * 1.1283791671f * __expf(-K.beta2 * r2));
-                vc = qq * (mf * (rinv - K.ewald_shift) - be);
+                const float2 ex = f2(__expf(-K.beta2 * r2.x), __expf(-K.beta2 * r2.y));
+                const float2 be = fma2(r2, bh, mul2(f2(K.beta * 1.1283791671f), ex));
+                vc = mul2(qq, add2(mul2(mf, add2(rinv, f2(-K.ewald_shift))), neg2(be)));
             } else {
-                vc = qq * (mf * rinv + K.krf * r2 - K.crf);
+                vc = mul2(qq, fma2(mf, rinv, fma2(f2(K.krf), r2, f2(-K.crf))));
             }
-            elj += within ? mf * vlj : 0.f;
-            ecoul += within ? vc : 0.f;
+            const float2 vl = mul2(mf, vlj);
+            elj += (w0 ? vl.x : 0.f) + (w1 ? vl.y : 0.f);
+            ecoul += (w0 ? vc.x : 0.f) + (w1 ? vc.y : 0.f);
         }
     }
 }
@@ -141,124 +167,86 @@ __device__ __forceinline__ void pair_step(const NbConst& K, const char* __restri
 template <int COUL, bool ENERGY>
 __global__ void __launch_bounds__(256, 2) k_force(ForceArgs A)
 {
-    extern __shared__ float2 s_lj[];
-    __shared__ int2 s_q[8][40];   // per-warp queue of cluster pairs without a mask for this i-cluster
-    __shared__ int2 s_m[8][40];   // per-warp queue of cluster pairs with a non-trivial mask (and the unit's tail)
+    // Paired LJ table of this block: s_ljp[(w*4 + p)*nt1 + tj] = (-6c6, -6c6', 12c12, 12c12') of the
+    // i atoms 2p, 2p+1 of i-cluster w against j type tj: one LDS.128 feeds both packed operands.
+    extern __shared__ float4 s_ljp[];
     const NbConst& K = A.kc;
-    const char* s_ljb = reinterpret_cast<const char*>(s_lj);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7;
-    for (int i = threadIdx.x; i < K.ntypes1 * K.ntypes1; i += blockDim.x) s_lj[i] = A.ljtab[i];
-    const int4 u = A.units[blockIdx.x];
+    const int uidx = A.unit_order ? A.unit_order[blockIdx.x] : blockIdx.x;
+    const int4 u = A.units[uidx];
     const int sci = u.w, h = u.x - sci * NB_NHALF, ci = sci * 8 + warp;
     const int sid = nb_half_shift_id(h);
+    const int nt1 = K.ntypes1;
+    for (int i = threadIdx.x; i < 32 * nt1; i += blockDim.x) {
+        const int wp = i / nt1, tj = i - wp * nt1;
+        const int ta = A.type_slot[sci * NB_SC_ATOMS + 2 * wp], tb = A.type_slot[sci * NB_SC_ATOMS + 2 * wp + 1];
+        const float2 ca = A.ljtab[ta * nt1 + tj], cb = A.ljtab[tb * nt1 + tj];
+        s_ljp[i] = make_float4(-ca.x, -cb.x, ca.y, cb.y);
+    }
     int sx, sy, sz;
     nb_shift_vec(sid, sx, sy, sz);
     IAtoms I;
 #pragma unroll
-    for (int a = 0; a < 8; a++) {
-        const float4 v = A.xq[ci * 8 + a];
-        I.x[a] = fmaf((float)sx, K.box[0], v.x);
-        I.y[a] = fmaf((float)sy, K.box[1], v.y);
-        I.z[a] = fmaf((float)sz, K.box[2], v.z);
-        I.q[a] = K.epsfac * v.w;
-        I.t[a] = A.type_slot[ci * 8 + a] * K.ntypes1 * 8;
+    for (int p = 0; p < 4; p++) {
+        const float4 v0 = A.xq[ci * 8 + 2 * p], v1 = A.xq[ci * 8 + 2 * p + 1];
+        I.x[p] = f2(fmaf((float)sx, K.box[0], v0.x), fmaf((float)sx, K.box[0], v1.x));
+        I.y[p] = f2(fmaf((float)sy, K.box[1], v0.y), fmaf((float)sy, K.box[1], v1.y));
+        I.z[p] = f2(fmaf((float)sz, K.box[2], v0.z), fmaf((float)sz, K.box[2], v1.z));
+        I.q[p] = f2(K.epsfac * v0.w, K.epsfac * v1.w);
     }
-    float fi[24];
+    float2 fix[4], fiy[4], fiz[4];
 #pragma unroll
-    for (int i = 0; i < 24; i++) fi[i] = 0.f;
+    for (int p = 0; p < 4; p++) { fix[p] = f2(0.f); fiy[p] = f2(0.f); fiz[p] = f2(0.f); }
     float elj = 0.f, ecoul = 0.f;
+    const int seg = uidx * 8 + warp;
+    const int2 cnt = A.il_cnt[seg];
+    const int* __restrict__ il = A.il + A.il_off[seg];
+    const int2* __restrict__ ilm = A.ilm + A.ilm_off[seg];
+    const float4* ljw = s_ljp + warp * 4 * nt1;
     __syncthreads();
 
-    int2* q = s_q[warp];
-    int2* m = s_m[warp];
-    int nq = 0, mq = 0;
-    const unsigned lt = (1u << lane) - 1u;
-    unsigned bits = A.plane[(size_t)u.y * 8 + warp];
-    unsigned ebits = A.plane_excl[(size_t)u.y * 8 + warp] & bits;
-    int2 ent = ((bits >> lane) & 1u) ? A.jl[(size_t)u.y * 32 + lane] : make_int2(0, 0);
-    for (int b = u.y; b < u.z; b++) {
-        const bool last = b + 1 == u.z;
-        unsigned bits_n = 0, ebits_n = 0;
-        int2 ent_n = make_int2(0, 0);
-        if (!last) {   // prefetch the next batch of the joint list
-            bits_n = A.plane[(size_t)(b + 1) * 8 + warp];
-            ebits_n = A.plane_excl[(size_t)(b + 1) * 8 + warp] & bits_n;
-            if ((bits_n >> lane) & 1u) ent_n = A.jl[(size_t)(b + 1) * 32 + lane];
-        }
-        // compact the entries whose mask bit is set into the warp's two queues
-        const unsigned nbits = bits & ~ebits;
-        if ((nbits >> lane) & 1u) q[nq + __popc(nbits & lt)] = ent;
-        if ((ebits >> lane) & 1u) m[mq + __popc(ebits & lt)] = ent;
-        nq += __popc(nbits);
-        mq += __popc(ebits);
-        __syncwarp();
-        // full unmasked steps; the j data of the next step is loaded before this step's arithmetic
-        int done = 0;
-        if (nq >= 4) {
-            int cj = q[g].x;
-            float4 xj = A.xq[cj * 8 + k];
-            int tjb = A.type_slot[cj * 8 + k] * 8;
-            while (true) {
-                done += 4;
-                const bool more = nq - done >= 4;
-                int cj_n = cj;
-                float4 xj_n = xj;
-                int tjb_n = tjb;
-                if (more) {
-                    cj_n = q[done + g].x;
-                    xj_n = A.xq[cj_n * 8 + k];
-                    tjb_n = A.type_slot[cj_n * 8 + k] * 8;
-                }
-                float fjx, fjy, fjz;
-                pair_step<COUL, ENERGY, false>(K, s_ljb, I, fi, elj, ecoul, xj, tjb, 0xffu, 0xffu, fjx, fjy, fjz);
-                red_add_v4(&A.f4[cj * 8 + k], fjx, fjy, fjz);
-                if (!more) break;
-                cj = cj_n;
-                xj = xj_n;
-                tjb = tjb_n;
+    // Cluster pairs without a mask: always full steps of 4 j-clusters; the j data of step s+1 and
+    // the list entries of step s+2 are requested before the arithmetic of step s.
+    const int ns = cnt.x >> 2;
+    if (ns > 0) {
+        int cj = il[g];
+        int cj_n = ns > 1 ? il[4 + g] : cj;
+        float4 xj = A.xq[cj * 8 + k];
+        int tj = A.type_slot[cj * 8 + k];
+        for (int s = 0; s < ns; s++) {
+            float4 xj_n = xj;
+            int tj_n = tj, cj_nn = cj_n;
+            if (s + 1 < ns) {
+                xj_n = A.xq[cj_n * 8 + k];
+                tj_n = A.type_slot[cj_n * 8 + k];
             }
+            if (s + 2 < ns) cj_nn = il[4 * (s + 2) + g];
+            float2 fjx, fjy, fjz;
+            pair_step<COUL, ENERGY, false>(K, ljw + tj, nt1, I, fix, fiy, fiz, elj, ecoul, xj, 0xffu, 0xffu, fjx, fjy, fjz);
+            red_add_v4(&A.f4[cj * 8 + k], -(fjx.x + fjx.y), -(fjy.x + fjy.y), -(fjz.x + fjz.y));
+            cj = cj_n; cj_n = cj_nn; xj = xj_n; tj = tj_n;
         }
-        const int rem = nq - done;
-        int2 t = make_int2(0, 0);
-        if (lane < rem) t = q[done + lane];
-        __syncwarp();
-        if (last) {   // the unit's tail goes through the masked queue (partly filled step allowed there)
-            if (lane < rem) m[mq + lane] = t;
-            mq += rem;
-            nq = 0;
-        } else {
-            if (lane < rem) q[lane] = t;
-            nq = rem;
-        }
-        __syncwarp();
-        int md = 0;
-        while (mq - md >= 4 || (last && mq - md > 0)) {
-            const bool valid = g < mq - md;
-            const int2 ce = valid ? m[md + g] : make_int2(ci, 0);
-            const float4 xj = A.xq[ce.x * 8 + k];
-            const int tjb = A.type_slot[ce.x * 8 + k] * 8;
-            const ulonglong2 mm = *reinterpret_cast<const ulonglong2*>(&A.masks[((size_t)ce.y * 8 + warp) * 2]);
-            const unsigned cbyte = valid ? (unsigned)(mm.y >> (8 * k)) & 0xffu : 0u;
-            const unsigned mbyte = (unsigned)(mm.x >> (8 * k)) & cbyte;
-            float fjx, fjy, fjz;
-            pair_step<COUL, ENERGY, true>(K, s_ljb, I, fi, elj, ecoul, xj, tjb, cbyte, mbyte, fjx, fjy, fjz);
-            if (valid) red_add_v4(&A.f4[ce.x * 8 + k], fjx, fjy, fjz);
-            md += 4;
-        }
-        if (!last) {
-            const int mrem = mq - md;
-            int2 tm = make_int2(0, 0);
-            if (lane < mrem) tm = m[md + lane];
-            __syncwarp();
-            if (lane < mrem) m[lane] = tm;
-            __syncwarp();
-            mq = mrem;
-        }
-        bits = bits_n;
-        ebits = ebits_n;
-        ent = ent_n;
+    }
+    // Cluster pairs with exclusion / self / diagonal masks, and the segment's tail (ref 0 = all ones).
+    for (int s = 0; s < cnt.y; s += 4) {
+        const bool valid = s + g < cnt.y;
+        const int2 ce = valid ? ilm[s + g] : make_int2(ci, 0);
+        const float4 xj = A.xq[ce.x * 8 + k];
+        const int tj = A.type_slot[ce.x * 8 + k];
+        const ulonglong2 mm = *reinterpret_cast<const ulonglong2*>(&A.masks[((size_t)ce.y * 8 + warp) * 2]);
+        const unsigned cbyte = valid ? (unsigned)(mm.y >> (8 * k)) & 0xffu : 0u;
+        const unsigned mbyte = (unsigned)(mm.x >> (8 * k)) & cbyte;
+        float2 fjx, fjy, fjz;
+        pair_step<COUL, ENERGY, true>(K, ljw + tj, nt1, I, fix, fiy, fiz, elj, ecoul, xj, cbyte, mbyte, fjx, fjy, fjz);
+        if (valid) red_add_v4(&A.f4[ce.x * 8 + k], -(fjx.x + fjx.y), -(fjy.x + fjy.y), -(fjz.x + fjz.y));
     }
 
+    float fi[24];
+#pragma unroll
+    for (int p = 0; p < 4; p++) {
+        fi[6 * p + 0] = fix[p].x; fi[6 * p + 1] = fiy[p].x; fi[6 * p + 2] = fiz[p].x;
+        fi[6 * p + 3] = fix[p].y; fi[6 * p + 4] = fiy[p].y; fi[6 * p + 5] = fiz[p].y;
+    }
     if (ENERGY) {
         // per-shift sum of i forces for the virial (reading A8) and the energies, fp64 atomics per warp
         float sxs = 0.f, sys = 0.f, szs = 0.f;
@@ -436,12 +424,9 @@ __global__ void __launch_bounds__(256) k_count_pairs(ForceArgs A, unsigned long 
 template <int COUL, bool ENERGY>
 int launch_force(nb_ctx* c, const ForceArgs& A)
 {
-    const size_t smem = sizeof(float2) * (size_t)c->kc.ntypes1 * c->kc.ntypes1;
-    static bool attr_set = false;
-    if (!attr_set || smem > 48 * 1024) {
-        NB_CUDA(c, cudaFuncSetAttribute(k_force<COUL, ENERGY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-        attr_set = true;
-    }
+    const size_t smem = sizeof(float4) * 32 * (size_t)c->kc.ntypes1;   // paired LJ table, 512 B per type
+    if (smem > 48 * 1024)
+        NB_CUDA(c, cudaFuncSetAttribute(k_force<COUL, ENERGY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k_force<COUL, ENERGY><<<c->nunits, 256, smem, c->stream>>>(A);
     NB_LAUNCH_CHECK(c);
     return NB_OK;
@@ -453,10 +438,15 @@ int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial)
 {
     cudaStream_t st = c->stream;
     ForceArgs A;
-    A.units = c->units_sorted.p;
+    A.units = c->units_canon.p;
+    A.unit_order = c->unit_order.p;
     A.jl = c->jl.p;
     A.plane = c->plane_inner.p;
-    A.plane_excl = c->plane_excl.p;
+    A.il_off = c->il_off.p;
+    A.ilm_off = c->ilm_off.p;
+    A.il_cnt = c->il_cnt.p;
+    A.il = c->il.p;
+    A.ilm = c->ilm.p;
     A.xq = c->xq.p;
     A.type_slot = c->type_slot.p;
     A.ljtab = c->ljtab.p;
@@ -465,8 +455,14 @@ int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial)
     A.kc = c->kc;
     for (int k = 0; k < 3; k++) A.kc.box[k] = c->box[k];
     {
-        const float P[6] = {NB_EWC_P0, NB_EWC_P1, NB_EWC_P2, NB_EWC_P3, NB_EWC_P4, NB_EWC_P5};
-        for (int k = 0; k < 6; k++) A.kc.ewp[k] = (float)((double)c->kc.beta3 * (double)P[k]);
+        const double P[6] = {NB_EWC_P0, NB_EWC_P1, NB_EWC_P2, NB_EWC_P3, NB_EWC_P4, NB_EWC_P5};
+        const double Q[6] = {NB_EWC_Q0, NB_EWC_Q1, NB_EWC_Q2, NB_EWC_Q3, NB_EWC_Q4, NB_EWC_Q5};
+        const double b = c->beta_d, b2 = b * b;
+        double bk = 1.0;   // beta^(2k)
+        for (int k = 0; k < 6; k++, bk *= b2) {
+            A.kc.ewp2[k] = make_float2((float)(b * b2 * bk * P[k]), (float)(b * b2 * bk * P[k]));
+            A.kc.ewq2[k] = make_float2((float)(bk * Q[k]), (float)(bk * Q[k]));
+        }
     }
     NB_CUDA(c, c->fshift.ensure(NB_NSHIFT * 3 + 9, st));
     A.fshift = c->fshift.p;

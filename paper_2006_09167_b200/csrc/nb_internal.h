@@ -61,7 +61,9 @@ struct NbConst {
     float two_krf, krf, crf;
     float lj_sh6, lj_sh12;  // rc^-6, rc^-12 if potential-shift else 0
     int ntypes1;          // ntypes + 1 (row length of the padded LJ table)
-    float ewp[6];         // beta^3 * P_k of the Ewald correction fit (numerator carries beta^3)
+    // Ewald correction fit as polynomials in r^2 (beta folded in), every coefficient duplicated
+    // for the packed FFMA2 form: ewp2[k] = beta^(3+2k) P_k, ewq2[k] = beta^(2k) Q_k.
+    float2 ewp2[6], ewq2[6];
 };
 
 struct nb_ctx {
@@ -71,6 +73,7 @@ struct nb_ctx {
     int natoms = 0, ntypes = 0;
     NbConst kc;
     float beta = 0.f;
+    double beta_d = 0.0;                       // Ewald beta in fp64 (coefficient folding)
 
     // --- state machine ---
     bool have_atoms = false, have_grid = false, have_list = false, atoms_since_search = false;
@@ -124,7 +127,14 @@ struct nb_ctx {
     // --- work units (a5) ---
     std::vector<int4> h_units;
     DevBuf<int4> units_canon, units_sorted;    // {entry slot, batch begin, batch end, sci}
+    DevBuf<int32_t> unit_order;                // canonical unit index, longest first (force kernel launch order)
     int nunits = 0;
+
+    // --- compact inner list (a6 -> a7): per (work unit, i-cluster) the j-clusters whose inner mask bit is set ---
+    DevBuf<int32_t> il_off, ilm_off;           // [nunits*8] first entry of the segment in il / ilm
+    DevBuf<int2> il_cnt;                       // [nunits*8] {unmasked entries (multiple of 4), masked entries}
+    DevBuf<int32_t> il;                        // cj of cluster pairs without a mask for this i-cluster
+    DevBuf<int2> ilm;                          // {cj, mask ref} of cluster pairs with a mask, plus each segment's tail
     DevBuf<double> fshift;                     // [27*3] per-shift i-force sums (virial)
 
     // --- per-stage device timing (nb_timing_enable / nb_timing_read) ---
@@ -183,6 +193,37 @@ __host__ __device__ inline void nb_shift_vec(int id, int& sx, int& sy, int& sz)
 }
 
 int nb_fail(nb_ctx* c, int code, const char* fmt, ...);
+
+#ifdef __CUDACC__
+// Writes the compact inner list segment of (unit, i-cluster warp) from the unit's inner mask
+// words `bits_of(b)` (b = batch index relative to the unit).  Entries whose exclusion mask is
+// trivial for this i-cluster go to `il` (cj only), the others to `ilm` {cj, mask ref}; the last
+// (count mod 4) unmasked entries are moved to `ilm` with ref 0 (the all-ones mask) so that the
+// force kernel's unmasked steps are always full.  One warp, all 32 lanes.
+template <typename BitsOf>
+__device__ __forceinline__ void nb_ilist_write(BitsOf bits_of, int b0, int b1, int warp, int lane,
+                                               const uint32_t* __restrict__ plane_excl, const int2* __restrict__ jl,
+                                               int32_t* __restrict__ il, int2* __restrict__ ilm, int2* __restrict__ cnt)
+{
+    const unsigned lt = (1u << lane) - 1u;
+    int nu = 0, nm = 0;
+    for (int b = b0; b < b1; b++) {
+        const unsigned bits = bits_of(b - b0);
+        const unsigned eb = plane_excl[(size_t)b * 8 + warp] & bits, nb = bits & ~eb;
+        if ((bits >> lane) & 1u) {
+            const int2 e = jl[(size_t)b * 32 + lane];
+            if ((nb >> lane) & 1u) il[nu + __popc(nb & lt)] = e.x;
+            else ilm[nm + __popc(eb & lt)] = e;
+        }
+        nu += __popc(nb);
+        nm += __popc(eb);
+    }
+    __syncwarp();
+    const int rem = nu & 3, nu4 = nu - rem;
+    if (lane < rem) ilm[nm + lane] = make_int2(il[nu4 + lane], 0);
+    if (lane == 0) *cnt = make_int2(nu4, nm + rem);
+}
+#endif
 
 #define NB_CUDA(c, expr)                                                                              \
     do {                                                                                              \

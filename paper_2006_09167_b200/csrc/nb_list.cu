@@ -312,6 +312,37 @@ __global__ void k_excl_planes(const int2* __restrict__ jl, const unsigned long l
     if (lane < 8) plane_excl[b * 8 + lane] = mine;
 }
 
+// ---------------------------------------------------------------- compact inner list (nb_internal.h)
+// Segment capacities per (work unit, i-cluster): every outer cluster pair can survive a prune.
+__global__ void k_ilist_caps(const int4* __restrict__ units, int nunits, const uint32_t* __restrict__ plane_outer,
+                             const uint32_t* __restrict__ plane_excl, int* __restrict__ capu, int* __restrict__ capm)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nunits * 8) return;
+    const int4 u = units[i >> 3];
+    const int w = i & 7;
+    int nu = 0, nm = 0;
+    for (int b = u.y; b < u.z; b++) {
+        const unsigned bits = plane_outer[(size_t)b * 8 + w], eb = plane_excl[(size_t)b * 8 + w] & bits;
+        nu += __popc(bits & ~eb);
+        nm += __popc(eb);
+    }
+    capu[i] = (nu + 3) & ~3;
+    capm[i] = nm + 3;
+}
+
+// inner := the given planes (after a search: the outer ones).  One block per work unit.
+__global__ void __launch_bounds__(256) k_ilist_build(const int4* __restrict__ units, const uint32_t* __restrict__ plane,
+                                                     const uint32_t* __restrict__ plane_excl, const int2* __restrict__ jl,
+                                                     const int* __restrict__ il_off, const int* __restrict__ ilm_off,
+                                                     int2* __restrict__ il_cnt, int32_t* __restrict__ il, int2* __restrict__ ilm)
+{
+    const int4 u = units[blockIdx.x];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, seg = blockIdx.x * 8 + warp;
+    nb_ilist_write([&](int b) { return plane[(size_t)(u.y + b) * 8 + warp]; }, u.y, u.z, warp, lane, plane_excl, jl,
+                   il + il_off[seg], ilm + ilm_off[seg], &il_cnt[seg]);
+}
+
 // ---------------------------------------------------------------- introspection
 __global__ void k_count_bits(const uint32_t* __restrict__ plane, long long nwords, long long* __restrict__ out)
 {
@@ -509,6 +540,11 @@ int nbi_search(nb_ctx* c, float rlist)
     std::vector<int4> sorted(c->h_units);
     std::stable_sort(sorted.begin(), sorted.end(),
                      [](const int4& a, const int4& b) { return (a.z - a.y) > (b.z - b.y); });
+    std::vector<int32_t> order(c->nunits);
+    for (int i = 0; i < c->nunits; i++) order[i] = i;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
+        return (c->h_units[a].z - c->h_units[a].y) > (c->h_units[b].z - c->h_units[b].y);
+    });
 
     NB_CUDA(c, c->jl.ensure(std::max<int64_t>(c->njslots, 1), st));
     NB_CUDA(c, c->imask_outer.ensure(std::max<int64_t>(c->njslots, 1), st));
@@ -518,6 +554,7 @@ int nbi_search(nb_ctx* c, float rlist)
     NB_CUDA(c, c->batch_ent.ensure(std::max<int64_t>(c->nbatch, 1) * 2, st));
     NB_CUDA(c, c->units_canon.ensure(std::max(c->nunits, 1), st));
     NB_CUDA(c, c->units_sorted.ensure(std::max(c->nunits, 1), st));
+    NB_CUDA(c, c->unit_order.ensure(std::max(c->nunits, 1), st));
     NB_CUDA(c, c->scan_tmp.ensure(std::max<int64_t>(c->njslots, 1) * 2 + 8, st));
     NB_CUDA(c, cudaMemcpyAsync(c->ent_jbegin.p, c->h_ent_jbegin.data(), sizeof(int) * (c->nent + 1), cudaMemcpyHostToDevice, st));
     int* d_batch_unit = c->batch_ent.p + std::max<int64_t>(c->nbatch, 1);
@@ -526,6 +563,7 @@ int nbi_search(nb_ctx* c, float rlist)
         NB_CUDA(c, cudaMemcpyAsync(d_batch_unit, h_batch_unit.data(), sizeof(int) * c->nbatch, cudaMemcpyHostToDevice, st));
         NB_CUDA(c, cudaMemcpyAsync(c->units_canon.p, c->h_units.data(), sizeof(int4) * c->nunits, cudaMemcpyHostToDevice, st));
         NB_CUDA(c, cudaMemcpyAsync(c->units_sorted.p, sorted.data(), sizeof(int4) * c->nunits, cudaMemcpyHostToDevice, st));
+        NB_CUDA(c, cudaMemcpyAsync(c->unit_order.p, order.data(), sizeof(int) * c->nunits, cudaMemcpyHostToDevice, st));
         NB_CUDA(c, cudaMemsetAsync(c->imask_outer.p, 0, c->njslots, st));
         k_init_jl<<<(unsigned)((c->njslots + 255) / 256), 256, 0, st>>>(c->jl.p, c->njslots);
         NB_LAUNCH_CHECK(c);
@@ -573,6 +611,27 @@ int nbi_search(nb_ctx* c, float rlist)
             NB_LAUNCH_CHECK(c);
         }
         k_excl_planes<<<(unsigned)((c->nbatch * 32 + 255) / 256), 256, 0, st>>>(c->jl.p, c->excl_masks.p, c->plane_excl.p, c->nbatch);
+        NB_LAUNCH_CHECK(c);
+        // compact inner list: segment offsets from the outer counts, then inner := outer
+        const int nseg = c->nunits * 8;
+        NB_CUDA(c, c->il_off.ensure(nseg, st));
+        NB_CUDA(c, c->ilm_off.ensure(nseg, st));
+        NB_CUDA(c, c->il_cnt.ensure(nseg, st));
+        int* capu = c->scan_tmp.p;
+        int* capm = c->scan_tmp.p + nseg;
+        k_ilist_caps<<<(nseg + 255) / 256, 256, 0, st>>>(c->units_canon.p, c->nunits, c->plane_outer.p, c->plane_excl.p, capu, capm);
+        NB_LAUNCH_CHECK(c);
+        rc = nbi_exclusive_scan(c, capu, c->il_off.p, nseg, total_dev);
+        if (rc != NB_OK) return rc;
+        rc = nbi_exclusive_scan(c, capm, c->ilm_off.p, nseg, total_dev + 1);
+        if (rc != NB_OK) return rc;
+        int tot[2] = {0, 0};
+        NB_CUDA(c, cudaMemcpyAsync(tot, total_dev, sizeof(tot), cudaMemcpyDeviceToHost, st));
+        NB_CUDA(c, cudaStreamSynchronize(st));
+        NB_CUDA(c, c->il.ensure((size_t)tot[0] + 4, st));
+        NB_CUDA(c, c->ilm.ensure((size_t)tot[1] + 4, st));
+        k_ilist_build<<<c->nunits, 256, 0, st>>>(c->units_canon.p, c->plane_inner.p, c->plane_excl.p, c->jl.p, c->il_off.p,
+                                                 c->ilm_off.p, c->il_cnt.p, c->il.p, c->ilm.p);
         NB_LAUNCH_CHECK(c);
     } else {
         std::vector<unsigned long long> ones(16, ~0ull);

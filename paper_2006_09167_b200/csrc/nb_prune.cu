@@ -26,6 +26,13 @@ struct PruneArgs {
     const float4* xq;
     float box[3];
     float rl2;   // fl32(rlist_inner^2), reading A12
+    // compact inner list written for the force kernel (nb_internal.h)
+    int u0;      // canonical index of units[0]
+    const uint32_t* plane_excl;
+    const int *il_off, *ilm_off;
+    int2* il_cnt;
+    int32_t* il;
+    int2* ilm;
 };
 
 // 8 exact (A12) distance checks of this lane's j atom; DIAG keeps only pairs b > a.
@@ -123,6 +130,9 @@ __global__ void __launch_bounds__(256) k_prune(PruneArgs A)
     }
     __syncwarp();
     if (lane < u.z - u.y) A.plane_inner[(size_t)(u.y + lane) * 8 + warp] = res[lane];
+    const int seg = (A.u0 + blockIdx.x) * 8 + warp;
+    nb_ilist_write([&](int b) { return res[b]; }, u.y, u.z, warp, lane, A.plane_excl, A.jl, A.il + A.il_off[seg],
+                   A.ilm + A.ilm_off[seg], &A.il_cnt[seg]);
 }
 
 }  // namespace
@@ -142,6 +152,10 @@ int nbi_prune(nb_ctx* c, float rlist_inner, int part, int nparts)
     A.xq = c->xq.p;
     for (int k = 0; k < 3; k++) A.box[k] = c->box[k];
     A.rl2 = rlist_inner * rlist_inner;
+    A.u0 = u0;
+    A.plane_excl = c->plane_excl.p;
+    A.il_off = c->il_off.p; A.ilm_off = c->ilm_off.p; A.il_cnt = c->il_cnt.p;
+    A.il = c->il.p; A.ilm = c->ilm.p;
     NbStageTimer tm(c, NB_T_PRUNE);
     k_prune<<<u1 - u0, 256, 0, c->stream>>>(A);
     NB_LAUNCH_CHECK(c);
