@@ -2,6 +2,7 @@
 // preparation and memory ownership.  All arithmetic of the method lives in the kernels of
 // nb_grid.cu / nb_list.cu / nb_prune.cu / nb_force.cu.  Links the CUDA runtime only.
 #include "nb_internal.h"
+#include "ewald_corr_coeffs.h"
 
 #include <math.h>
 #include <stdarg.h>
@@ -56,7 +57,8 @@ extern "C" int nb_init(const nb_params* p, nb_ctx** out)
             }
             beta = 0.5 * (lo + hi);
         }
-        if (beta * rc * beta * rc > 16.0) return nb_fail(c, NB_ERR_ARG, "(beta*rc)^2 = %g exceeds 16, the range of the Ewald correction fit", beta * rc * beta * rc);
+        if (beta * rc * beta * rc > (double)NB_EWALD_ZMAX)
+            return nb_fail(c, NB_ERR_ARG, "(beta*rc)^2 = %g exceeds %g, the range of the Ewald correction fit", beta * rc * beta * rc, (double)NB_EWALD_ZMAX);
     }
     NbConst& K = c->kc;
     memset(&K, 0, sizeof(K));
@@ -205,7 +207,7 @@ extern "C" void nb_free(nb_ctx* c)
     c->plane_outer.release(); c->plane_inner.release(); c->plane_excl.release(); c->batch_ent.release(); c->scan_tmp.release();
     c->scan_blk.release(); c->excl_masks.release(); c->counters.release(); c->units_canon.release();
     c->units_sorted.release(); c->fshift.release(); c->unit_order.release();
-    c->il_off.release(); c->ilm_off.release(); c->il_cnt.release(); c->il.release(); c->ilm.release();
+    c->il_off.release(); c->ilm_off.release(); c->seg.release(); c->unit_pos.release(); c->il.release(); c->ilm.release();
     delete c;
 }
 

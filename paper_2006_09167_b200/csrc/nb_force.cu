@@ -22,17 +22,14 @@
 namespace {
 
 struct ForceArgs {
-    const int4* units;          // canonical work units {entry slot, batch begin, batch end, sci}
-    const int* unit_order;      // launch order (longest first) -> canonical unit index; nullptr = identity
+    const int4* units;          // work units {entry slot, batch begin, batch end, sci}: launch order (k_force), canonical (k_count_pairs)
     const int2* jl;
     const uint32_t* plane;
     const float4* xq;
     const int* type_slot;
     const float2* ljtab;
     const unsigned long long* masks;
-    const int* il_off;          // compact inner list, see nb_internal.h
-    const int* ilm_off;
-    const int2* il_cnt;
+    const int4* seg;            // compact inner list, see nb_internal.h
     const int* il;
     const int2* ilm;
     float4* f4;
@@ -48,11 +45,21 @@ __device__ __forceinline__ void red_add_v4(float4* addr, float x, float y, float
 }
 
 // Single-instruction MUFU forms: the arguments are clamped away from zero/denormals by the
-// caller (r^2 >= 1e-6, Q(z) >= 1), so the denormal fix-up code of rsqrtf()/__fdividef() is dead weight.
+// caller (r^2 >= 1e-6 or distinct atoms, monic Q(r^2) >= 1/30), so the denormal fix-up code of rsqrtf()/__fdividef() is dead weight.
+__device__ __forceinline__ void prefetch_l1(const void* p)
+{
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
+}
 __device__ __forceinline__ float rsqrt_fast(float x)
 {
     float y;
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float fma_sat(float a, float b, float c)
+{
+    float y;
+    asm("fma.rn.sat.f32 %0, %1, %2, %3;" : "=f"(y) : "f"(a), "f"(b), "f"(c));
     return y;
 }
 __device__ __forceinline__ float rcp_fast(float x)
@@ -73,12 +80,14 @@ __device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a
 __device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
 __device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
 
-// beta^3 h(z) for two pairs, as P5(r^2)/Q5(r^2) with beta folded into the coefficients.
-__device__ __forceinline__ float2 ewald_bh2(float2 r2, const NbConst& K)
+// beta^3 h(z) for two pairs, as P4(r^2)/Q5(r^2) with beta folded into the coefficients and Q made
+// monic (P divided by Q's leading coefficient): Q's first Horner step is then an FADD2 with one
+// constant operand, and P's first step takes its addend from a register pair (p3) kept by the
+// caller -- an FFMA2 cannot take two constant-bank operands, ptxas would rebuild them with MOVs.
+__device__ __forceinline__ float2 ewald_bh2(float2 r2, const NbConst& K, const float2 p3)
 {
-    float2 p = fma2(K.ewp2[5], r2, K.ewp2[4]);
-    float2 q = fma2(K.ewq2[5], r2, K.ewq2[4]);
-    p = fma2(p, r2, K.ewp2[3]);
+    float2 p = fma2(K.ewp2[4], r2, p3);
+    float2 q = add2(r2, K.ewq2[4]);
     q = fma2(q, r2, K.ewq2[3]);
     p = fma2(p, r2, K.ewp2[2]);
     q = fma2(q, r2, K.ewq2[2]);
@@ -103,7 +112,7 @@ template <int COUL, bool ENERGY, bool MASKED>
 __device__ __forceinline__ void pair_step(const NbConst& K, const float4* __restrict__ ljj, const int ljs, const IAtoms& I,
                                           float2 (&fix)[4], float2 (&fiy)[4], float2 (&fiz)[4], float& elj, float& ecoul,
                                           const float4 xj, unsigned cbyte, unsigned mbyte, float2& fjx, float2& fjy,
-                                          float2& fjz)
+                                          float2& fjz, const float2 p3)
 {
     const float2 nxj = f2(-xj.x), nyj = f2(-xj.y), nzj = f2(-xj.z), qj = f2(xj.w);
     fjx = f2(0.f); fjy = f2(0.f); fjz = f2(0.f);
@@ -111,12 +120,19 @@ __device__ __forceinline__ void pair_step(const NbConst& K, const float4* __rest
     for (int p = 0; p < 4; p++) {
         const float2 dx = add2(I.x[p], nxj), dy = add2(I.y[p], nyj), dz = add2(I.z[p], nzj);
         const float2 r2u = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
-        bool w0 = r2u.x < K.rc2, w1 = r2u.y < K.rc2;        // A7: strict
+        // A7: interact iff r^2 < rc^2 (strict).  MASKED steps select with predicates and clamp r^2 so
+        // that self pairs stay finite; unmasked steps have no r = 0 pairs (padding atoms sit at
+        // distinct finite positions, nb_grid.cu) and multiply by w = sat((rc^2 - r^2) 2^60), which
+        // is exactly 1 or 0 and costs FP32-pipe slots instead of the half-rate ALU pipe.
+        bool w0 = true, w1 = true;
+        float2 r2 = r2u, wc = f2(1.f);
         if (MASKED) {
-            w0 = w0 && ((cbyte >> (2 * p)) & 1u);
-            w1 = w1 && ((cbyte >> (2 * p + 1)) & 1u);
+            w0 = r2u.x < K.rc2 && ((cbyte >> (2 * p)) & 1u);
+            w1 = r2u.y < K.rc2 && ((cbyte >> (2 * p + 1)) & 1u);
+            r2 = f2(fmaxf(r2u.x, 1e-6f), fmaxf(r2u.y, 1e-6f));
+        } else {
+            wc = f2(fma_sat(r2u.x, -K.cut_big, K.cut_rc2big), fma_sat(r2u.y, -K.cut_big, K.cut_rc2big));
         }
-        const float2 r2 = f2(fmaxf(r2u.x, 1e-6f), fmaxf(r2u.y, 1e-6f));   // keeps masked / padding pairs finite
         const float2 rinv = f2(rsqrt_fast(r2.x), rsqrt_fast(r2.y));
         const float2 rinv2 = mul2(rinv, rinv);
         const float4 c = ljj[p * ljs];                        // (-6 c6_a, -6 c6_b, 12 c12_a, 12 c12_b)
@@ -132,12 +148,13 @@ __device__ __forceinline__ void pair_step(const NbConst& K, const float4* __rest
         }
         float2 fs, bh = f2(0.f);
         if (COUL == NB_COUL_EWALD) {
-            bh = ewald_bh2(r2, K);
+            bh = ewald_bh2(r2, K, p3);
             fs = fma2(rinv2, t1, neg2(mul2(qq, bh)));         // F/r = (F_lj r + A m/r)/r^2 - A beta^3 h
         } else {
             fs = fma2(rinv2, t1, neg2(mul2(qq, f2(K.two_krf))));   // F/r = ... - 2 A k_rf
         }
-        fs = f2(w0 ? fs.x : 0.f, w1 ? fs.y : 0.f);
+        if (MASKED) fs = f2(w0 ? fs.x : 0.f, w1 ? fs.y : 0.f);
+        else fs = mul2(fs, wc);
         fix[p] = fma2(fs, dx, fix[p]);
         fiy[p] = fma2(fs, dy, fiy[p]);
         fiz[p] = fma2(fs, dz, fiz[p]);
@@ -157,7 +174,8 @@ __device__ __forceinline__ void pair_step(const NbConst& K, const float4* __rest
             } else {
                 vc = mul2(qq, fma2(mf, rinv, fma2(f2(K.krf), r2, f2(-K.crf))));
             }
-            const float2 vl = mul2(mf, vlj);
+            const float2 vl = mul2(mul2(mf, vlj), wc);
+            vc = mul2(vc, wc);
             elj += (w0 ? vl.x : 0.f) + (w1 ? vl.y : 0.f);
             ecoul += (w0 ? vc.x : 0.f) + (w1 ? vc.y : 0.f);
         }
@@ -172,16 +190,28 @@ __global__ void __launch_bounds__(256, 2) k_force(ForceArgs A)
     extern __shared__ float4 s_ljp[];
     const NbConst& K = A.kc;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7;
-    const int uidx = A.unit_order ? A.unit_order[blockIdx.x] : blockIdx.x;
-    const int4 u = A.units[uidx];
+    const int4 u = A.units[blockIdx.x];
+    const int4 sg = A.seg[blockIdx.x * 8 + warp];
     const int sci = u.w, h = u.x - sci * NB_NHALF, ci = sci * 8 + warp;
     const int sid = nb_half_shift_id(h);
     const int nt1 = K.ntypes1;
-    for (int i = threadIdx.x; i < 32 * nt1; i += blockDim.x) {
-        const int wp = i / nt1, tj = i - wp * nt1;
-        const int ta = A.type_slot[sci * NB_SC_ATOMS + 2 * wp], tb = A.type_slot[sci * NB_SC_ATOMS + 2 * wp + 1];
+    // each warp builds its own part of the table: no block-level barrier
+    float4* ljw = s_ljp + warp * 4 * nt1;
+    for (int i = lane; i < 4 * nt1; i += 32) {
+        const int p = i / nt1, tj = i - p * nt1;
+        const int ta = A.type_slot[ci * 8 + 2 * p], tb = A.type_slot[ci * 8 + 2 * p + 1];
         const float2 ca = A.ljtab[ta * nt1 + tj], cb = A.ljtab[tb * nt1 + tj];
-        s_ljp[i] = make_float4(-ca.x, -cb.x, ca.y, cb.y);
+        ljw[i] = make_float4(-ca.x, -cb.x, ca.y, cb.y);
+    }
+    const int2 cnt = make_int2(sg.z, sg.w);
+    const int* __restrict__ il = A.il + sg.x;
+    const int2* __restrict__ ilm = A.ilm + sg.y;
+    const int ns = cnt.x >> 2;
+    // first list entries of both loops are requested before anything else is waited for
+    int cj = 0, cj_n = 0;
+    if (ns > 0) {
+        cj = il[g];
+        cj_n = il[4 * min(1, ns - 1) + g];
     }
     int sx, sy, sz;
     nb_shift_vec(sid, sx, sy, sz);
@@ -198,47 +228,50 @@ __global__ void __launch_bounds__(256, 2) k_force(ForceArgs A)
 #pragma unroll
     for (int p = 0; p < 4; p++) { fix[p] = f2(0.f); fiy[p] = f2(0.f); fiz[p] = f2(0.f); }
     float elj = 0.f, ecoul = 0.f;
-    const int seg = uidx * 8 + warp;
-    const int2 cnt = A.il_cnt[seg];
-    const int* __restrict__ il = A.il + A.il_off[seg];
-    const int2* __restrict__ ilm = A.ilm + A.ilm_off[seg];
-    const float4* ljw = s_ljp + warp * 4 * nt1;
-    __syncthreads();
-
-    // Cluster pairs without a mask: always full steps of 4 j-clusters; the j data of step s+1 and
-    // the list entries of step s+2 are requested before the arithmetic of step s.
-    const int ns = cnt.x >> 2;
-    if (ns > 0) {
-        int cj = il[g];
-        int cj_n = ns > 1 ? il[4 + g] : cj;
-        float4 xj = A.xq[cj * 8 + k];
-        int tj = A.type_slot[cj * 8 + k];
-        for (int s = 0; s < ns; s++) {
-            float4 xj_n = xj;
-            int tj_n = tj, cj_nn = cj_n;
-            if (s + 1 < ns) {
-                xj_n = A.xq[cj_n * 8 + k];
-                tj_n = A.type_slot[cj_n * 8 + k];
-            }
-            if (s + 2 < ns) cj_nn = il[4 * (s + 2) + g];
-            float2 fjx, fjy, fjz;
-            pair_step<COUL, ENERGY, false>(K, ljw + tj, nt1, I, fix, fiy, fiz, elj, ecoul, xj, 0xffu, 0xffu, fjx, fjy, fjz);
-            red_add_v4(&A.f4[cj * 8 + k], -(fjx.x + fjx.y), -(fjy.x + fjy.y), -(fjz.x + fjz.y));
-            cj = cj_n; cj_n = cj_nn; xj = xj_n; tj = tj_n;
-        }
+    const float2 p3 = K.ewp2[3];
+    float4 xj = make_float4(0.f, 0.f, 0.f, 0.f);
+    int tj = 0;
+    if (ns > 0) {   // j data of the first unmasked step: in flight during the masked steps
+        xj = A.xq[cj * 8 + k];
+        tj = A.type_slot[cj * 8 + k];
     }
+    __syncwarp();
+
     // Cluster pairs with exclusion / self / diagonal masks, and the segment's tail (ref 0 = all ones).
     for (int s = 0; s < cnt.y; s += 4) {
         const bool valid = s + g < cnt.y;
         const int2 ce = valid ? ilm[s + g] : make_int2(ci, 0);
-        const float4 xj = A.xq[ce.x * 8 + k];
-        const int tj = A.type_slot[ce.x * 8 + k];
+        const float4 xm = A.xq[ce.x * 8 + k];
+        const int tm = A.type_slot[ce.x * 8 + k];
         const ulonglong2 mm = *reinterpret_cast<const ulonglong2*>(&A.masks[((size_t)ce.y * 8 + warp) * 2]);
         const unsigned cbyte = valid ? (unsigned)(mm.y >> (8 * k)) & 0xffu : 0u;
         const unsigned mbyte = (unsigned)(mm.x >> (8 * k)) & cbyte;
         float2 fjx, fjy, fjz;
-        pair_step<COUL, ENERGY, true>(K, ljw + tj, nt1, I, fix, fiy, fiz, elj, ecoul, xj, cbyte, mbyte, fjx, fjy, fjz);
+        pair_step<COUL, ENERGY, true>(K, ljw + tm, nt1, I, fix, fiy, fiz, elj, ecoul, xm, cbyte, mbyte, fjx, fjy, fjz, p3);
         if (valid) red_add_v4(&A.f4[ce.x * 8 + k], -(fjx.x + fjx.y), -(fjy.x + fjy.y), -(fjz.x + fjz.y));
+    }
+
+    // Cluster pairs without a mask: always full steps of 4 j-clusters.  ptxas schedules memory
+    // operations whose consumer is an iteration away at the END of the step, so the j data of
+    // step s+1 is loaded there; to make that load an L1 hit the lines are prefetched one step
+    // earlier still (distance 2), and the list entries are read 3 steps ahead (indices clamped).
+    int cj_nn = 0;
+    if (ns > 0) {
+        cj_nn = il[4 * min(2, ns - 1) + g];
+        prefetch_l1(&A.xq[cj_n * 8 + k]);
+        prefetch_l1(&A.type_slot[cj_n * 8 + k]);
+    }
+#pragma unroll 2
+    for (int s = 0; s < ns; s++) {
+        const int cj_3 = il[4 * min(s + 3, ns - 1) + g];
+        prefetch_l1(&A.xq[cj_nn * 8 + k]);
+        prefetch_l1(&A.type_slot[cj_nn * 8 + k]);
+        float2 fjx, fjy, fjz;
+        pair_step<COUL, ENERGY, false>(K, ljw + tj, nt1, I, fix, fiy, fiz, elj, ecoul, xj, 0xffu, 0xffu, fjx, fjy, fjz, p3);
+        red_add_v4(&A.f4[cj * 8 + k], -(fjx.x + fjx.y), -(fjy.x + fjy.y), -(fjz.x + fjz.y));
+        cj = cj_n; cj_n = cj_nn; cj_nn = cj_3;
+        xj = A.xq[cj * 8 + k];        // L1 hit: prefetched a step ago
+        tj = A.type_slot[cj * 8 + k];
     }
 
     float fi[24];
@@ -438,13 +471,10 @@ int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial)
 {
     cudaStream_t st = c->stream;
     ForceArgs A;
-    A.units = c->units_canon.p;
-    A.unit_order = c->unit_order.p;
+    A.units = c->units_sorted.p;
     A.jl = c->jl.p;
     A.plane = c->plane_inner.p;
-    A.il_off = c->il_off.p;
-    A.ilm_off = c->ilm_off.p;
-    A.il_cnt = c->il_cnt.p;
+    A.seg = c->seg.p;
     A.il = c->il.p;
     A.ilm = c->ilm.p;
     A.xq = c->xq.p;
@@ -455,14 +485,17 @@ int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial)
     A.kc = c->kc;
     for (int k = 0; k < 3; k++) A.kc.box[k] = c->box[k];
     {
-        const double P[6] = {NB_EWC_P0, NB_EWC_P1, NB_EWC_P2, NB_EWC_P3, NB_EWC_P4, NB_EWC_P5};
+        const double P[5] = {NB_EWC_P0, NB_EWC_P1, NB_EWC_P2, NB_EWC_P3, NB_EWC_P4};
         const double Q[6] = {NB_EWC_Q0, NB_EWC_Q1, NB_EWC_Q2, NB_EWC_Q3, NB_EWC_Q4, NB_EWC_Q5};
         const double b = c->beta_d, b2 = b * b;
         double bk = 1.0;   // beta^(2k)
+        const double qlead = b2 * b2 * b2 * b2 * b2 * Q[5];   // Q is made monic in r^2
         for (int k = 0; k < 6; k++, bk *= b2) {
-            A.kc.ewp2[k] = make_float2((float)(b * b2 * bk * P[k]), (float)(b * b2 * bk * P[k]));
-            A.kc.ewq2[k] = make_float2((float)(bk * Q[k]), (float)(bk * Q[k]));
+            if (k < 5) A.kc.ewp2[k] = make_float2((float)(b * b2 * bk * P[k] / qlead), (float)(b * b2 * bk * P[k] / qlead));
+            A.kc.ewq2[k] = make_float2((float)(bk * Q[k] / qlead), (float)(bk * Q[k] / qlead));
         }
+        A.kc.cut_big = 1.152921504606846976e18f;              // 2^60: products with it are exact
+        A.kc.cut_rc2big = A.kc.rc2 * 1.152921504606846976e18f;
     }
     NB_CUDA(c, c->fshift.ensure(NB_NSHIFT * 3 + 9, st));
     A.fshift = c->fshift.p;

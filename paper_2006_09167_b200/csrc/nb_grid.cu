@@ -146,7 +146,7 @@ k_col_layout(int ncy, const int* __restrict__ col_atom_off, const int* __restric
              const int* __restrict__ type, int pad_type, int np2_max, float4* __restrict__ xq,
              int* __restrict__ type_slot, int* __restrict__ atom_of_slot, int* __restrict__ slot_of_atom,
              float4* __restrict__ bb_lo, float4* __restrict__ bb_hi, float4* __restrict__ sbb_lo,
-             float4* __restrict__ sbb_hi)
+             float4* __restrict__ sbb_hi, float3 pad_base, float3 pad_step)
 {
     extern __shared__ unsigned long long s_keys[];
     __shared__ SlabScratch s_slab[8];
@@ -204,10 +204,14 @@ k_col_layout(int ncy, const int* __restrict__ col_atom_off, const int* __restric
                 v = xw_atom[a];
                 slot_of_atom[a] = slot;
             } else {
-                // padding: far away, distinct per (slot, column); zero charge, zero-LJ type
+                // padding (reading A11): zero charge, zero-LJ type, outside every cut-off of every
+                // real atom under every shift (x < -(2 Lx + 8)), distinct per (slot, column mod 64)
+                // with a spacing d_k chosen so that L_k / d_k is a half-integer: two padding atoms
+                // never coincide under any shift, and all distances stay small enough (< ~1e3 nm)
+                // for the force kernel's arithmetic to remain finite without a clamp.
                 int cx = col / ncy, cy = col % ncy;
-                v = make_float4(1.0e4f + 61.803f * (float)e, 1.0e4f + 61.803f * (float)cy,
-                                -1.0e4f - 61.803f * (float)cx, 0.f);
+                v = make_float4(pad_base.x - pad_step.x * (float)e, pad_base.y - pad_step.y * (float)(cy & 63),
+                                pad_base.z - pad_step.z * (float)(cx & 63), 0.f);
             }
             xq[slot] = v;
             type_slot[slot] = real ? type[a] : pad_type;
@@ -324,21 +328,40 @@ int nbi_grid(nb_ctx* c)
     if (smem > 200 * 1024)
         return nb_fail(c, NB_ERR_OVERFLOW, "grid column holds %d atoms; the in-shared-memory z-sort takes at most 25600",
                        c->max_col_count);
-    NB_CUDA(c, c->xq.ensure(c->nslots, st));
-    NB_CUDA(c, c->type_slot.ensure(c->nslots, st));
+    NB_CUDA(c, c->xq.ensure(c->nslots + NB_C, st));          // + one dummy cluster (index nclusters), see below
+    NB_CUDA(c, c->type_slot.ensure(c->nslots + NB_C, st));
     NB_CUDA(c, c->atom_of_slot.ensure(c->nslots, st));
     NB_CUDA(c, c->bb_lo.ensure(c->nclusters, st));
     NB_CUDA(c, c->bb_hi.ensure(c->nclusters, st));
     NB_CUDA(c, c->sbb_lo.ensure(c->nsc, st));
     NB_CUDA(c, c->sbb_hi.ensure(c->nsc, st));
-    NB_CUDA(c, c->f4.ensure(c->nslots, st));
+    NB_CUDA(c, c->f4.ensure(c->nslots + NB_C, st));
     NB_CUDA(c, cudaMemsetAsync(c->f4.p, 0, sizeof(float4) * c->nslots, st));
     NB_CUDA(c, cudaFuncSetAttribute(k_col_layout, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    float pb[3], pd[3];
+    for (int k = 0; k < 3; k++) {
+        pd[k] = (float)(L[k] / (floor(L[k] / 3.0) + 0.5));   // L/d half-integer, d in (2, 6] nm (2L for L < 3)
+        pb[k] = (float)(-(2.0 * L[k] + 8.0));
+    }
     k_col_layout<<<c->ncol, 256, smem, st>>>(c->ncy, c->col_atom_off.p, c->col_sc_off.p, c->col_atoms.p,
                                              c->xw_atom.p, c->type.p, c->ntypes, np2, c->xq.p, c->type_slot.p,
                                              c->atom_of_slot.p, c->slot_of_atom.p, c->bb_lo.p, c->bb_hi.p,
-                                             c->sbb_lo.p, c->sbb_hi.p);
+                                             c->sbb_lo.p, c->sbb_hi.p, make_float3(pb[0], pb[1], pb[2]),
+                                             make_float3(pd[0], pd[1], pd[2]));
     NB_LAUNCH_CHECK(c);
+    {
+        // Dummy j-cluster (index nclusters): padding-like atoms beyond the padding lattice; interacts
+        // with nothing.  Available to kernels that need a harmless list entry.
+        float4 hx[NB_C];
+        int32_t ht[NB_C];
+        for (int k = 0; k < NB_C; k++) {
+            hx[k] = make_float4(pb[0] - pd[0] * (float)(64 + k), pb[1], pb[2], 0.f);
+            ht[k] = c->ntypes;
+        }
+        NB_CUDA(c, cudaMemcpyAsync(c->xq.p + c->nslots, hx, sizeof(hx), cudaMemcpyHostToDevice, st));
+        NB_CUDA(c, cudaMemcpyAsync(c->type_slot.p + c->nslots, ht, sizeof(ht), cudaMemcpyHostToDevice, st));
+        NB_CUDA(c, cudaStreamSynchronize(st));
+    }
     c->grid_box[0] = L[0];
     c->grid_box[1] = L[1];
     c->grid_box[2] = L[2];

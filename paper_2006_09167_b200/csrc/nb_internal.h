@@ -63,7 +63,8 @@ struct NbConst {
     int ntypes1;          // ntypes + 1 (row length of the padded LJ table)
     // Ewald correction fit as polynomials in r^2 (beta folded in), every coefficient duplicated
     // for the packed FFMA2 form: ewp2[k] = beta^(3+2k) P_k, ewq2[k] = beta^(2k) Q_k.
-    float2 ewp2[6], ewq2[6];
+    float2 ewp2[5], ewq2[6];
+    float cut_big, cut_rc2big;   // 2^60 and rc^2 2^60: w = sat(rc2big - r2 big) is 1 inside the cut-off, else 0
 };
 
 struct nb_ctx {
@@ -131,8 +132,10 @@ struct nb_ctx {
     int nunits = 0;
 
     // --- compact inner list (a6 -> a7): per (work unit, i-cluster) the j-clusters whose inner mask bit is set ---
-    DevBuf<int32_t> il_off, ilm_off;           // [nunits*8] first entry of the segment in il / ilm
-    DevBuf<int2> il_cnt;                       // [nunits*8] {unmasked entries (multiple of 4), masked entries}
+    DevBuf<int32_t> il_off, ilm_off;           // [nunits*8] scan scratch: first entry of the segment in il / ilm
+    DevBuf<int4> seg;                          // [nunits*8], index = launch position*8 + i-cluster:
+                                               // {il offset, ilm offset, unmasked entries (multiple of 4), masked entries}
+    DevBuf<int32_t> unit_pos;                  // canonical unit index -> launch position (inverse of unit_order)
     DevBuf<int32_t> il;                        // cj of cluster pairs without a mask for this i-cluster
     DevBuf<int2> ilm;                          // {cj, mask ref} of cluster pairs with a mask, plus each segment's tail
     DevBuf<double> fshift;                     // [27*3] per-shift i-force sums (virial)
@@ -199,9 +202,10 @@ int nb_fail(nb_ctx* c, int code, const char* fmt, ...);
 // words `bits_of(b)` (b = batch index relative to the unit).  Entries whose exclusion mask is
 // trivial for this i-cluster go to `il` (cj only), the others to `ilm` {cj, mask ref}; the last
 // (count mod 4) unmasked entries are moved to `ilm` with ref 0 (the all-ones mask) so that the
-// force kernel's unmasked steps are always full.  One warp, all 32 lanes.
+// force kernel's unmasked steps are always full (padding them with the dummy cluster `cj_dummy`
+// instead was measured slower: one more step per segment).  One warp, all 32 lanes.
 template <typename BitsOf>
-__device__ __forceinline__ void nb_ilist_write(BitsOf bits_of, int b0, int b1, int warp, int lane,
+__device__ __forceinline__ void nb_ilist_write(BitsOf bits_of, int b0, int b1, int warp, int lane, int cj_dummy,
                                                const uint32_t* __restrict__ plane_excl, const int2* __restrict__ jl,
                                                int32_t* __restrict__ il, int2* __restrict__ ilm, int2* __restrict__ cnt)
 {

@@ -335,12 +335,14 @@ __global__ void k_ilist_caps(const int4* __restrict__ units, int nunits, const u
 __global__ void __launch_bounds__(256) k_ilist_build(const int4* __restrict__ units, const uint32_t* __restrict__ plane,
                                                      const uint32_t* __restrict__ plane_excl, const int2* __restrict__ jl,
                                                      const int* __restrict__ il_off, const int* __restrict__ ilm_off,
-                                                     int2* __restrict__ il_cnt, int32_t* __restrict__ il, int2* __restrict__ ilm)
+                                                     int4* __restrict__ seg, int32_t* __restrict__ il, int2* __restrict__ ilm, int cj_dummy)
 {
-    const int4 u = units[blockIdx.x];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, seg = blockIdx.x * 8 + warp;
-    nb_ilist_write([&](int b) { return plane[(size_t)(u.y + b) * 8 + warp]; }, u.y, u.z, warp, lane, plane_excl, jl,
-                   il + il_off[seg], ilm + ilm_off[seg], &il_cnt[seg]);
+    const int4 u = units[blockIdx.x];   // units in launch order
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, s = blockIdx.x * 8 + warp;
+    const int o = il_off[s], om = ilm_off[s];
+    if (lane == 0) { seg[s].x = o; seg[s].y = om; }
+    nb_ilist_write([&](int b) { return plane[(size_t)(u.y + b) * 8 + warp]; }, u.y, u.z, warp, lane, cj_dummy, plane_excl, jl,
+                   il + o, ilm + om, reinterpret_cast<int2*>(&seg[s]) + 1);
 }
 
 // ---------------------------------------------------------------- introspection
@@ -517,7 +519,9 @@ int nbi_search(nb_ctx* c, float rlist)
     // at most `ub` batches of one element; `ub` is chosen so that there are about 16 units per SM.
     int nsm = 148;
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, c->prm.device);
-    int64_t target = (int64_t)16 * nsm;
+    int per_sm = 6;
+    if (const char* e = getenv("NB_UNITS_PER_SM")) per_sm = std::max(1, atoi(e));   // tuning knob
+    int64_t target = (int64_t)per_sm * nsm;
     int ub = (int)std::min<int64_t>(NB_MAX_UNIT_BATCHES, std::max<int64_t>(1, c->nbatch / target));
     c->h_units.clear();
     std::vector<int32_t> h_batch_ent(c->nbatch), h_batch_unit(c->nbatch);
@@ -525,8 +529,9 @@ int nbi_search(nb_ctx* c, float rlist)
         int cnt = c->h_ent_count[e];
         if (!cnt) continue;
         int b0 = c->h_ent_jbegin[e] / NB_BATCH, nb = (cnt + NB_BATCH - 1) / NB_BATCH;
-        for (int b = 0; b < nb; b += ub) {
-            int bend = std::min(nb, b + ub);
+        const int nsplit = (nb + ub - 1) / ub;   // equal-sized chunks of at most ub batches
+        for (int k = 0; k < nsplit; k++) {
+            const int b = (int)((int64_t)nb * k / nsplit), bend = (int)((int64_t)nb * (k + 1) / nsplit);
             for (int bb = b; bb < bend; bb++) {
                 h_batch_ent[b0 + bb] = e;
                 h_batch_unit[b0 + bb] = (int)c->h_units.size();
@@ -540,11 +545,12 @@ int nbi_search(nb_ctx* c, float rlist)
     std::vector<int4> sorted(c->h_units);
     std::stable_sort(sorted.begin(), sorted.end(),
                      [](const int4& a, const int4& b) { return (a.z - a.y) > (b.z - b.y); });
-    std::vector<int32_t> order(c->nunits);
+    std::vector<int32_t> order(c->nunits), pos(c->nunits);
     for (int i = 0; i < c->nunits; i++) order[i] = i;
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
         return (c->h_units[a].z - c->h_units[a].y) > (c->h_units[b].z - c->h_units[b].y);
     });
+    for (int i = 0; i < c->nunits; i++) pos[order[i]] = i;
 
     NB_CUDA(c, c->jl.ensure(std::max<int64_t>(c->njslots, 1), st));
     NB_CUDA(c, c->imask_outer.ensure(std::max<int64_t>(c->njslots, 1), st));
@@ -555,6 +561,7 @@ int nbi_search(nb_ctx* c, float rlist)
     NB_CUDA(c, c->units_canon.ensure(std::max(c->nunits, 1), st));
     NB_CUDA(c, c->units_sorted.ensure(std::max(c->nunits, 1), st));
     NB_CUDA(c, c->unit_order.ensure(std::max(c->nunits, 1), st));
+    NB_CUDA(c, c->unit_pos.ensure(std::max(c->nunits, 1), st));
     NB_CUDA(c, c->scan_tmp.ensure(std::max<int64_t>(c->njslots, 1) * 2 + 8, st));
     NB_CUDA(c, cudaMemcpyAsync(c->ent_jbegin.p, c->h_ent_jbegin.data(), sizeof(int) * (c->nent + 1), cudaMemcpyHostToDevice, st));
     int* d_batch_unit = c->batch_ent.p + std::max<int64_t>(c->nbatch, 1);
@@ -564,6 +571,7 @@ int nbi_search(nb_ctx* c, float rlist)
         NB_CUDA(c, cudaMemcpyAsync(c->units_canon.p, c->h_units.data(), sizeof(int4) * c->nunits, cudaMemcpyHostToDevice, st));
         NB_CUDA(c, cudaMemcpyAsync(c->units_sorted.p, sorted.data(), sizeof(int4) * c->nunits, cudaMemcpyHostToDevice, st));
         NB_CUDA(c, cudaMemcpyAsync(c->unit_order.p, order.data(), sizeof(int) * c->nunits, cudaMemcpyHostToDevice, st));
+        NB_CUDA(c, cudaMemcpyAsync(c->unit_pos.p, pos.data(), sizeof(int) * c->nunits, cudaMemcpyHostToDevice, st));
         NB_CUDA(c, cudaMemsetAsync(c->imask_outer.p, 0, c->njslots, st));
         k_init_jl<<<(unsigned)((c->njslots + 255) / 256), 256, 0, st>>>(c->jl.p, c->njslots);
         NB_LAUNCH_CHECK(c);
@@ -616,10 +624,10 @@ int nbi_search(nb_ctx* c, float rlist)
         const int nseg = c->nunits * 8;
         NB_CUDA(c, c->il_off.ensure(nseg, st));
         NB_CUDA(c, c->ilm_off.ensure(nseg, st));
-        NB_CUDA(c, c->il_cnt.ensure(nseg, st));
+        NB_CUDA(c, c->seg.ensure(nseg, st));
         int* capu = c->scan_tmp.p;
         int* capm = c->scan_tmp.p + nseg;
-        k_ilist_caps<<<(nseg + 255) / 256, 256, 0, st>>>(c->units_canon.p, c->nunits, c->plane_outer.p, c->plane_excl.p, capu, capm);
+        k_ilist_caps<<<(nseg + 255) / 256, 256, 0, st>>>(c->units_sorted.p, c->nunits, c->plane_outer.p, c->plane_excl.p, capu, capm);
         NB_LAUNCH_CHECK(c);
         rc = nbi_exclusive_scan(c, capu, c->il_off.p, nseg, total_dev);
         if (rc != NB_OK) return rc;
@@ -630,8 +638,8 @@ int nbi_search(nb_ctx* c, float rlist)
         NB_CUDA(c, cudaStreamSynchronize(st));
         NB_CUDA(c, c->il.ensure((size_t)tot[0] + 4, st));
         NB_CUDA(c, c->ilm.ensure((size_t)tot[1] + 4, st));
-        k_ilist_build<<<c->nunits, 256, 0, st>>>(c->units_canon.p, c->plane_inner.p, c->plane_excl.p, c->jl.p, c->il_off.p,
-                                                 c->ilm_off.p, c->il_cnt.p, c->il.p, c->ilm.p);
+        k_ilist_build<<<c->nunits, 256, 0, st>>>(c->units_sorted.p, c->plane_inner.p, c->plane_excl.p, c->jl.p, c->il_off.p,
+                                                 c->ilm_off.p, c->seg.p, c->il.p, c->ilm.p, c->nclusters);
         NB_LAUNCH_CHECK(c);
     } else {
         std::vector<unsigned long long> ones(16, ~0ull);

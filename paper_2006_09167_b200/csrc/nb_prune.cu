@@ -28,9 +28,10 @@ struct PruneArgs {
     float rl2;   // fl32(rlist_inner^2), reading A12
     // compact inner list written for the force kernel (nb_internal.h)
     int u0;      // canonical index of units[0]
+    int cj_dummy;
     const uint32_t* plane_excl;
-    const int *il_off, *ilm_off;
-    int2* il_cnt;
+    const int* unit_pos;
+    int4* seg;
     int32_t* il;
     int2* ilm;
 };
@@ -130,9 +131,10 @@ __global__ void __launch_bounds__(256) k_prune(PruneArgs A)
     }
     __syncwarp();
     if (lane < u.z - u.y) A.plane_inner[(size_t)(u.y + lane) * 8 + warp] = res[lane];
-    const int seg = (A.u0 + blockIdx.x) * 8 + warp;
-    nb_ilist_write([&](int b) { return res[b]; }, u.y, u.z, warp, lane, A.plane_excl, A.jl, A.il + A.il_off[seg],
-                   A.ilm + A.ilm_off[seg], &A.il_cnt[seg]);
+    int4* sg = &A.seg[A.unit_pos[A.u0 + blockIdx.x] * 8 + warp];
+    const int2 off = *reinterpret_cast<const int2*>(sg);
+    nb_ilist_write([&](int b) { return res[b]; }, u.y, u.z, warp, lane, A.cj_dummy, A.plane_excl, A.jl, A.il + off.x, A.ilm + off.y,
+                   reinterpret_cast<int2*>(sg) + 1);
 }
 
 }  // namespace
@@ -153,8 +155,9 @@ int nbi_prune(nb_ctx* c, float rlist_inner, int part, int nparts)
     for (int k = 0; k < 3; k++) A.box[k] = c->box[k];
     A.rl2 = rlist_inner * rlist_inner;
     A.u0 = u0;
+    A.cj_dummy = c->nclusters;
     A.plane_excl = c->plane_excl.p;
-    A.il_off = c->il_off.p; A.ilm_off = c->ilm_off.p; A.il_cnt = c->il_cnt.p;
+    A.unit_pos = c->unit_pos.p; A.seg = c->seg.p;
     A.il = c->il.p; A.ilm = c->ilm.p;
     NbStageTimer tm(c, NB_T_PRUNE);
     k_prune<<<u1 - u0, 256, 0, c->stream>>>(A);
