@@ -255,23 +255,26 @@ __global__ void __launch_bounds__(256, 2) k_force(ForceArgs A)
     // operations whose consumer is an iteration away at the END of the step, so the j data of
     // step s+1 is loaded there; to make that load an L1 hit the lines are prefetched one step
     // earlier still (distance 2), and the list entries are read 3 steps ahead (indices clamped).
-    int cj_nn = 0;
+    int cj2 = 0, cj3 = 0;
+    float4 xj1 = xj;
+    int tj1 = tj;
     if (ns > 0) {
-        cj_nn = il[4 * min(2, ns - 1) + g];
-        prefetch_l1(&A.xq[cj_n * 8 + k]);
-        prefetch_l1(&A.type_slot[cj_n * 8 + k]);
+        cj2 = il[4 * min(2, ns - 1) + g];
+        cj3 = il[4 * min(3, ns - 1) + g];
+        xj1 = A.xq[cj_n * 8 + k];
+        tj1 = A.type_slot[cj_n * 8 + k];
     }
 #pragma unroll 2
     for (int s = 0; s < ns; s++) {
-        const int cj_3 = il[4 * min(s + 3, ns - 1) + g];
-        prefetch_l1(&A.xq[cj_nn * 8 + k]);
-        prefetch_l1(&A.type_slot[cj_nn * 8 + k]);
+        const int cj4 = il[4 * min(s + 4, ns - 1) + g];
+        const float4 x2 = A.xq[cj2 * 8 + k];
+        const int t2 = A.type_slot[cj2 * 8 + k];
         float2 fjx, fjy, fjz;
         pair_step<COUL, ENERGY, false>(K, ljw + tj, nt1, I, fix, fiy, fiz, elj, ecoul, xj, 0xffu, 0xffu, fjx, fjy, fjz, p3);
         red_add_v4(&A.f4[cj * 8 + k], -(fjx.x + fjx.y), -(fjy.x + fjy.y), -(fjz.x + fjz.y));
-        cj = cj_n; cj_n = cj_nn; cj_nn = cj_3;
-        xj = A.xq[cj * 8 + k];        // L1 hit: prefetched a step ago
-        tj = A.type_slot[cj * 8 + k];
+        cj = cj_n; xj = xj1; tj = tj1;
+        cj_n = cj2; xj1 = x2; tj1 = t2;
+        cj2 = cj3; cj3 = cj4;
     }
 
     float fi[24];
