@@ -328,15 +328,15 @@ int nbi_grid(nb_ctx* c)
     if (smem > 200 * 1024)
         return nb_fail(c, NB_ERR_OVERFLOW, "grid column holds %d atoms; the in-shared-memory z-sort takes at most 25600",
                        c->max_col_count);
-    NB_CUDA(c, c->xq.ensure(c->nslots + NB_C, st));          // + one dummy cluster (index nclusters), see below
-    NB_CUDA(c, c->type_slot.ensure(c->nslots + NB_C, st));
+    NB_CUDA(c, c->xq.ensure(c->nslots + NB_C * NB_NDUMMY, st));   // + dummy clusters (index >= nclusters), see below
+    NB_CUDA(c, c->type_slot.ensure(c->nslots + NB_C * NB_NDUMMY, st));
     NB_CUDA(c, c->atom_of_slot.ensure(c->nslots, st));
     NB_CUDA(c, c->bb_lo.ensure(c->nclusters, st));
     NB_CUDA(c, c->bb_hi.ensure(c->nclusters, st));
     NB_CUDA(c, c->sbb_lo.ensure(c->nsc, st));
     NB_CUDA(c, c->sbb_hi.ensure(c->nsc, st));
-    NB_CUDA(c, c->f4.ensure(c->nslots + NB_C, st));
-    NB_CUDA(c, cudaMemsetAsync(c->f4.p, 0, sizeof(float4) * c->nslots, st));
+    NB_CUDA(c, c->f4.ensure(c->nslots + NB_C * NB_NDUMMY, st));
+    NB_CUDA(c, cudaMemsetAsync(c->f4.p, 0, sizeof(float4) * (c->nslots + NB_C * NB_NDUMMY), st));
     NB_CUDA(c, cudaFuncSetAttribute(k_col_layout, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     float pb[3], pd[3];
     for (int k = 0; k < 3; k++) {
@@ -350,16 +350,16 @@ int nbi_grid(nb_ctx* c)
                                              make_float3(pd[0], pd[1], pd[2]));
     NB_LAUNCH_CHECK(c);
     {
-        // Dummy j-cluster (index nclusters): padding-like atoms beyond the padding lattice; interacts
-        // with nothing.  Available to kernels that need a harmless list entry.
-        float4 hx[NB_C];
-        int32_t ht[NB_C];
-        for (int k = 0; k < NB_C; k++) {
-            hx[k] = make_float4(pb[0] - pd[0] * (float)(64 + k), pb[1], pb[2], 0.f);
-            ht[k] = c->ntypes;
-        }
-        NB_CUDA(c, cudaMemcpyAsync(c->xq.p + c->nslots, hx, sizeof(hx), cudaMemcpyHostToDevice, st));
-        NB_CUDA(c, cudaMemcpyAsync(c->type_slot.p + c->nslots, ht, sizeof(ht), cudaMemcpyHostToDevice, st));
+        // Dummy j-clusters (index nclusters .. nclusters + NB_NDUMMY - 1): padding-like atoms beyond the
+        // padding lattice that interact with nothing.  The prune kernel may fill an inner list
+        // segment up to a multiple of 4 with them; the (zero) forces the force kernel adds to their
+        // slots are never read, and spreading them over NB_NDUMMY clusters avoids atomic hot spots.
+        std::vector<float4> hx((size_t)NB_C * NB_NDUMMY);
+        std::vector<int32_t> ht((size_t)NB_C * NB_NDUMMY, c->ntypes);
+        for (size_t i = 0; i < hx.size(); i++)
+            hx[i] = make_float4(pb[0] - pd[0] * (float)(64 + (i % NB_C)), pb[1], pb[2], 0.f);
+        NB_CUDA(c, cudaMemcpyAsync(c->xq.p + c->nslots, hx.data(), sizeof(float4) * hx.size(), cudaMemcpyHostToDevice, st));
+        NB_CUDA(c, cudaMemcpyAsync(c->type_slot.p + c->nslots, ht.data(), sizeof(int32_t) * ht.size(), cudaMemcpyHostToDevice, st));
         NB_CUDA(c, cudaStreamSynchronize(st));
     }
     c->grid_box[0] = L[0];

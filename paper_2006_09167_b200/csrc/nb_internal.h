@@ -17,6 +17,7 @@
 #define NB_NHALF 14                   // zero shift + 13 shifts with s >lex 0
 #define NB_BATCH 32                   // joint j entries per mask word (one ballot)
 #define NB_MAX_UNIT_BATCHES 16        // a work unit spans at most this many batches of one list element
+#define NB_NDUMMY 1024                // dummy j-clusters behind the real ones (spread the never-read force adds)
 #define NB_PAD_TYPE_ROW 1             // LJ table carries one extra all-zero type for padding atoms
 
 // One growable device array.
@@ -200,10 +201,9 @@ int nb_fail(nb_ctx* c, int code, const char* fmt, ...);
 #ifdef __CUDACC__
 // Writes the compact inner list segment of (unit, i-cluster warp) from the unit's inner mask
 // words `bits_of(b)` (b = batch index relative to the unit).  Entries whose exclusion mask is
-// trivial for this i-cluster go to `il` (cj only), the others to `ilm` {cj, mask ref}; the last
-// (count mod 4) unmasked entries are moved to `ilm` with ref 0 (the all-ones mask) so that the
-// force kernel's unmasked steps are always full (padding them with the dummy cluster `cj_dummy`
-// instead was measured slower: one more step per segment).  One warp, all 32 lanes.
+// trivial for this i-cluster go to `il` (cj only), the others to `ilm` {cj, mask ref}; the
+// unmasked count is made a multiple of 4 (see below) so that the force kernel's unmasked steps
+// are always full.  One warp, all 32 lanes.
 template <typename BitsOf>
 __device__ __forceinline__ void nb_ilist_write(BitsOf bits_of, int b0, int b1, int warp, int lane, int cj_dummy,
                                                const uint32_t* __restrict__ plane_excl, const int2* __restrict__ jl,
@@ -223,9 +223,23 @@ __device__ __forceinline__ void nb_ilist_write(BitsOf bits_of, int b0, int b1, i
         nm += __popc(eb);
     }
     __syncwarp();
-    const int rem = nu & 3, nu4 = nu - rem;
-    if (lane < rem) ilm[nm + lane] = make_int2(il[nu4 + lane], 0);
-    if (lane == 0) *cnt = make_int2(nu4, nm + rem);
+    // The (nu mod 4) unmasked entries left over: if they fit into the free lanes of the masked
+    // steps that run anyway they go there (ref 0 = all-ones mask); otherwise the unmasked list is
+    // filled up to a multiple of 4 with the dummy cluster -- a full unmasked step is cheaper than
+    // an extra masked one.
+    const int rem = nu & 3;
+#ifndef NB_TAIL_POLICY
+#define NB_TAIL_POLICY 1
+#endif
+    if (rem != 0 && (NB_TAIL_POLICY == 0 || (nm > 0 && (nm + rem + 3) / 4 == (nm + 3) / 4))) {
+        if (lane < rem) ilm[nm + lane] = make_int2(il[nu - rem + lane], 0);
+        nu -= rem;
+        nm += rem;
+    } else if (rem != 0) {
+        if (lane < 4 - rem) il[nu + lane] = cj_dummy + ((b0 * 8 + warp + lane) & (NB_NDUMMY - 1));
+        nu += 4 - rem;
+    }
+    if (lane == 0) *cnt = make_int2(nu, nm);
 }
 #endif
 
