@@ -117,21 +117,26 @@ static int put_atoms_common(nb_ctx* c, const float* x, const float* q, const int
     cudaStream_t st = c->stream;
     const int n = c->natoms;
     NbStageTimer tm(c, NB_T_PUT);
-    NB_CUDA(c, cudaMemcpyAsync(c->x.p, x, sizeof(float) * 3 * n, kind, st));
-    NB_CUDA(c, cudaMemcpyAsync(c->q.p, q, sizeof(float) * n, kind, st));
-    NB_CUDA(c, cudaMemcpyAsync(c->type.p, type, sizeof(int32_t) * n, kind, st));
+    const bool device = kind == cudaMemcpyDeviceToDevice;
+    if (!device) {
+        NB_CUDA(c, cudaMemcpyAsync(c->x.p, x, sizeof(float) * 3 * n, kind, st));
+        NB_CUDA(c, cudaMemcpyAsync(c->q.p, q, sizeof(float) * n, kind, st));
+        NB_CUDA(c, cudaMemcpyAsync(c->type.p, type, sizeof(int32_t) * n, kind, st));
+    }
     for (int k = 0; k < 3; k++) c->box[k] = box[k];
     c->have_atoms = true;
     c->atoms_since_search = true;
+    bool refresh = false;
     if (c->have_grid) {
         if (box[0] != c->grid_box[0] || box[1] != c->grid_box[1] || box[2] != c->grid_box[2]) {
             c->have_list = false;   // a new box needs a new search
             c->have_grid = false;
         } else {
-            return nbi_refresh_xq(c);
+            refresh = true;
         }
     }
-    return NB_OK;
+    if (device) return nbi_put_device(c, x, q, type, refresh);   // one launch: copies + refresh
+    return refresh ? nbi_refresh_xq(c) : NB_OK;
 }
 
 extern "C" int nb_put_atoms(nb_ctx* c, const float* x, const float* q, const int32_t* type, const float box[3])

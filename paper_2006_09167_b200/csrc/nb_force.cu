@@ -265,7 +265,7 @@ __global__ void __launch_bounds__(256, 2) k_force(ForceArgs A)
         xj1 = A.xq[cj_n * 8 + k];
         tj1 = A.type_slot[cj_n * 8 + k];
     }
-#pragma unroll 2
+#pragma unroll 2   // (unroll 3, the period of the rotation below, was measured slower)
     for (int s = 0; s < ns; s++) {
         const int cj4 = il[4 * min(s + 4, ns - 1) + g];
         const float4 x2 = A.xq[cj2 * 8 + k];

@@ -268,7 +268,36 @@ __global__ void k_refresh_xq(int n, const float* __restrict__ x, const float* __
     xq[slot_of_atom[i]] = v;
 }
 
+// (a1) device-pointer nb_put_atoms in ONE launch: copy the caller's x, q, type into the context
+// (the next search reads them) and, when a grid exists, refresh the cluster-ordered coordinates.
+__global__ void __launch_bounds__(256) k_put(int n, const float* __restrict__ x, const float* __restrict__ q,
+                                             const int* __restrict__ type, float* __restrict__ cx, float* __restrict__ cq,
+                                             int* __restrict__ ctype, const char4* __restrict__ image,
+                                             const int* __restrict__ slot_of_atom, float3 box, float4* __restrict__ xq)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float px = x[3 * i], py = x[3 * i + 1], pz = x[3 * i + 2], pq = q[i];
+    cx[3 * i] = px; cx[3 * i + 1] = py; cx[3 * i + 2] = pz;
+    cq[i] = pq;
+    ctype[i] = type[i];
+    if (xq) {
+        const char4 im = image[i];
+        xq[slot_of_atom[i]] = make_float4(__fmaf_rn(-(float)im.x, box.x, px), __fmaf_rn(-(float)im.y, box.y, py),
+                                          __fmaf_rn(-(float)im.z, box.z, pz), pq);
+    }
+}
+
 }  // namespace
+
+int nbi_put_device(nb_ctx* c, const float* x, const float* q, const int32_t* type, bool refresh)
+{
+    int n = c->natoms;
+    k_put<<<(n + 255) / 256, 256, 0, c->stream>>>(n, x, q, type, c->x.p, c->q.p, c->type.p, c->image.p, c->slot_of_atom.p,
+                                                  make_float3(c->box[0], c->box[1], c->box[2]), refresh ? c->xq.p : nullptr);
+    NB_LAUNCH_CHECK(c);
+    return NB_OK;
+}
 
 int nbi_refresh_xq(nb_ctx* c)
 {

@@ -199,6 +199,29 @@ __host__ __device__ inline void nb_shift_vec(int id, int& sx, int& sy, int& sz)
 int nb_fail(nb_ctx* c, int code, const char* fmt, ...);
 
 #ifdef __CUDACC__
+#ifndef NB_TAIL_POLICY
+#define NB_TAIL_POLICY 1
+#endif
+// Closes an inner list segment of nu unmasked + nm masked entries (one warp; the entries must be
+// visible to the warp).  The (nu mod 4) unmasked entries left over: if they fit into the free
+// lanes of the masked steps that run anyway they go there (ref 0 = all-ones mask); otherwise the
+// unmasked list is filled up to a multiple of 4 with dummy clusters -- a full unmasked step is
+// cheaper than an extra masked one.
+__device__ __forceinline__ void nb_ilist_finish(int nu, int nm, int salt, int lane, int cj_dummy,
+                                                int32_t* __restrict__ il, int2* __restrict__ ilm, int2* __restrict__ cnt)
+{
+    const int rem = nu & 3;
+    if (rem != 0 && (NB_TAIL_POLICY == 0 || (nm > 0 && (nm + rem + 3) / 4 == (nm + 3) / 4))) {
+        if (lane < rem) ilm[nm + lane] = make_int2(il[nu - rem + lane], 0);
+        nu -= rem;
+        nm += rem;
+    } else if (rem != 0) {
+        if (lane < 4 - rem) il[nu + lane] = cj_dummy + ((salt + lane) & (NB_NDUMMY - 1));
+        nu += 4 - rem;
+    }
+    if (lane == 0) *cnt = make_int2(nu, nm);
+}
+
 // Writes the compact inner list segment of (unit, i-cluster warp) from the unit's inner mask
 // words `bits_of(b)` (b = batch index relative to the unit).  Entries whose exclusion mask is
 // trivial for this i-cluster go to `il` (cj only), the others to `ilm` {cj, mask ref}; the
@@ -223,23 +246,7 @@ __device__ __forceinline__ void nb_ilist_write(BitsOf bits_of, int b0, int b1, i
         nm += __popc(eb);
     }
     __syncwarp();
-    // The (nu mod 4) unmasked entries left over: if they fit into the free lanes of the masked
-    // steps that run anyway they go there (ref 0 = all-ones mask); otherwise the unmasked list is
-    // filled up to a multiple of 4 with the dummy cluster -- a full unmasked step is cheaper than
-    // an extra masked one.
-    const int rem = nu & 3;
-#ifndef NB_TAIL_POLICY
-#define NB_TAIL_POLICY 1
-#endif
-    if (rem != 0 && (NB_TAIL_POLICY == 0 || (nm > 0 && (nm + rem + 3) / 4 == (nm + 3) / 4))) {
-        if (lane < rem) ilm[nm + lane] = make_int2(il[nu - rem + lane], 0);
-        nu -= rem;
-        nm += rem;
-    } else if (rem != 0) {
-        if (lane < 4 - rem) il[nu + lane] = cj_dummy + ((b0 * 8 + warp + lane) & (NB_NDUMMY - 1));
-        nu += 4 - rem;
-    }
-    if (lane == 0) *cnt = make_int2(nu, nm);
+    nb_ilist_finish(nu, nm, b0 * 8 + warp, lane, cj_dummy, il, ilm, cnt);
 }
 #endif
 
@@ -260,6 +267,7 @@ __device__ __forceinline__ void nb_ilist_write(BitsOf bits_of, int b0, int b1, i
 // Stage implementations (one translation unit each).
 int nbi_grid(nb_ctx* c);                                   // (a2) nb_grid.cu
 int nbi_refresh_xq(nb_ctx* c);                             // (a1) nb_grid.cu
+int nbi_put_device(nb_ctx* c, const float* x, const float* q, const int32_t* type, bool refresh);   // (a1) nb_grid.cu
 int nbi_search(nb_ctx* c, float rlist);                    // (a3)-(a5) nb_list.cu
 int nbi_prune(nb_ctx* c, float rlist_inner, int part, int nparts);   // (a6) nb_prune.cu
 int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial);   // (a7)-(a8) nb_force.cu

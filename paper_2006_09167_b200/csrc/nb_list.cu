@@ -331,11 +331,12 @@ __global__ void k_ilist_caps(const int4* __restrict__ units, int nunits, const u
     capm[i] = nm + 3;
 }
 
-// inner := the given planes (after a search: the outer ones).  One block per work unit.
+// After a search, one block per work unit (launch order): inner := outer.
 __global__ void __launch_bounds__(256) k_ilist_build(const int4* __restrict__ units, const uint32_t* __restrict__ plane,
                                                      const uint32_t* __restrict__ plane_excl, const int2* __restrict__ jl,
                                                      const int* __restrict__ il_off, const int* __restrict__ ilm_off,
-                                                     int4* __restrict__ seg, int32_t* __restrict__ il, int2* __restrict__ ilm, int cj_dummy)
+                                                     int4* __restrict__ seg, int32_t* __restrict__ il, int2* __restrict__ ilm,
+                                                     int cj_dummy)
 {
     const int4 u = units[blockIdx.x];   // units in launch order
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, s = blockIdx.x * 8 + warp;
