@@ -183,20 +183,20 @@ __device__ __forceinline__ void pair_step(const NbConst& K, const float4* __rest
 }
 
 template <int COUL, bool ENERGY>
-__global__ void __launch_bounds__(256, 2) k_force(ForceArgs A)
+__global__ void __launch_bounds__(32, 16) k_force(ForceArgs A)
 {
     // Paired LJ table of this block: s_ljp[(w*4 + p)*nt1 + tj] = (-6c6, -6c6', 12c12, 12c12') of the
     // i atoms 2p, 2p+1 of i-cluster w against j type tj: one LDS.128 feeds both packed operands.
     extern __shared__ float4 s_ljp[];
     const NbConst& K = A.kc;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7;
-    const int4 u = A.units[blockIdx.x];
-    const int4 sg = A.seg[blockIdx.x * 8 + warp];
+    const int warp = blockIdx.x & 7, lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7;
+    const int4 u = A.units[blockIdx.x >> 3];
+    const int4 sg = A.seg[blockIdx.x];
     const int sci = u.w, h = u.x - sci * NB_NHALF, ci = sci * 8 + warp;
     const int sid = nb_half_shift_id(h);
     const int nt1 = K.ntypes1;
     // each warp builds its own part of the table: no block-level barrier
-    float4* ljw = s_ljp + warp * 4 * nt1;
+    float4* ljw = s_ljp;
     for (int i = lane; i < 4 * nt1; i += 32) {
         const int p = i / nt1, tj = i - p * nt1;
         const int ta = A.type_slot[ci * 8 + 2 * p], tb = A.type_slot[ci * 8 + 2 * p + 1];
@@ -461,10 +461,10 @@ __global__ void __launch_bounds__(256) k_count_pairs(ForceArgs A, unsigned long 
 template <int COUL, bool ENERGY>
 int launch_force(nb_ctx* c, const ForceArgs& A)
 {
-    const size_t smem = sizeof(float4) * 32 * (size_t)c->kc.ntypes1;   // paired LJ table, 512 B per type
+    const size_t smem = sizeof(float4) * 4 * (size_t)c->kc.ntypes1;   // paired LJ table of one i-cluster, 64 B per type
     if (smem > 48 * 1024)
         NB_CUDA(c, cudaFuncSetAttribute(k_force<COUL, ENERGY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_force<COUL, ENERGY><<<c->nunits, 256, smem, c->stream>>>(A);
+    k_force<COUL, ENERGY><<<c->nunits * 8, 32, smem, c->stream>>>(A);
     NB_LAUNCH_CHECK(c);
     return NB_OK;
 }
