@@ -30,6 +30,7 @@ struct ForceArgs {
     const float2* ljtab;
     const unsigned long long* masks;
     const int4* seg;            // compact inner list, see nb_internal.h
+    const int2* seg_ci;
     const int* il;
     const int2* ilm;
     float4* f4;
@@ -189,11 +190,10 @@ __global__ void __launch_bounds__(32, 16) k_force(ForceArgs A)
     // i atoms 2p, 2p+1 of i-cluster w against j type tj: one LDS.128 feeds both packed operands.
     extern __shared__ float4 s_ljp[];
     const NbConst& K = A.kc;
-    const int warp = blockIdx.x & 7, lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7;
-    const int4 u = A.units[blockIdx.x >> 3];
+    const int lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7;
     const int4 sg = A.seg[blockIdx.x];
-    const int sci = u.w, h = u.x - sci * NB_NHALF, ci = sci * 8 + warp;
-    const int sid = nb_half_shift_id(h);
+    const int2 sc = A.seg_ci[blockIdx.x];
+    const int ci = sc.x, sid = sc.y, warp = ci & 7;
     const int nt1 = K.ntypes1;
     // each warp builds its own part of the table: no block-level barrier
     float4* ljw = s_ljp;
@@ -464,7 +464,7 @@ int launch_force(nb_ctx* c, const ForceArgs& A)
     const size_t smem = sizeof(float4) * 4 * (size_t)c->kc.ntypes1;   // paired LJ table of one i-cluster, 64 B per type
     if (smem > 48 * 1024)
         NB_CUDA(c, cudaFuncSetAttribute(k_force<COUL, ENERGY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_force<COUL, ENERGY><<<c->nunits * 8, 32, smem, c->stream>>>(A);
+    k_force<COUL, ENERGY><<<c->nseg_launch, 32, smem, c->stream>>>(A);
     NB_LAUNCH_CHECK(c);
     return NB_OK;
 }
@@ -479,6 +479,7 @@ int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial)
     A.jl = c->jl.p;
     A.plane = c->plane_inner.p;
     A.seg = c->seg.p;
+    A.seg_ci = c->seg_ci.p;
     A.il = c->il.p;
     A.ilm = c->ilm.p;
     A.xq = c->xq.p;
@@ -510,7 +511,7 @@ int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial)
         NB_CUDA(c, cudaMemsetAsync(c->fshift.p, 0, (NB_NSHIFT * 3 + 9) * sizeof(double), st));
     }
     int rc = NB_OK;
-    if (c->nunits > 0) {
+    if (c->nunits > 0 && c->nseg_launch > 0) {
         NbStageTimer tm(c, NB_T_FORCE);
         if (c->prm.coulomb == NB_COUL_EWALD)
             rc = energy ? launch_force<NB_COUL_EWALD, true>(c, A) : launch_force<NB_COUL_EWALD, false>(c, A);

@@ -134,9 +134,13 @@ struct nb_ctx {
 
     // --- compact inner list (a6 -> a7): per (work unit, i-cluster) the j-clusters whose inner mask bit is set ---
     DevBuf<int32_t> il_off, ilm_off;           // [nunits*8] scan scratch: first entry of the segment in il / ilm
-    DevBuf<int4> seg;                          // [nunits*8], index = launch position*8 + i-cluster:
+    DevBuf<int4> seg;                          // [nunits*8], one per (work unit, i-cluster), longest outer list first:
                                                // {il offset, ilm offset, unmasked entries (multiple of 4), masked entries}
     DevBuf<int32_t> unit_pos;                  // canonical unit index -> launch position (inverse of unit_order)
+    DevBuf<int32_t> seg_pos;                   // [nunits*8] (unit launch position*8 + i-cluster) -> index into seg (longest first)
+    DevBuf<int2> seg_ci;                       // [nunits*8] {i-cluster, shift id} of each seg entry
+    int nseg_launch = 0;                       // seg entries with a non-empty outer list (= force kernel grid)
+    std::vector<int32_t> h_caps;               // host scratch
     DevBuf<int32_t> il;                        // cj of cluster pairs without a mask for this i-cluster
     DevBuf<int2> ilm;                          // {cj, mask ref} of cluster pairs with a mask, plus each segment's tail
     DevBuf<double> fshift;                     // [27*3] per-shift i-force sums (virial)

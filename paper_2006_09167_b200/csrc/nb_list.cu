@@ -335,13 +335,19 @@ __global__ void k_ilist_caps(const int4* __restrict__ units, int nunits, const u
 __global__ void __launch_bounds__(256) k_ilist_build(const int4* __restrict__ units, const uint32_t* __restrict__ plane,
                                                      const uint32_t* __restrict__ plane_excl, const int2* __restrict__ jl,
                                                      const int* __restrict__ il_off, const int* __restrict__ ilm_off,
-                                                     int4* __restrict__ seg, int32_t* __restrict__ il, int2* __restrict__ ilm,
-                                                     int cj_dummy)
+                                                     const int* __restrict__ seg_pos, int4* __restrict__ seg,
+                                                     int2* __restrict__ seg_ci, int32_t* __restrict__ il,
+                                                     int2* __restrict__ ilm, int cj_dummy)
 {
     const int4 u = units[blockIdx.x];   // units in launch order
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, s = blockIdx.x * 8 + warp;
-    const int o = il_off[s], om = ilm_off[s];
-    if (lane == 0) { seg[s].x = o; seg[s].y = om; }
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, s0 = blockIdx.x * 8 + warp;
+    const int o = il_off[s0], om = ilm_off[s0];
+    const int s = seg_pos[s0];
+    if (lane == 0) {
+        seg[s].x = o;
+        seg[s].y = om;
+        seg_ci[s] = make_int2(u.w * 8 + warp, nb_half_shift_id(u.x - u.w * NB_NHALF));
+    }
     nb_ilist_write([&](int b) { return plane[(size_t)(u.y + b) * 8 + warp]; }, u.y, u.z, warp, lane, cj_dummy, plane_excl, jl,
                    il + o, ilm + om, reinterpret_cast<int2*>(&seg[s]) + 1);
 }
@@ -636,11 +642,30 @@ int nbi_search(nb_ctx* c, float rlist)
         if (rc != NB_OK) return rc;
         int tot[2] = {0, 0};
         NB_CUDA(c, cudaMemcpyAsync(tot, total_dev, sizeof(tot), cudaMemcpyDeviceToHost, st));
+        c->h_caps.resize((size_t)2 * nseg);
+        NB_CUDA(c, cudaMemcpyAsync(c->h_caps.data(), capu, sizeof(int) * 2 * nseg, cudaMemcpyDeviceToHost, st));
         NB_CUDA(c, cudaStreamSynchronize(st));
+        {
+            // L199: longest lists first, now per i-cluster list: counting sort of the segments by
+            // outer length (descending, stable); empty segments are not launched.
+            const int* cu = c->h_caps.data();
+            const int* cm = cu + nseg;
+            int maxlen = 0;
+            for (int i = 0; i < nseg; i++) maxlen = std::max(maxlen, cu[i] + cm[i] - 3);
+            std::vector<int32_t> start(maxlen + 2, 0), pos(nseg);
+            for (int i = 0; i < nseg; i++) start[maxlen - (cu[i] + cm[i] - 3) + 1]++;
+            for (int l = 0; l <= maxlen; l++) start[l + 1] += start[l];
+            c->nseg_launch = start[maxlen];   // everything before the length-0 bucket
+            for (int i = 0; i < nseg; i++) pos[i] = start[maxlen - (cu[i] + cm[i] - 3)]++;
+            NB_CUDA(c, c->seg_pos.ensure(nseg, st));
+            NB_CUDA(c, c->seg_ci.ensure(nseg, st));
+            NB_CUDA(c, cudaMemcpyAsync(c->seg_pos.p, pos.data(), sizeof(int) * nseg, cudaMemcpyHostToDevice, st));
+            NB_CUDA(c, cudaStreamSynchronize(st));
+        }
         NB_CUDA(c, c->il.ensure((size_t)tot[0] + 4, st));
         NB_CUDA(c, c->ilm.ensure((size_t)tot[1] + 4, st));
         k_ilist_build<<<c->nunits, 256, 0, st>>>(c->units_sorted.p, c->plane_inner.p, c->plane_excl.p, c->jl.p, c->il_off.p,
-                                                 c->ilm_off.p, c->seg.p, c->il.p, c->ilm.p, c->nclusters);
+                                                 c->ilm_off.p, c->seg_pos.p, c->seg.p, c->seg_ci.p, c->il.p, c->ilm.p, c->nclusters);
         NB_LAUNCH_CHECK(c);
     } else {
         std::vector<unsigned long long> ones(16, ~0ull);

@@ -31,6 +31,7 @@ struct PruneArgs {
     int cj_dummy;
     const uint32_t* plane_excl;
     const int* unit_pos;
+    const int* seg_pos;
     int4* seg;
     int32_t* il;
     int2* ilm;
@@ -131,7 +132,7 @@ __global__ void __launch_bounds__(256) k_prune(PruneArgs A)
     }
     __syncwarp();
     if (lane < u.z - u.y) A.plane_inner[(size_t)(u.y + lane) * 8 + warp] = res[lane];
-    int4* sg = &A.seg[A.unit_pos[A.u0 + blockIdx.x] * 8 + warp];
+    int4* sg = &A.seg[A.seg_pos[A.unit_pos[A.u0 + blockIdx.x] * 8 + warp]];
     const int2 off = *reinterpret_cast<const int2*>(sg);
     nb_ilist_write([&](int b) { return res[b]; }, u.y, u.z, warp, lane, A.cj_dummy, A.plane_excl, A.jl, A.il + off.x, A.ilm + off.y,
                    reinterpret_cast<int2*>(sg) + 1);
@@ -157,7 +158,7 @@ int nbi_prune(nb_ctx* c, float rlist_inner, int part, int nparts)
     A.u0 = u0;
     A.cj_dummy = c->nclusters;
     A.plane_excl = c->plane_excl.p;
-    A.unit_pos = c->unit_pos.p; A.seg = c->seg.p;
+    A.unit_pos = c->unit_pos.p; A.seg_pos = c->seg_pos.p; A.seg = c->seg.p;
     A.il = c->il.p; A.ilm = c->ilm.p;
     NbStageTimer tm(c, NB_T_PRUNE);
     k_prune<<<u1 - u0, 256, 0, c->stream>>>(A);
