@@ -31,9 +31,14 @@ if ROOT not in sys.path:
 
 METRIC = "effective non-bonded pair interactions/s (cluster-pair step: put_atoms+search/prune+forces)"
 UNIT = "pairs/s"
-# Algorithmic FP32 work of the force kernel per atom-pair slot (DESIGN.md "Roofline of the force
-# kernel"): FFMA = 2 flop, FADD/FMUL/compare/select = 1, MUFU = 1.
-FLOP_PER_SLOT = {"ewald": 60.0, "rf": 37.0}
+# FP32 work of the force kernel per atom-pair slot: what the unmasked F-only
+# step executes, counted in its SASS -- packed FFMA2 = 4 flop, FMUL2/FADD2 = 2, FFMA = 2,
+# FADD/FMUL/MUFU = 1 -- divided by the 256 slots of a warp step.  (SURVEY 8.4's estimate of the
+# method's work was 62 / 40; the smaller executed count is the one used.)
+FLOP_PER_SLOT = {"ewald": 55.75, "rf": 36.75}
+# DRAM bytes of one force-kernel launch from the committed ncu --set full capture (profiles/r1c_force_full_cfg2.md);
+# the kernel is ALU-bound, its HBM traffic is ~0.2 % of what the HBM roofline would allow in the same time.
+NCU_DRAM_BYTES_PER_LAUNCH = {(2, "ewald"): 12.6e6}
 N_SM, FP32_LANES_PER_SM = 148, 128   # B200_PROFILING.md: 148 SMs; 128 FP32 lanes/SM (4 SMSP x 32)
 
 
@@ -365,7 +370,9 @@ def run_b200(args):
     force_us = 1e3 * f_ms / max(f_n, 1)
     achieved = flop_slot * slots_per_launch / (force_us * 1e-6) / 1e12 if f_n else 0.0
     roofline = {"bound": "alu", "kernel": "k_force (a7)", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-                "frac": achieved / peak_tflops, "traffic": None,
+                "frac": achieved / peak_tflops, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((args.config, w.coulomb)),
+                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one k_force launch, ncu --set full "
+                                  "(profiles/, latest force_full summary); null = not captured for this workload",
                 "peak_source": f"derived: {N_SM} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x {sm_max} MHz (clocks.max.sm); "
                                "MEASURED_PEAKS.json has no FP32 entry",
                 "measured_ffma_chain_tflops": 2 * fma_peak / 1e12,
