@@ -130,6 +130,10 @@ struct nb_ctx {
     std::vector<int4> h_units;
     DevBuf<int4> units_canon, units_sorted;    // {entry slot, batch begin, batch end, sci}
     DevBuf<int32_t> unit_order;                // canonical unit index, longest first (force kernel launch order)
+    DevBuf<int32_t> prune_order;               // canonical unit indices, each rolling part sorted longest first
+    std::vector<int32_t> h_prune_order;
+    int prune_order_nparts = 0;
+    int64_t prune_order_search = -1;
     int nunits = 0;
 
     // --- compact inner list (a6 -> a7): per (work unit, i-cluster) the j-clusters whose inner mask bit is set ---

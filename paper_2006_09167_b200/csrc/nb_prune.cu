@@ -16,10 +16,13 @@
 // the current step's arithmetic.
 #include "nb_internal.h"
 
+#include <algorithm>
+
 namespace {
 
 struct PruneArgs {
-    const int4* units;
+    const int4* units;        // canonical order
+    const int* order;         // launch order of this part: canonical unit indices, longest first
     const int2* jl;
     const uint32_t* plane_outer;
     uint32_t* plane_inner;
@@ -58,7 +61,8 @@ __global__ void __launch_bounds__(256) k_prune(PruneArgs A)
 {
     __shared__ int2 s_q[8][40];                          // {cj, unit-local joint slot}
     __shared__ unsigned s_res[8][NB_MAX_UNIT_BATCHES];   // inner mask words of this warp's plane
-    const int4 u = A.units[blockIdx.x];
+    const int ucan = A.order[blockIdx.x];
+    const int4 u = A.units[ucan];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7;
     const int sci = u.w, h = u.x - sci * NB_NHALF, ci = sci * 8 + warp;
     int sx, sy, sz;
@@ -132,7 +136,7 @@ __global__ void __launch_bounds__(256) k_prune(PruneArgs A)
     }
     __syncwarp();
     if (lane < u.z - u.y) A.plane_inner[(size_t)(u.y + lane) * 8 + warp] = res[lane];
-    int4* sg = &A.seg[A.seg_pos[A.unit_pos[A.u0 + blockIdx.x] * 8 + warp]];
+    int4* sg = &A.seg[A.seg_pos[A.unit_pos[ucan] * 8 + warp]];
     const int2 off = *reinterpret_cast<const int2*>(sg);
     nb_ilist_write([&](int b) { return res[b]; }, u.y, u.z, warp, lane, A.cj_dummy, A.plane_excl, A.jl, A.il + off.x, A.ilm + off.y,
                    reinterpret_cast<int2*>(sg) + 1);
@@ -147,8 +151,25 @@ int nbi_prune(nb_ctx* c, float rlist_inner, int part, int nparts)
     c->last_nparts = nparts;
     c->st.prune_count++;
     if (u1 <= u0) return NB_OK;
+    if (c->prune_order_nparts != nparts || c->prune_order_search != c->st.search_count) {
+        // launch order inside each rolling part: longest work unit first, so that the last
+        // wave of blocks is made of short units; rebuilt once per search / change of nparts
+        c->h_prune_order.resize(nu);
+        for (int i = 0; i < nu; i++) c->h_prune_order[i] = i;
+        for (int p = 0; p < nparts; p++) {
+            const long long a = (long long)p * nu / nparts, b = (long long)(p + 1) * nu / nparts;
+            std::stable_sort(c->h_prune_order.begin() + a, c->h_prune_order.begin() + b, [&](int x, int y) {
+                return (c->h_units[x].z - c->h_units[x].y) > (c->h_units[y].z - c->h_units[y].y);
+            });
+        }
+        NB_CUDA(c, c->prune_order.ensure(nu, c->stream));
+        NB_CUDA(c, cudaMemcpyAsync(c->prune_order.p, c->h_prune_order.data(), sizeof(int) * nu, cudaMemcpyHostToDevice, c->stream));
+        c->prune_order_nparts = nparts;
+        c->prune_order_search = c->st.search_count;
+    }
     PruneArgs A;
-    A.units = c->units_canon.p + u0;
+    A.units = c->units_canon.p;
+    A.order = c->prune_order.p + u0;
     A.jl = c->jl.p;
     A.plane_outer = c->plane_outer.p;
     A.plane_inner = c->plane_inner.p;
