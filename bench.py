@@ -35,7 +35,7 @@ UNIT = "pairs/s"
 # step executes, counted in its SASS -- packed FFMA2 = 4 flop, FMUL2/FADD2 = 2, FFMA = 2,
 # FADD/FMUL/MUFU = 1 -- divided by the 256 slots of a warp step.  (SURVEY 8.4's estimate of the
 # method's work was 62 / 40; the smaller executed count is the one used.)
-FLOP_PER_SLOT = {"ewald": 55.75, "rf": 36.75}
+FLOP_PER_SLOT = {"ewald": 55.75, "rf": 36.75, "none": 31.75}
 # DRAM bytes of one force-kernel launch from the committed ncu --set full capture (profiles/r1c_force_full_cfg2.md);
 # the kernel is ALU-bound, its HBM traffic is ~0.2 % of what the HBM roofline would allow in the same time.
 NCU_DRAM_BYTES_PER_LAUNCH = {(2, "ewald"): 12.6e6}
@@ -50,6 +50,8 @@ def parse_args():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[k] (default 2: ~96k atoms)")
     ap.add_argument("--coulomb", default="ewald", choices=["ewald", "rf"], help="config 2 only")
+    ap.add_argument("--lj-rc", type=float, default=0.0,
+                    help="instead of a BASELINE config: the LJ-only fluid of PAPER.md Fig. 6 (157 464 atoms) at this cut-off, nm")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-flush", action="store_true", help="do not flush L2 between timed steps")
@@ -58,13 +60,16 @@ def parse_args():
 
 def load_workload(args):
     from paper_2006_09167_b200 import workloads
+    if args.lj_rc > 0:
+        return workloads.lj_fluid(54, rc=args.lj_rc)
     if args.config == 2:
         return workloads.config2(args.coulomb)
     return workloads.by_index(args.config)
 
 
 def workload_config(w, args, extra=None):
-    cfg = {"workload": f"BASELINE.json configs[{args.config}] {w.name}: {w.natoms} atoms, box "
+    origin = "PAPER.md Fig. 6 stand-in (SURVEY 8.1 f2)" if args.lj_rc > 0 else f"BASELINE.json configs[{args.config}]"
+    cfg = {"workload": f"{origin} {w.name}: {w.natoms} atoms, box "
                        f"{float(w.box[0]):.4f}x{float(w.box[1]):.4f}x{float(w.box[2]):.4f} nm, {w.coulomb} rc={w.rc}, "
                        f"rlist_outer={w.rlist_outer}, rlist_inner={w.rlist_inner}, nstlist={w.nstlist}, "
                        f"rolling prune in {w.nparts} parts",
@@ -370,7 +375,7 @@ def run_b200(args):
     force_us = 1e3 * f_ms / max(f_n, 1)
     achieved = flop_slot * slots_per_launch / (force_us * 1e-6) / 1e12 if f_n else 0.0
     roofline = {"bound": "alu", "kernel": "k_force (a7)", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-                "frac": achieved / peak_tflops, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((args.config, w.coulomb)),
+                "frac": achieved / peak_tflops, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((args.config, w.coulomb)) if args.lj_rc <= 0 else None,
                 "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one k_force launch, ncu --set full "
                                   "(profiles/, latest force_full summary); null = not captured for this workload",
                 "peak_source": f"derived: {N_SM} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x {sm_max} MHz (clocks.max.sm); "

@@ -47,7 +47,8 @@ typedef struct nb_ctx nb_ctx; /* opaque, owned by the library */
 
 enum { NB_OK = 0, NB_ERR_ARG = -1, NB_ERR_STATE = -2, NB_ERR_CUTOFF = -3, NB_ERR_BOX = -4,
        NB_ERR_NOMEM = -5, NB_ERR_CUDA = -6, NB_ERR_OVERFLOW = -7 };
-enum { NB_COUL_EWALD = 0, NB_COUL_RF = 1 };
+enum { NB_COUL_EWALD = 0, NB_COUL_RF = 1,
+       NB_COUL_NONE = 2 /* LJ-only flavour (Fig. 6 workload): charges are ignored, E_coul = 0 */ };
 enum { NB_MOD_NONE = 0, NB_MOD_POTSHIFT = 1 };
 
 typedef struct {

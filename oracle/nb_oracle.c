@@ -36,7 +36,7 @@
 #endif
 
 typedef struct {
-    int32_t coulomb;     /* 0 = Ewald real space, 1 = reaction field */
+    int32_t coulomb;     /* 0 = Ewald real space, 1 = reaction field, 2 = none (LJ only: charges ignored) */
     int32_t lj_shift;    /* 1 = potential-shift on LJ energy */
     int32_t coul_shift;  /* 1 = potential-shift on Ewald energy (RF: c_rf always applied, A6) */
     int32_t ntypes;
@@ -99,7 +99,10 @@ void oracle_pair(const oracle_params* p, double r, double qq, double c6, double 
         }
         *F_lj = 12.0 * c12 / (r12 * r) - 6.0 * c6 / (r6 * r);
     }
-    if (p->coulomb == 0) {
+    if (p->coulomb == 2) {
+        *V_c = 0.0;
+        *F_c = 0.0;
+    } else if (p->coulomb == 0) {
         double b = p->beta;
         double g = TWO_OVER_SQRT_PI * b * exp(-b * b * r * r);
         if (!excluded) {

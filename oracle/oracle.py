@@ -29,7 +29,7 @@ EPSFAC = 138.935458  # reading A2
 class Params:
     rc: float
     ntypes: int
-    coulomb: str = "ewald"  # "ewald" | "rf"
+    coulomb: str = "ewald"  # "ewald" | "rf" | "none" (LJ only)
     beta: float = 0.0
     eps_rf: float = 0.0  # <= 0: infinity
     epsfac: float = EPSFAC
@@ -37,7 +37,7 @@ class Params:
     coul_shift: bool = True
 
     def c(self) -> _Params:
-        return _Params(0 if self.coulomb == "ewald" else 1, int(self.lj_shift), int(self.coul_shift),
+        return _Params({"ewald": 0, "rf": 1, "none": 2}[self.coulomb], int(self.lj_shift), int(self.coul_shift),
                        int(self.ntypes), float(self.rc), float(self.beta), float(self.eps_rf),
                        float(self.epsfac))
 

@@ -27,7 +27,7 @@ extern "C" int nb_init(const nb_params* p, nb_ctx** out)
     if (!p || !out) return NB_ERR_ARG;
     *out = nullptr;
     if (p->natoms <= 0 || p->ntypes <= 0 || p->ntypes > NB_MAX_TYPES || !p->lj_c6c12 || !finite_pos(p->rc)) return NB_ERR_ARG;
-    if (p->coulomb != NB_COUL_EWALD && p->coulomb != NB_COUL_RF) return NB_ERR_ARG;
+    if (p->coulomb != NB_COUL_EWALD && p->coulomb != NB_COUL_RF && p->coulomb != NB_COUL_NONE) return NB_ERR_ARG;
     if (p->excl_off && p->excl_off[p->natoms] > 0 && !p->excl_idx) return NB_ERR_ARG;
     if (cudaSetDevice(p->device) != cudaSuccess) return NB_ERR_CUDA;
     nb_ctx* c = new (std::nothrow) nb_ctx();

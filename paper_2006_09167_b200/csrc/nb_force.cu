@@ -141,7 +141,7 @@ __device__ __forceinline__ void pair_step(const NbConst& K, const float4* __rest
         const float2 rinv6 = mul2(mul2(rinv2, rinv2), rinv2);
         const float2 flj = mul2(fma2(c12, rinv6, nc6), rinv6);
         const float2 qq = mul2(I.q[p], qj);                   // epsfac folded into the i charge
-        float2 t1 = fma2(qq, rinv, flj);                      // (F_lj + A/r) r
+        float2 t1 = COUL == NB_COUL_NONE ? flj : fma2(qq, rinv, flj);   // (F_lj + A/r) r
         float2 mf = f2(1.f);
         if (MASKED) {
             mf = f2(((mbyte >> (2 * p)) & 1u) ? 1.f : 0.f, ((mbyte >> (2 * p + 1)) & 1u) ? 1.f : 0.f);
@@ -151,8 +151,10 @@ __device__ __forceinline__ void pair_step(const NbConst& K, const float4* __rest
         if (COUL == NB_COUL_EWALD) {
             bh = ewald_bh2(r2, K, p3);
             fs = fma2(rinv2, t1, neg2(mul2(qq, bh)));         // F/r = (F_lj r + A m/r)/r^2 - A beta^3 h
-        } else {
+        } else if (COUL == NB_COUL_RF) {
             fs = fma2(rinv2, t1, neg2(mul2(qq, f2(K.two_krf))));   // F/r = ... - 2 A k_rf
+        } else {
+            fs = mul2(rinv2, t1);                             // LJ only: charges are ignored
         }
         if (MASKED) fs = f2(w0 ? fs.x : 0.f, w1 ? fs.y : 0.f);
         else fs = mul2(fs, wc);
@@ -172,8 +174,10 @@ __device__ __forceinline__ void pair_step(const NbConst& K, const float4* __rest
                 const float2 ex = f2(__expf(-K.beta2 * r2.x), __expf(-K.beta2 * r2.y));
                 const float2 be = fma2(r2, bh, mul2(f2(K.beta * 1.1283791671f), ex));
                 vc = mul2(qq, add2(mul2(mf, add2(rinv, f2(-K.ewald_shift))), neg2(be)));
-            } else {
+            } else if (COUL == NB_COUL_RF) {
                 vc = mul2(qq, fma2(mf, rinv, fma2(f2(K.krf), r2, f2(-K.crf))));
+            } else {
+                vc = f2(0.f);
             }
             const float2 vl = mul2(mul2(mf, vlj), wc);
             vc = mul2(vc, wc);
@@ -515,8 +519,10 @@ int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial)
         NbStageTimer tm(c, NB_T_FORCE);
         if (c->prm.coulomb == NB_COUL_EWALD)
             rc = energy ? launch_force<NB_COUL_EWALD, true>(c, A) : launch_force<NB_COUL_EWALD, false>(c, A);
-        else
+        else if (c->prm.coulomb == NB_COUL_RF)
             rc = energy ? launch_force<NB_COUL_RF, true>(c, A) : launch_force<NB_COUL_RF, false>(c, A);
+        else
+            rc = energy ? launch_force<NB_COUL_NONE, true>(c, A) : launch_force<NB_COUL_NONE, false>(c, A);
         if (rc != NB_OK) return rc;
     }
     double* xf = c->fshift.p + NB_NSHIFT * 3;

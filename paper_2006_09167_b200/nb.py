@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libnb_b200.so")
 NB_OK = 0
 NB_ERR = {-1: "NB_ERR_ARG", -2: "NB_ERR_STATE", -3: "NB_ERR_CUTOFF", -4: "NB_ERR_BOX", -5: "NB_ERR_NOMEM",
           -6: "NB_ERR_CUDA", -7: "NB_ERR_OVERFLOW"}
-NB_COUL_EWALD, NB_COUL_RF = 0, 1
+NB_COUL_EWALD, NB_COUL_RF, NB_COUL_NONE = 0, 1, 2
 NB_MOD_NONE, NB_MOD_POTSHIFT = 0, 1
 NB_SHIFT_CENTER = 13
 
@@ -97,7 +97,7 @@ class Context:
         self.device = torch.device("cuda", device)
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         p = nb_params(self.natoms, self.ntypes, _hptr(lj), _hptr(eo), _hptr(ei), float(rc),
-                      NB_COUL_EWALD if coulomb == "ewald" else NB_COUL_RF, float(ewald_beta), float(ewald_rtol),
+                      {"ewald": NB_COUL_EWALD, "rf": NB_COUL_RF, "none": NB_COUL_NONE}[coulomb], float(ewald_beta), float(ewald_rtol),
                       float(eps_rf), float(epsfac), int(lj_modifier), int(coul_modifier), int(device),
                       C.c_void_p(self.stream.cuda_stream))
         self._h = C.c_void_p(0)

@@ -49,7 +49,7 @@ class Workload:
     rlist_inner: float
     nstlist: int
     nparts: int
-    coulomb: str = "ewald"  # "ewald" | "rf"
+    coulomb: str = "ewald"  # "ewald" | "rf" | "none" (LJ only)
     ewald_rtol: float = 1e-5
     delta_per_step: float = 2.5e-4  # nm/step drift along unit_dir
 
@@ -280,6 +280,37 @@ def small_water(nmol: int, box_len: float, seed: int, rc: float, rlist_outer: fl
     rot = _orient_without_clashes(rng, o_pos, box, 0.13)
     return _finish(f"water{3 * nmol}", rng, o_pos, rot, box, rc=rc, rlist_outer=rlist_outer,
                    rlist_inner=rlist_inner, nstlist=100, nparts=1, coulomb=coulomb)
+
+
+# Second workload of the paper (Fig. 6): a Lennard-Jones fluid whose cut-off is
+# swept to vary the number of pairs per atom ("157k-atom argon-like system"; the figure's values
+# are an image, only the recipe is taken).  Stand-in: one LJ type, no charges, no exclusions,
+# jittered simple-cubic lattice at 26 atoms/nm^3, sigma = 0.3345 nm, eps = 0.996 kJ/mol.
+LJ_SIGMA, LJ_EPS, LJ_RHO = 0.3345, 0.996, 26.0
+
+
+def lj_fluid(nside: int = 54, rc: float = 1.0, buffer_outer: float = 0.1, buffer_inner: float = 0.03,
+             seed: int = SEED_BASE + 10) -> Workload:
+    """nside^3 single-type LJ atoms (54^3 = 157 464), each its own 'molecule' in the motion recipe."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    n = nside**3
+    box_len = (n / LJ_RHO) ** (1.0 / 3.0)
+    spacing = box_len / nside
+    g = np.arange(nside)
+    sites = np.stack(np.meshgrid(g, g, g, indexing="ij"), axis=-1).reshape(-1, 3).astype(np.float64)
+    pos = (sites + 0.5) * spacing + rng.uniform(-0.15, 0.15, size=sites.shape) * spacing
+    box = np.full(3, box_len)
+    x = np.mod(pos, box).astype(np.float32)
+    x = np.where(x >= box.astype(np.float32), np.float32(0.0), x).astype(np.float32)
+    u = rng.normal(size=(n, 3))
+    u /= np.linalg.norm(u, axis=1, keepdims=True)
+    return Workload(
+        name=f"lj_fluid{n}_rc{rc:g}", x=x, q=np.zeros(n, np.float32), type=np.zeros(n, np.int32), box=box.astype(np.float32),
+        ntypes=1, lj_c6c12=lj_table(np.array([LJ_SIGMA]), np.array([LJ_EPS])),
+        excl_off=np.zeros(n + 1, np.int32), excl_idx=np.zeros(0, np.int32), mol_of_atom=np.arange(n, dtype=np.int32),
+        unit_dir=u.astype(np.float32), rc=rc, rlist_outer=rc + buffer_outer, rlist_inner=rc + buffer_inner,
+        nstlist=100, nparts=2, coulomb="none",
+    )
 
 
 def by_index(k: int, **kw) -> Workload:

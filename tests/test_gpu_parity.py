@@ -141,6 +141,33 @@ def test_small_rectangular_box(coulomb):
     assert rel_rms(d.forces(), ref.f) <= TOL_F
 
 
+def test_lj_only_flavour():
+    """LJ-only kernel flavour on the Fig. 6 stand-in (no charges, no exclusions) and on
+    a water box whose charges must be ignored; lists bit-exact, forces / energy / virial vs the oracle."""
+    w = W.lj_fluid(12, rc=0.9)
+    d = Driver(w)
+    d.put()
+    d.ctx.search(w.rlist_outer)
+    check_layout(d, w)
+    d.ctx.prune(w.rlist_inner)
+    check_lists(d, w, w.rlist_outer, w.rlist_inner)
+    ref = oracle_forces(w)
+    f, e, vir = d.forces(energy=True, virial=True)
+    assert rel_rms(f, ref.f) <= TOL_F
+    assert e[1] == 0.0 and abs(e[0] - ref.e_lj) / abs(ref.e_lj) <= TOL_E
+    assert np.linalg.norm(vir - ref.virial) / np.linalg.norm(ref.virial) <= TOL_E
+    assert rel_rms(d.forces(), ref.f) <= TOL_F
+    ww = W.small_water(150, 2.0, seed=23, rc=0.8, rlist_outer=0.9, rlist_inner=0.84, coulomb="none")
+    d = Driver(ww)
+    d.put()
+    d.ctx.search(ww.rlist_outer)
+    d.ctx.prune(ww.rlist_inner)
+    ref = oracle_forces(ww)
+    f, e = d.forces(energy=True)
+    assert rel_rms(f, ref.f) <= TOL_F
+    assert e[1] == 0.0 and abs(e[0] - ref.e_lj) / abs(ref.e_lj) <= TOL_E
+
+
 def test_modifiers_none_and_finite_eps_rf(small_rect):
     w = small_rect
     from paper_2006_09167_b200 import nb
