@@ -286,6 +286,39 @@ def test_config1_parity_and_rolling_prune(cfg1):
         assert np.array_equal(a, b)
 
 
+@pytest.mark.parametrize("which", ["cfg2_ewald", "cfg2_rf", "cfg4", "cfg3"])
+def test_full_size_configs_in_bench_schedule(which):
+    """BASELINE.json configs[2] (both Coulomb flavours), [4] and [3] at full size, driven the way bench.py
+    drives them (search, full prune, then rolling parts on the motion recipe): list parity on sampled
+    cluster ranges (the list oracle is O(n^2)), forces / energy / virial against the fp64 linked-cell
+    oracle (pinned equal to all-pairs), effective pair count against the oracle's."""
+    w = {"cfg2_ewald": lambda: W.config2("ewald"), "cfg2_rf": lambda: W.config2("rf"), "cfg4": W.config4,
+         "cfg3": W.config3}[which]()
+    d = Driver(w)
+    d.put()
+    d.ctx.search(w.rlist_outer)
+    check_layout(d, w)
+    d.ctx.prune(w.rlist_inner)
+    ncl = d.ctx.get_layout()["nclusters"]
+    for c0 in (0, ncl // 3 + 5, ncl - 16):
+        check_lists(d, w, w.rlist_outer, w.rlist_inner, c_range=(c0, c0 + 16))
+    ref = oracle_forces(w, method="cells")
+    f, e, vir = d.forces(energy=True, virial=True)
+    assert rel_rms(f, ref.f) <= TOL_F
+    assert abs(e.sum() - ref.energy) / abs(ref.energy) <= TOL_E
+    assert np.linalg.norm(vir - ref.virial) / np.linalg.norm(ref.virial) <= TOL_E
+    npairs, _ = d.ctx.count_pairs()
+    assert abs(npairs - ref.npairs) <= 2 + 1e-6 * ref.npairs     # fp32 vs fp64 at r = rc
+    fsum = np.abs(f.sum(axis=0)).max() / (np.sqrt((f**2).mean()) * w.natoms)
+    assert fsum < 1e-6                                           # T6 on the GPU
+    for t in (1, 2, w.nparts + 1):
+        x = w.positions_at(t)
+        d.put(x)
+        d.ctx.prune(w.rlist_inner, t % w.nparts, w.nparts)
+        r = oracle_forces(w, x=x, method="cells")
+        assert rel_rms(d.forces(), r.f) <= TOL_F
+
+
 def test_host_entry_points(cfg0):
     w = cfg0
     d = Driver(w)
