@@ -50,6 +50,8 @@ def parse_args():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[k] (default 2: ~96k atoms)")
     ap.add_argument("--coulomb", default="ewald", choices=["ewald", "rf"], help="config 2 only")
+    ap.add_argument("--water-nside", type=int, default=0,
+                    help="instead of a BASELINE config: nside^3 water molecules, run parameters of config 1 (PAPER.md Fig. 7 size sweep)")
     ap.add_argument("--lj-rc", type=float, default=0.0,
                     help="instead of a BASELINE config: the LJ-only fluid of PAPER.md Fig. 6 (157 464 atoms) at this cut-off, nm")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -62,13 +64,17 @@ def load_workload(args):
     from paper_2006_09167_b200 import workloads
     if args.lj_rc > 0:
         return workloads.lj_fluid(54, rc=args.lj_rc)
+    if args.water_nside > 0:
+        return workloads.water_box(args.water_nside)
     if args.config == 2:
         return workloads.config2(args.coulomb)
     return workloads.by_index(args.config)
 
 
 def workload_config(w, args, extra=None):
-    origin = "PAPER.md Fig. 6 stand-in (SURVEY 8.1 f2)" if args.lj_rc > 0 else f"BASELINE.json configs[{args.config}]"
+    origin = ("PAPER.md Fig. 6 stand-in (SURVEY 8.1 f2)" if args.lj_rc > 0 else
+              "PAPER.md Fig. 7 size sweep stand-in (SURVEY 8.1 f2)" if args.water_nside > 0 else
+              f"BASELINE.json configs[{args.config}]")
     cfg = {"workload": f"{origin} {w.name}: {w.natoms} atoms, box "
                        f"{float(w.box[0]):.4f}x{float(w.box[1]):.4f}x{float(w.box[2]):.4f} nm, {w.coulomb} rc={w.rc}, "
                        f"rlist_outer={w.rlist_outer}, rlist_inner={w.rlist_inner}, nstlist={w.nstlist}, "
@@ -375,7 +381,7 @@ def run_b200(args):
     force_us = 1e3 * f_ms / max(f_n, 1)
     achieved = flop_slot * slots_per_launch / (force_us * 1e-6) / 1e12 if f_n else 0.0
     roofline = {"bound": "alu", "kernel": "k_force (a7)", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-                "frac": achieved / peak_tflops, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((args.config, w.coulomb)) if args.lj_rc <= 0 else None,
+                "frac": achieved / peak_tflops, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((args.config, w.coulomb)) if args.lj_rc <= 0 and args.water_nside <= 0 else None,
                 "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one k_force launch, ncu --set full "
                                   "(profiles/, latest force_full summary); null = not captured for this workload",
                 "peak_source": f"derived: {N_SM} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x {sm_max} MHz (clocks.max.sm); "

@@ -313,5 +313,13 @@ def lj_fluid(nside: int = 54, rc: float = 1.0, buffer_outer: float = 0.1, buffer
     )
 
 
+def water_box(nside: int) -> Workload:
+    """Size sweep of the water workload (Fig. 7: 3k to 3M atoms): nside^3 molecules on
+    the jittered lattice of configs 1-3 at 33.4 molecules/nm^3, run parameters of config 1."""
+    L = (nside**3 / MOLECULES_PER_NM3) ** (1.0 / 3.0)
+    return _lattice_water(f"water{3 * nside**3}", SEED_BASE + 20 + nside, nside, 0, L, rc=1.0, rlist_outer=1.1,
+                          rlist_inner=1.03, nstlist=100, nparts=2)
+
+
 def by_index(k: int, **kw) -> Workload:
     return [config0, config1, config2, config3, config4][k](**kw)
