@@ -299,6 +299,7 @@ def run_reference(args):
 def run_b200(args):
     import torch
     import torch.distributed as dist
+    from paper_2006_09167_b200 import nb
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -340,6 +341,12 @@ def run_b200(args):
     # ---------------- device-resident leg: `value` ----------------
     for i in range(W):
         rep.step_device(i)
+    # Inside the timed region only the force kernel (the roofline's kernel) carries an event pair:
+    # every timed stage costs two event records per call (~3 us of stream time per stage and step;
+    # with all seven stages timed the step was 13-26 % longer).  The other stages are timed in a
+    # second pass over the same K steps that does not count towards `value`.
+    force_bit = 1 << nb.NB_T_NAMES.index("force")
+    ctx.timing_stages(force_bit)
     ctx.timing_enable(True)
     ctx.timing_read(reset=True)
     launches0 = ctx.get_stats()["kernel_launches"]
@@ -350,8 +357,14 @@ def run_b200(args):
     barrier()
     clocks = sampler.result()
     stages = ctx.timing_read(reset=True)
+    launches1 = ctx.get_stats()["kernel_launches"]
+    ctx.timing_stages(0xFFFFFFFF & ~force_bit)
+    rep.timed(rep.step_device, W, K)
+    stages_other = ctx.timing_read(reset=True)
+    stages = {k: (stages[k] if k == "force" else stages_other[k]) for k in stages}
+    ctx.timing_stages(0xFFFFFFFF)
     ctx.timing_enable(False)
-    launches = ctx.get_stats()["kernel_launches"] - launches0 - 1   # get_stats itself launches one counting kernel
+    launches = launches1 - launches0 - 1   # get_stats itself launches one counting kernel
     ms_max = max_over_ranks(ms)
     pairs_all = sum_over_ranks(float(pairs))
     value = pairs_all / (ms_max * 1e-3)
@@ -403,6 +416,7 @@ def run_b200(args):
                 "work_efficiency": pairs / max(slots, 1),
                 "stage_us": per_stage_us,
                 "stage_share_of_step": {k: v[0] / ms for k, v in stages.items()},
+                "stage_timing": "force: event pair inside the timed region; other stages: second pass over the same steps",
                 "list": {k: st[k] for k in ("nsuper", "n_sci_entries", "n_joint_outer", "n_pairs_outer", "n_pairs_inner",
                                             "n_excl_masks", "n_work_units")}}
         if world == 1 and not args.no_cpu_baseline:

@@ -59,7 +59,7 @@ typedef struct {
     float rc;                        /* interaction cut-off, nm (LJ and Coulomb; interact iff r^2 < rc^2) */
     int32_t coulomb;                 /* NB_COUL_* */
     float ewald_beta;                /* nm^-1; if <= 0 derived from ewald_rtol: erfc(beta*rc) = rtol.
-                                        (beta*rc)^2 must be <= 16 (range of the correction fit) */
+                                        (beta*rc)^2 must be <= 12 (range of the correction fit) */
     float ewald_rtol;
     float eps_rf;                    /* reaction-field dielectric; <= 0 or inf -> infinity (eps_r = 1) */
     float epsfac;                    /* 1/(4 pi eps0); 0 -> 138.935458 kJ mol^-1 nm e^-2 */
@@ -88,7 +88,7 @@ typedef struct {
 } nb_stats;
 
 /* Creates a context.  Copies the LJ table and exclusions.  NB_ERR_ARG on bad sizes,
- * an exclusion index out of range, rc <= 0, or (beta*rc)^2 > 16. */
+ * an exclusion index out of range, rc <= 0, or (beta*rc)^2 > 12. */
 int nb_init(const nb_params* p, nb_ctx** out);
 
 /* (a1) Coordinate staging.  x [dev] natoms*3 fp32, q [dev] natoms,
@@ -150,13 +150,17 @@ int nb_count_pairs(nb_ctx*, int64_t* n_interacting, int64_t* n_excluded);
 enum { NB_T_PUT = 0,      /* (a1) nb_put_atoms: copies + cluster-order refresh */
        NB_T_GRID = 1,     /* (a2) gridding + cluster sort */
        NB_T_SEARCH = 2,   /* (a3)+(a5) pair search count/fill passes, unit table upload */
-       NB_T_MASKS = 3,    /* (a4) exclusion masks (+ list statistics) */
+       NB_T_MASKS = 3,    /* (a4) exclusion masks, (a5) compact inner list set-up and its launch order (+ list statistics) */
        NB_T_PRUNE = 4,    /* (a6) prune kernel */
        NB_T_FORCE = 5,    /* (a7) force kernel alone */
        NB_T_REDUCE = 6,   /* (a8) gather to caller order, virial/energy finalisation */
        NB_T_NKINDS = 7 };
 /* on != 0: record an event pair around every stage from now on.  Off by default. */
 int nb_timing_enable(nb_ctx*, int on);
+/* Restricts the timing to the stages whose bit (1u << NB_T_*) is set in stage_mask (default: all).
+ * Every timed stage costs two event records per call, about 1.5 us of stream time each on a B200:
+ * time one stage when the surrounding step is being timed as well. */
+int nb_timing_stages(nb_ctx*, unsigned stage_mask);
 /* Synchronises the stream, then returns the accumulated milliseconds and number of timed
  * intervals per stage (host arrays of NB_T_NKINDS; either may be NULL); reset != 0 zeroes
  * the accumulators afterwards. */

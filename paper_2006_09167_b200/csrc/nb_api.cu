@@ -290,6 +290,13 @@ extern "C" int nb_timing_enable(nb_ctx* c, int on)
     return NB_OK;
 }
 
+extern "C" int nb_timing_stages(nb_ctx* c, unsigned stage_mask)
+{
+    if (!c) return NB_ERR_ARG;
+    c->timing_mask = stage_mask;
+    return NB_OK;
+}
+
 extern "C" int nb_timing_read(nb_ctx* c, double* ms, int64_t* count, int reset)
 {
     if (!c) return NB_ERR_ARG;

@@ -151,6 +151,7 @@ struct nb_ctx {
 
     // --- per-stage device timing (nb_timing_enable / nb_timing_read) ---
     bool timing = false;
+    unsigned timing_mask = ~0u;                // stages to time (nb_timing_stages)
     struct TimRec { int kind; cudaEvent_t e0, e1; };
     std::vector<TimRec> tim_open;              // recorded, not yet read
     std::vector<cudaEvent_t> tim_pool;         // recycled events
@@ -175,7 +176,7 @@ struct NbStageTimer {
     }
     NbStageTimer(nb_ctx* c_, int kind_) : c(c_), kind(kind_)
     {
-        if (!c->timing) return;
+        if (!c->timing || !((c->timing_mask >> kind_) & 1u)) return;
         e0 = get(c);
         e1 = get(c);
         cudaEventRecord(e0, c->stream);

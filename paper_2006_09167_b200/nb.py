@@ -24,7 +24,7 @@ NB_SHIFT_CENTER = 13
 EXPORTS = ["nb_init", "nb_put_atoms", "nb_put_atoms_host", "nb_search", "nb_prune", "nb_forces",
            "nb_forces_host", "nb_free", "nb_last_error", "nb_get_layout", "nb_get_slots", "nb_list_count",
            "nb_list_dump", "nb_get_stats", "nb_measure_fp32_peak", "nb_count_pairs", "nb_timing_enable",
-           "nb_timing_read"]
+           "nb_timing_read", "nb_timing_stages"]
 NB_T_NAMES = ["put", "grid", "search", "masks", "prune", "force", "reduce"]
 
 
@@ -193,6 +193,9 @@ class Context:
 
     def timing_enable(self, on=True):
         self._check(lib().nb_timing_enable(self._h, C.c_int(int(on))))
+
+    def timing_stages(self, mask=0xFFFFFFFF):
+        self._check(lib().nb_timing_stages(self._h, C.c_uint(int(mask))))
 
     def timing_read(self, reset=True):
         """{stage: (milliseconds, intervals)} accumulated since the last reset."""
