@@ -211,8 +211,8 @@ extern "C" void nb_free(nb_ctx* c)
     c->ent_count.release(); c->ent_jbegin.release(); c->jl.release(); c->imask_outer.release();
     c->plane_outer.release(); c->plane_inner.release(); c->plane_excl.release(); c->batch_ent.release(); c->scan_tmp.release();
     c->scan_blk.release(); c->excl_masks.release(); c->counters.release(); c->units_canon.release();
-    c->units_sorted.release(); c->fshift.release(); c->unit_order.release(); c->prune_order.release();
-    c->il_off.release(); c->ilm_off.release(); c->seg.release(); c->unit_pos.release(); c->seg_pos.release(); c->seg_ci.release(); c->il.release(); c->ilm.release();
+    c->units_sorted.release(); c->fshift.release(); c->unit_order.release(); for (auto& po : c->prune_orders) po.d.release();
+    c->il_off.release(); c->ilm_off.release(); c->seg.release(); c->unit_pos.release(); c->seg_pos.release(); c->seg_ci.release(); c->il.release(); c->ilm.release(); c->ol.release(); c->ol_cnt.release();
     delete c;
 }
 

@@ -130,10 +130,12 @@ struct nb_ctx {
     std::vector<int4> h_units;
     DevBuf<int4> units_canon, units_sorted;    // {entry slot, batch begin, batch end, sci}
     DevBuf<int32_t> unit_order;                // canonical unit index, longest first (force kernel launch order)
-    DevBuf<int32_t> prune_order;               // canonical unit indices, each rolling part sorted longest first
-    std::vector<int32_t> h_prune_order;
-    int prune_order_nparts = 0;
-    int64_t prune_order_search = -1;
+    // prune launch order: (canonical unit*8 + i-cluster), each rolling part longest list first; one
+    // cached table per recently used nparts, rebuilt lazily after a search
+    struct PruneOrder { int nparts = 0; int64_t search = -1; DevBuf<int32_t> d; };
+    PruneOrder prune_orders[4];
+    int prune_order_next = 0;
+    std::vector<int32_t> h_prune_order, h_unit_order, h_seg_sorted;   // host scratch / copies made at search time
     int nunits = 0;
 
     // --- compact inner list (a6 -> a7): per (work unit, i-cluster) the j-clusters whose inner mask bit is set ---
@@ -147,6 +149,9 @@ struct nb_ctx {
     std::vector<int32_t> h_caps;               // host scratch
     DevBuf<int32_t> il;                        // cj of cluster pairs without a mask for this i-cluster
     DevBuf<int2> ilm;                          // {cj, mask ref} of cluster pairs with a mask, plus each segment's tail
+    // compact OUTER list (a3 -> a6): what the prune kernel streams; written once per search
+    DevBuf<int2> ol;                           // {cj, unit-local joint slot | masked << 30}; segment at il offset + ilm offset
+    DevBuf<int32_t> ol_cnt;                    // [nunits*8] entries per segment (index: unit launch position*8 + i-cluster)
     DevBuf<double> fshift;                     // [27*3] per-shift i-force sums (virial)
 
     // --- per-stage device timing (nb_timing_enable / nb_timing_read) ---

@@ -337,7 +337,8 @@ __global__ void __launch_bounds__(256) k_ilist_build(const int4* __restrict__ un
                                                      const int* __restrict__ il_off, const int* __restrict__ ilm_off,
                                                      const int* __restrict__ seg_pos, int4* __restrict__ seg,
                                                      int2* __restrict__ seg_ci, int32_t* __restrict__ il,
-                                                     int2* __restrict__ ilm, int cj_dummy)
+                                                     int2* __restrict__ ilm, int2* __restrict__ ol, int* __restrict__ ol_cnt,
+                                                     int cj_dummy)
 {
     const int4 u = units[blockIdx.x];   // units in launch order
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, s0 = blockIdx.x * 8 + warp;
@@ -347,6 +348,19 @@ __global__ void __launch_bounds__(256) k_ilist_build(const int4* __restrict__ un
         seg[s].x = o;
         seg[s].y = om;
         seg_ci[s] = make_int2(u.w * 8 + warp, nb_half_shift_id(u.x - u.w * NB_NHALF));
+    }
+    {   // compact outer list of this i-cluster: what the prune kernel streams
+        int2* ols = ol + o + om;
+        const unsigned lt = (1u << lane) - 1u;
+        int n = 0;
+        for (int b = u.y; b < u.z; b++) {
+            const unsigned bits = plane[(size_t)b * 8 + warp], eb = plane_excl[(size_t)b * 8 + warp] & bits;
+            if ((bits >> lane) & 1u)
+                ols[n + __popc(bits & lt)] =
+                    make_int2(jl[(size_t)b * 32 + lane].x, ((b - u.y) * 32 + lane) | (int)(((eb >> lane) & 1u) << 30));
+            n += __popc(bits);
+        }
+        if (lane == 0) ol_cnt[s0] = n;
     }
     nb_ilist_write([&](int b) { return plane[(size_t)(u.y + b) * 8 + warp]; }, u.y, u.z, warp, lane, cj_dummy, plane_excl, jl,
                    il + o, ilm + om, reinterpret_cast<int2*>(&seg[s]) + 1);
@@ -558,6 +572,7 @@ int nbi_search(nb_ctx* c, float rlist)
         return (c->h_units[a].z - c->h_units[a].y) > (c->h_units[b].z - c->h_units[b].y);
     });
     for (int i = 0; i < c->nunits; i++) pos[order[i]] = i;
+    c->h_unit_order = order;
 
     NB_CUDA(c, c->jl.ensure(std::max<int64_t>(c->njslots, 1), st));
     NB_CUDA(c, c->imask_outer.ensure(std::max<int64_t>(c->njslots, 1), st));
@@ -657,6 +672,8 @@ int nbi_search(nb_ctx* c, float rlist)
             for (int l = 0; l <= maxlen; l++) start[l + 1] += start[l];
             c->nseg_launch = start[maxlen];   // everything before the length-0 bucket
             for (int i = 0; i < nseg; i++) pos[i] = start[maxlen - (cu[i] + cm[i] - 3)]++;
+            c->h_seg_sorted.resize(nseg);   // sorted position -> (unit launch position*8 + i-cluster)
+            for (int i = 0; i < nseg; i++) c->h_seg_sorted[pos[i]] = i;
             NB_CUDA(c, c->seg_pos.ensure(nseg, st));
             NB_CUDA(c, c->seg_ci.ensure(nseg, st));
             NB_CUDA(c, cudaMemcpyAsync(c->seg_pos.p, pos.data(), sizeof(int) * nseg, cudaMemcpyHostToDevice, st));
@@ -664,8 +681,10 @@ int nbi_search(nb_ctx* c, float rlist)
         }
         NB_CUDA(c, c->il.ensure((size_t)tot[0] + 4, st));
         NB_CUDA(c, c->ilm.ensure((size_t)tot[1] + 4, st));
+        NB_CUDA(c, c->ol.ensure((size_t)tot[0] + (size_t)tot[1] + 4, st));
+        NB_CUDA(c, c->ol_cnt.ensure(nseg, st));
         k_ilist_build<<<c->nunits, 256, 0, st>>>(c->units_sorted.p, c->plane_inner.p, c->plane_excl.p, c->jl.p, c->il_off.p,
-                                                 c->ilm_off.p, c->seg_pos.p, c->seg.p, c->seg_ci.p, c->il.p, c->ilm.p, c->nclusters);
+                                                 c->ilm_off.p, c->seg_pos.p, c->seg.p, c->seg_ci.p, c->il.p, c->ilm.p, c->ol.p, c->ol_cnt.p, c->nclusters);
         NB_LAUNCH_CHECK(c);
     } else {
         std::vector<unsigned long long> ones(16, ~0ull);

@@ -25,6 +25,8 @@ struct PruneArgs {
     const int* order;         // launch order of this part: canonical unit indices, longest first
     const int2* jl;
     const uint32_t* plane_outer;
+    const int2* ol;           // compact outer list (nb_list.cu k_ilist_build)
+    const int* ol_cnt;
     uint32_t* plane_inner;
     const float4* xq;
     float box[3];
@@ -40,106 +42,132 @@ struct PruneArgs {
     int2* ilm;
 };
 
-// 8 exact (A12) distance checks of this lane's j atom; DIAG keeps only pairs b > a.
+// 8 exact (A12) distance checks of this lane's j atom against the i atoms (packed pairs 2p, 2p+1:
+// the FP32x2 instructions round each half like their scalar forms, and x_a + (-x_b) is x_a - x_b
+// exactly, so list parity with the oracle is unchanged); DIAG keeps only pairs b > a.
 template <bool DIAG>
-__device__ __forceinline__ bool prune_checks(const float (&xi)[8], const float (&yi)[8], const float (&zi)[8],
+__device__ __forceinline__ bool prune_checks(const float2 (&xi)[4], const float2 (&yi)[4], const float2 (&zi)[4],
                                              const float4 xj, float rl2, bool diag, int k)
 {
+    const float2 nx = make_float2(-xj.x, -xj.x), ny = make_float2(-xj.y, -xj.y), nz = make_float2(-xj.z, -xj.z);
     bool found = false;
 #pragma unroll
-    for (int a = 0; a < 8; a++) {
-        const float dx = __fsub_rn(xi[a], xj.x), dy = __fsub_rn(yi[a], xj.y), dz = __fsub_rn(zi[a], xj.z);
-        const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-        bool ok = d2 < rl2;
-        if (DIAG) ok = ok && (!diag || k > a);   // zero-shift diagonal: only b > a are pairs
-        found = found || ok;
+    for (int p = 0; p < 4; p++) {
+        const float2 dx = __fadd2_rn(xi[p], nx), dy = __fadd2_rn(yi[p], ny), dz = __fadd2_rn(zi[p], nz);
+        const float2 d2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+        bool ok0 = d2.x < rl2, ok1 = d2.y < rl2;
+        if (DIAG) {   // zero-shift diagonal: only b > a are pairs
+            ok0 = ok0 && (!diag || k > 2 * p);
+            ok1 = ok1 && (!diag || k > 2 * p + 1);
+        }
+        found = found || ok0 || ok1;
     }
     return found;
 }
 
-__global__ void __launch_bounds__(256) k_prune(PruneArgs A)
+// One survivor-append step: 4 j-clusters (lane groups), entry e = {cj, unit-local joint slot | masked << 30}.
+struct PruneState {
+    int nu, nm;
+};
+
+template <bool DIAG>
+__device__ __forceinline__ void prune_step(const PruneArgs& A, const float2 (&xi)[4], const float2 (&yi)[4],
+                                           const float2 (&zi)[4], const int2 e, const float4 x, const bool valid, const int ci,
+                                           const int b0, const int lane, unsigned* res, int32_t* il, int2* ilm,
+                                           PruneState& st)
 {
-    __shared__ int2 s_q[8][40];                          // {cj, unit-local joint slot}
-    __shared__ unsigned s_res[8][NB_MAX_UNIT_BATCHES];   // inner mask words of this warp's plane
-    const int ucan = A.order[blockIdx.x];
+    const int g = lane >> 3, k = lane & 7;
+    const int cj = e.x, slot = e.y & 0x3fffffff;
+    const bool found = prune_checks<DIAG>(xi, yi, zi, x, A.rl2, DIAG && cj == ci, k);
+    const unsigned gm = __ballot_sync(0xffffffffu, found && valid);
+    const bool keep = k == 0 && ((gm >> (8 * g)) & 0xffu) != 0u;     // group leader of a surviving cluster pair
+    const bool masked = (e.y >> 30) & 1;
+    const unsigned bu = __ballot_sync(0xffffffffu, keep && !masked), bm = __ballot_sync(0xffffffffu, keep && masked);
+    if (keep) {
+        const unsigned lt = (1u << lane) - 1u;
+        atomicOr(&res[slot >> 5], 1u << (slot & 31));
+        if (!masked) il[st.nu + __popc(bu & lt)] = cj;
+        else ilm[st.nm + __popc(bm & lt)] = make_int2(cj, A.jl[(size_t)b0 * 32 + slot].y);
+    }
+    st.nu += __popc(bu);
+    st.nm += __popc(bm);
+}
+
+// One warp per block = one i-cluster of one work unit: streams its compact outer list segment.
+__global__ void __launch_bounds__(32) k_prune(PruneArgs A)
+{
+    __shared__ unsigned s_res[NB_MAX_UNIT_BATCHES];   // inner mask words of this i-cluster's plane
+    const int sidx = A.order[blockIdx.x];   // canonical unit * 8 + i-cluster, longest list first within the part
+    const int ucan = sidx >> 3, warp = sidx & 7;
     const int4 u = A.units[ucan];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7;
+    const int lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7;
     const int sci = u.w, h = u.x - sci * NB_NHALF, ci = sci * 8 + warp;
+    const int s0 = A.unit_pos[ucan] * 8 + warp;
+    int4* sg = &A.seg[A.seg_pos[s0]];
+    const int2 off = *reinterpret_cast<const int2*>(sg);
+    const int n = A.ol_cnt[s0];
+    const int2* __restrict__ ol = A.ol + off.x + off.y;
+    int32_t* il = A.il + off.x;
+    int2* ilm = A.ilm + off.y;
+    const int ns = (n + 3) >> 2;
+    int2 ea = make_int2(ci, 0), eb = ea, ea2 = ea, eb2 = ea;
+    if (ns > 0) {
+        ea = ol[min(g, n - 1)];
+        eb = ol[min(4 + g, n - 1)];
+        ea2 = ol[min(8 + g, n - 1)];
+        eb2 = ol[min(12 + g, n - 1)];
+    }
     int sx, sy, sz;
     nb_shift_vec(nb_half_shift_id(h), sx, sy, sz);
-    float xi[8], yi[8], zi[8];
+    float2 xi[4], yi[4], zi[4];
 #pragma unroll
-    for (int a = 0; a < 8; a++) {
-        const float4 v = A.xq[ci * 8 + a];
-        xi[a] = __fmaf_rn((float)sx, A.box[0], v.x);   // A12: t = fmaf(s, L, x_a), one rounding
-        yi[a] = __fmaf_rn((float)sy, A.box[1], v.y);
-        zi[a] = __fmaf_rn((float)sz, A.box[2], v.z);
+    for (int p = 0; p < 4; p++) {
+        const float4 v0 = A.xq[ci * 8 + 2 * p], v1 = A.xq[ci * 8 + 2 * p + 1];
+        // A12: t = fmaf(s, L, x_a), one rounding
+        xi[p] = make_float2(__fmaf_rn((float)sx, A.box[0], v0.x), __fmaf_rn((float)sx, A.box[0], v1.x));
+        yi[p] = make_float2(__fmaf_rn((float)sy, A.box[1], v0.y), __fmaf_rn((float)sy, A.box[1], v1.y));
+        zi[p] = make_float2(__fmaf_rn((float)sz, A.box[2], v0.z), __fmaf_rn((float)sz, A.box[2], v1.z));
     }
-    int2* q = s_q[warp];
-    unsigned* res = s_res[warp];
+    unsigned* res = s_res;
     if (lane < NB_MAX_UNIT_BATCHES) res[lane] = 0u;
-    const unsigned lt = (1u << lane) - 1u;
-    int nq = 0;
-    unsigned bits = A.plane_outer[(size_t)u.y * 8 + warp];
-    int cje = ((bits >> lane) & 1u) ? A.jl[(size_t)u.y * 32 + lane].x : 0;
     __syncwarp();
-    for (int b = u.y; b < u.z; b++) {
-        const bool last = b + 1 == u.z;
-        unsigned bits_n = 0;
-        int cje_n = 0;
-        if (!last) {
-            bits_n = A.plane_outer[(size_t)(b + 1) * 8 + warp];
-            if ((bits_n >> lane) & 1u) cje_n = A.jl[(size_t)(b + 1) * 32 + lane].x;
-        }
-        if ((bits >> lane) & 1u) q[nq + __popc(bits & lt)] = make_int2(cje, (b - u.y) * 32 + lane);
-        nq += __popc(bits);
-        __syncwarp();
-        int done = 0;
-        const int need = last ? 1 : 4;   // the unit's last batch also runs the partly filled step
-        if (nq >= need) {
-            bool valid = g < nq;
-            int2 ce = valid ? q[g] : make_int2(ci, 0);
-            float4 xj = A.xq[ce.x * 8 + k];
-            while (true) {
-                done += 4;
-                const bool more = nq - done >= need;
-                bool valid_n = false;
-                int2 ce_n = ce;
-                float4 xj_n = xj;
-                if (more) {
-                    valid_n = done + g < nq;
-                    ce_n = valid_n ? q[done + g] : make_int2(ci, 0);
-                    xj_n = A.xq[ce_n.x * 8 + k];
-                }
-                const bool diag = ce.x == ci && h == 0;
-                bool found;
-                if (__any_sync(0xffffffffu, diag)) found = prune_checks<true>(xi, yi, zi, xj, A.rl2, diag, k);
-                else found = prune_checks<false>(xi, yi, zi, xj, A.rl2, false, k);
-                const unsigned gm = __ballot_sync(0xffffffffu, found && valid);
-                if (k == 0 && ((gm >> (8 * g)) & 0xffu)) atomicOr(&res[ce.y >> 5], 1u << (ce.y & 31));
-                if (!more) break;
-                valid = valid_n;
-                ce = ce_n;
-                xj = xj_n;
+    PruneState st = {0, 0};
+    if (ns > 0) {
+        // two alternating register sets (a: even steps, b: odd steps); j coordinates two steps ahead,
+        // list entries four steps ahead, indices clamped to the segment (as in the force kernel)
+        float4 xa = A.xq[ea.x * 8 + k], xb = A.xq[eb.x * 8 + k];
+        int s = 0;
+        // The joint list of a zero-shift element holds cj >= ci in ascending order, so the diagonal
+        // cluster pair (cj == ci), if listed, is in the first step of the segment: only that step
+        // needs the b > a predicate.
+        if (h == 0) {
+            prune_step<true>(A, xi, yi, zi, ea, xa, g < n, ci, u.y, lane, res, il, ilm, st);
+            ea = ea2;
+            xa = A.xq[ea.x * 8 + k];
+            ea2 = ol[min(4 * 4 + g, n - 1)];
+            if (ns > 1) {
+                prune_step<false>(A, xi, yi, zi, eb, xb, 4 + g < n, ci, u.y, lane, res, il, ilm, st);
+                eb = eb2;
+                xb = A.xq[eb.x * 8 + k];
+                eb2 = ol[min(4 * 5 + g, n - 1)];
             }
-            done = min(done, nq);
+            s = 2;
         }
-        const int rem = nq - done;
-        int2 t = make_int2(0, 0);
-        if (lane < rem) t = q[done + lane];
-        __syncwarp();
-        if (lane < rem) q[lane] = t;
-        __syncwarp();
-        nq = rem;
-        bits = bits_n;
-        cje = cje_n;
+        for (; s + 1 < ns; s += 2) {
+            prune_step<false>(A, xi, yi, zi, ea, xa, 4 * s + g < n, ci, u.y, lane, res, il, ilm, st);
+            ea = ea2;
+            xa = A.xq[ea.x * 8 + k];
+            ea2 = ol[min(4 * (s + 4) + g, n - 1)];
+            prune_step<false>(A, xi, yi, zi, eb, xb, 4 * (s + 1) + g < n, ci, u.y, lane, res, il, ilm, st);
+            eb = eb2;
+            xb = A.xq[eb.x * 8 + k];
+            eb2 = ol[min(4 * (s + 5) + g, n - 1)];
+        }
+        if (s < ns) prune_step<false>(A, xi, yi, zi, ea, xa, 4 * s + g < n, ci, u.y, lane, res, il, ilm, st);
     }
     __syncwarp();
+    nb_ilist_finish(st.nu, st.nm, u.y * 8 + warp, lane, A.cj_dummy, il, ilm, reinterpret_cast<int2*>(sg) + 1);
     if (lane < u.z - u.y) A.plane_inner[(size_t)(u.y + lane) * 8 + warp] = res[lane];
-    int4* sg = &A.seg[A.seg_pos[A.unit_pos[ucan] * 8 + warp]];
-    const int2 off = *reinterpret_cast<const int2*>(sg);
-    nb_ilist_write([&](int b) { return res[b]; }, u.y, u.z, warp, lane, A.cj_dummy, A.plane_excl, A.jl, A.il + off.x, A.ilm + off.y,
-                   reinterpret_cast<int2*>(sg) + 1);
 }
 
 }  // namespace
@@ -151,27 +179,39 @@ int nbi_prune(nb_ctx* c, float rlist_inner, int part, int nparts)
     c->last_nparts = nparts;
     c->st.prune_count++;
     if (u1 <= u0) return NB_OK;
-    if (c->prune_order_nparts != nparts || c->prune_order_search != c->st.search_count) {
-        // launch order inside each rolling part: longest work unit first, so that the last
-        // wave of blocks is made of short units; rebuilt once per search / change of nparts
-        c->h_prune_order.resize(nu);
-        for (int i = 0; i < nu; i++) c->h_prune_order[i] = i;
+    // Launch order inside each rolling part: longest i-cluster list first, so that the last
+    // wave of blocks is made of short lists.  Derived in one pass from the force kernel's global
+    // longest-first order (made at search time); cached per nparts until the next search.
+    nb_ctx::PruneOrder* po = nullptr;
+    for (auto& e : c->prune_orders)
+        if (e.nparts == nparts && e.search == c->st.search_count) po = &e;
+    if (!po) {
+        po = &c->prune_orders[c->prune_order_next];
+        c->prune_order_next = (c->prune_order_next + 1) % 4;
+        std::vector<int32_t> fill(nparts), part_of(nu);
         for (int p = 0; p < nparts; p++) {
             const long long a = (long long)p * nu / nparts, b = (long long)(p + 1) * nu / nparts;
-            std::stable_sort(c->h_prune_order.begin() + a, c->h_prune_order.begin() + b, [&](int x, int y) {
-                return (c->h_units[x].z - c->h_units[x].y) > (c->h_units[y].z - c->h_units[y].y);
-            });
+            fill[p] = (int)(a * 8);
+            for (long long i = a; i < b; i++) part_of[i] = p;
         }
-        NB_CUDA(c, c->prune_order.ensure(nu, c->stream));
-        NB_CUDA(c, cudaMemcpyAsync(c->prune_order.p, c->h_prune_order.data(), sizeof(int) * nu, cudaMemcpyHostToDevice, c->stream));
-        c->prune_order_nparts = nparts;
-        c->prune_order_search = c->st.search_count;
+        c->h_prune_order.resize(nu * 8);
+        for (long long t = 0; t < nu * 8; t++) {
+            const int s0 = c->h_seg_sorted[t], ucan = c->h_unit_order[s0 >> 3];
+            c->h_prune_order[fill[part_of[ucan]]++] = ucan * 8 + (s0 & 7);
+        }
+        NB_CUDA(c, po->d.ensure(nu * 8, c->stream));
+        NB_CUDA(c, cudaMemcpyAsync(po->d.p, c->h_prune_order.data(), sizeof(int) * nu * 8, cudaMemcpyHostToDevice, c->stream));
+        NB_CUDA(c, cudaStreamSynchronize(c->stream));   // h_prune_order is reused
+        po->nparts = nparts;
+        po->search = c->st.search_count;
     }
     PruneArgs A;
     A.units = c->units_canon.p;
-    A.order = c->prune_order.p + u0;
+    A.order = po->d.p + (size_t)u0 * 8;
     A.jl = c->jl.p;
     A.plane_outer = c->plane_outer.p;
+    A.ol = c->ol.p;
+    A.ol_cnt = c->ol_cnt.p;
     A.plane_inner = c->plane_inner.p;
     A.xq = c->xq.p;
     for (int k = 0; k < 3; k++) A.box[k] = c->box[k];
@@ -182,7 +222,7 @@ int nbi_prune(nb_ctx* c, float rlist_inner, int part, int nparts)
     A.unit_pos = c->unit_pos.p; A.seg_pos = c->seg_pos.p; A.seg = c->seg.p;
     A.il = c->il.p; A.ilm = c->ilm.p;
     NbStageTimer tm(c, NB_T_PRUNE);
-    k_prune<<<u1 - u0, 256, 0, c->stream>>>(A);
+    k_prune<<<(u1 - u0) * 8, 32, 0, c->stream>>>(A);
     NB_LAUNCH_CHECK(c);
     return NB_OK;
 }
