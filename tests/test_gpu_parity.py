@@ -319,6 +319,26 @@ def test_full_size_configs_in_bench_schedule(which):
         assert rel_rms(d.forces(), r.f) <= TOL_F
 
 
+def test_work_efficiency_table_against_oracle():
+    """SURVEY 8.1 (f3), Fig. 5 definition: the table's numerator is the oracle's count of atom pairs
+    within rc (interacting + excluded), its denominator 64 x the listed cluster pairs; the efficiency falls
+    with the buffer, the pruned list is at least as efficient as the searched one, and both stay below 1x1."""
+    from paper_2006_09167_b200 import work_efficiency as WE
+    tab = WE.efficiency_table(10, [0.8, 1.0], [0.0, 0.1, 0.2])
+    w = W.water_box(10)
+    for rc in (0.8, 1.0):
+        rows = [r for r in tab["rows"] if r["rc"] == rc]
+        assert len(rows) == 3
+        ref = O.forces(w.x, w.q, w.type, w.box, w.lj_c6c12, w.excl_off, w.excl_idx,
+                       O.Params(rc=rc, ntypes=w.ntypes, coulomb="ewald", beta=O.beta_from_rtol(rc, 1e-5)))
+        for r in rows:
+            assert abs(r["pairs_within_rc"] - (ref.npairs + ref.npairs_excl)) <= 2
+            assert r["cluster_pairs_pruned"] <= r["cluster_pairs_searched"]
+            assert r["eff_searched"] <= r["eff_pruned"] < r["eff_1x1_ideal"] <= 1.0
+        effs = [r["eff_searched"] for r in rows]
+        assert effs[0] > effs[1] > effs[2]
+
+
 def test_host_entry_points(cfg0):
     w = cfg0
     d = Driver(w)
