@@ -339,6 +339,51 @@ def test_work_efficiency_table_against_oracle():
         assert effs[0] > effs[1] > effs[2]
 
 
+@pytest.mark.parametrize("n", [1, 2, 7, 9, 65])
+def test_tiny_and_ragged_systems(n):
+    """Degenerate sizes: one atom (no pair at all), two atoms (one cluster, diagonal pair only), fewer atoms
+    than a cluster, one more than a cluster, one more than a super-cluster; sparse box, most slots padding."""
+    rng = np.random.default_rng(100 + n)
+    L = 2.8
+    # n ADJACENT sites of a jittered 0.35 nm lattice (a compact droplet in an otherwise empty box): nearest
+    # neighbours at liquid-like distances, so the relative force tolerance is meaningful
+    g = np.stack(np.meshgrid(*[np.arange(8)] * 3, indexing="ij"), axis=-1).reshape(-1, 3)
+    order = np.argsort(((g - 3.5) ** 2).sum(axis=1), kind="stable")
+    x = ((g[order[:n]] + 0.5) * (L / 8) + rng.uniform(-0.04, 0.04, (n, 3))).astype(np.float32)
+    q = rng.uniform(-0.5, 0.5, n).astype(np.float32)
+    typ = (np.arange(n) % 2).astype(np.int32)
+    tab = W.lj_table(np.array([0.3, 0.25]), np.array([0.6, 0.3]))
+    eo, ei = np.zeros(n + 1, np.int32), np.zeros(0, np.int32)
+    import torch
+    from paper_2006_09167_b200 import nb
+    for coul in ("ewald", "rf", "none"):
+        ctx = nb.Context(n, tab, eo, ei, rc=1.0, coulomb=coul, ewald_rtol=1e-5)
+        dev = torch.device("cuda", 0)
+        xd, qd, td = (torch.from_numpy(a).to(dev) for a in (x, q, typ))
+        f = torch.full((n, 3), float("nan"), dtype=torch.float32, device=dev)
+        e = torch.zeros(2, dtype=torch.float64, device=dev)
+        v = torch.zeros(9, dtype=torch.float64, device=dev)
+        box = np.full(3, L, np.float32)
+        ctx.put_atoms(xd, qd, td, box)
+        ctx.search(1.2)
+        for part in range(3):
+            ctx.prune(1.1, part, 3)          # more parts than work units is legal
+        ctx.forces(f, e, v)
+        torch.cuda.synchronize()
+        ref = O.forces(x, q, typ, box, tab, eo, ei,
+                       O.Params(rc=1.0, ntypes=2, coulomb=coul, beta=O.beta_from_rtol(1.0, 1e-5) if coul == "ewald" else 0.0))
+        fg = f.cpu().numpy().astype(np.float64)
+        assert np.isfinite(fg).all()
+        if ref.npairs == 0:
+            assert np.all(fg == 0.0) and float(e.sum()) == 0.0
+        else:
+            assert rel_rms(fg, ref.f) <= TOL_F
+            assert abs(float(e.sum()) - ref.energy) <= TOL_E * max(abs(ref.energy), abs(ref.e_lj) + abs(ref.e_coul))
+            assert np.linalg.norm(v.cpu().numpy().reshape(3, 3) - ref.virial) <= TOL_E * np.linalg.norm(ref.virial)
+        assert ctx.count_pairs()[0] == ref.npairs
+        ctx.close()
+
+
 def test_host_entry_points(cfg0):
     w = cfg0
     d = Driver(w)
