@@ -164,7 +164,8 @@ class Replica:
         """Inputs already in HBM (the `value` leg)."""
         w, c = self.w, self.ctx
         fr = t % w.nstlist
-        c.put_atoms(self.x_dev[fr], self.q_dev, self.t_dev, w.box)
+        # charges and types are constant (PAPER.md L71): handed over with the coordinates of a search step only
+        c.put_atoms(self.x_dev[fr], self.q_dev if fr == 0 else None, self.t_dev if fr == 0 else None, w.box)
         if fr == 0:
             c.search(w.rlist_outer)
             c.prune(w.rlist_inner, 0, 1)           # first use of a fresh list: full prune (PAPER.md L187)
@@ -177,7 +178,8 @@ class Replica:
         """Host buffers in, host buffers out (the `e2e` leg): copies inside the timed region."""
         w, c = self.w, self.ctx
         fr = t % w.nstlist
-        c.put_atoms_host(self.x_host[fr].numpy(), self.q_host.numpy(), self.t_host.numpy(), w.box)
+        c.put_atoms_host(self.x_host[fr].numpy(), self.q_host.numpy() if fr == 0 else None,
+                         self.t_host.numpy() if fr == 0 else None, w.box)
         if fr == 0:
             c.search(w.rlist_outer)
             c.prune(w.rlist_inner, 0, 1)
@@ -381,7 +383,7 @@ def run_b200(args):
         n = w.natoms
         n_energy_steps = sum(1 for i in range(W, W + K) if i % w.nstlist == 0)
         e2e = {"value": sum_over_ranks(float(pairs_h)) / (ms_h_max * 1e-3), "unit": UNIT,
-               "h2d_bytes_per_step": n * (12 + 4 + 4),
+               "h2d_bytes_per_step": n * 12 + n * 8 * n_energy_steps / max(K, 1),   # x every step; q, type on search steps
                "d2h_bytes_per_step": n * 12 + (11 * 8 * n_energy_steps) / max(K, 1),
                "ms_per_step": ms_h_max / max(K, 1)}
 

@@ -93,7 +93,9 @@ int nb_init(const nb_params* p, nb_ctx** out);
 
 /* (a1) Coordinate staging.  x [dev] natoms*3 fp32, q [dev] natoms,
  * type [dev] natoms (0 <= type < ntypes), box host [3] (Lx,Ly,Lz > 0).  Copies them; if a
- * grid exists and the box is unchanged, also refreshes the cluster-ordered (x,y,z,q) array. */
+ * grid exists and the box is unchanged, also refreshes the cluster-ordered (x,y,z,q) array.
+ * q and/or type may be NULL after the first call: "unchanged since the previous nb_put_atoms"
+ * (only positions change from step to step); NB_ERR_ARG on the first call. */
 int nb_put_atoms(nb_ctx*, const float* x, const float* q, const int32_t* type, const float box[3]);
 /* Same with host pointers (pageable or pinned); copies are enqueued on the stream. */
 int nb_put_atoms_host(nb_ctx*, const float* x, const float* q, const int32_t* type, const float box[3]);

@@ -111,7 +111,9 @@ extern "C" int nb_init(const nb_params* p, nb_ctx** out)
 static int put_atoms_common(nb_ctx* c, const float* x, const float* q, const int32_t* type, const float box[3], cudaMemcpyKind kind)
 {
     if (!c) return NB_ERR_ARG;
-    if (!x || !q || !type || !box) return nb_fail(c, NB_ERR_ARG, "nb_put_atoms: null argument");
+    if (!x || !box) return nb_fail(c, NB_ERR_ARG, "nb_put_atoms: null argument");
+    if ((!q || !type) && !c->have_atoms)
+        return nb_fail(c, NB_ERR_ARG, "nb_put_atoms: q and type may be NULL only after a call that passed them");
     for (int k = 0; k < 3; k++)
         if (!finite_pos(box[k])) return nb_fail(c, NB_ERR_BOX, "box[%d] = %g is not positive", k, box[k]);
     cudaStream_t st = c->stream;
@@ -120,8 +122,8 @@ static int put_atoms_common(nb_ctx* c, const float* x, const float* q, const int
     const bool device = kind == cudaMemcpyDeviceToDevice;
     if (!device) {
         NB_CUDA(c, cudaMemcpyAsync(c->x.p, x, sizeof(float) * 3 * n, kind, st));
-        NB_CUDA(c, cudaMemcpyAsync(c->q.p, q, sizeof(float) * n, kind, st));
-        NB_CUDA(c, cudaMemcpyAsync(c->type.p, type, sizeof(int32_t) * n, kind, st));
+        if (q) NB_CUDA(c, cudaMemcpyAsync(c->q.p, q, sizeof(float) * n, kind, st));
+        if (type) NB_CUDA(c, cudaMemcpyAsync(c->type.p, type, sizeof(int32_t) * n, kind, st));
     }
     for (int k = 0; k < 3; k++) c->box[k] = box[k];
     c->have_atoms = true;

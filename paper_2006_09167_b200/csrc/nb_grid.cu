@@ -277,10 +277,11 @@ __global__ void __launch_bounds__(256) k_put(int n, const float* __restrict__ x,
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const float px = x[3 * i], py = x[3 * i + 1], pz = x[3 * i + 2], pq = q[i];
+    const float px = x[3 * i], py = x[3 * i + 1], pz = x[3 * i + 2];
     cx[3 * i] = px; cx[3 * i + 1] = py; cx[3 * i + 2] = pz;
-    cq[i] = pq;
-    ctype[i] = type[i];
+    float pq;
+    if (q) { pq = q[i]; cq[i] = pq; } else pq = cq[i];   // NULL: unchanged since the previous call
+    if (type) ctype[i] = type[i];
     if (xq) {
         const char4 im = image[i];
         xq[slot_of_atom[i]] = make_float4(__fmaf_rn(-(float)im.x, box.x, px), __fmaf_rn(-(float)im.y, box.y, py),

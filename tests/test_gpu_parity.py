@@ -384,6 +384,28 @@ def test_tiny_and_ragged_systems(n):
         ctx.close()
 
 
+def test_put_atoms_without_charges_and_types(cfg0):
+    """q / type = NULL means "unchanged since the previous nb_put_atoms" (device and host entry points);
+    NULL on the very first call is an argument error."""
+    import torch
+    from paper_2006_09167_b200 import nb
+    w = cfg0
+    d = Driver(w)
+    with pytest.raises(nb.NbError):
+        d.ctx.put_atoms(torch.from_numpy(w.x).to(d.dev), None, None, w.box)
+    d.put()
+    d.ctx.search(w.rlist_outer)
+    x1 = w.positions_at(3)
+    d.put(x1)
+    f_full = d.forces()
+    d.put()                                         # back to frame 0 with everything
+    d.ctx.put_atoms(torch.from_numpy(x1).to(d.dev), None, None, w.box)
+    assert rel_rms(d.forces(), f_full) < 1e-6      # same inputs up to atomic summation order
+    d.put()
+    d.ctx.put_atoms_host(x1, None, None, w.box)
+    assert rel_rms(d.forces(), f_full) < 1e-6
+
+
 def test_host_entry_points(cfg0):
     w = cfg0
     d = Driver(w)
