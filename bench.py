@@ -298,6 +298,50 @@ def run_reference(args):
     return 0
 
 
+class Ranks:
+    """Barrier and max / sum over the ranks of a torchrun launch.  The path does not shard ("replicas
+    only"): every rank runs an independent replica, so these are the ONLY
+    inter-rank operations -- timing scalars, no data-path collective.  `device` is the CUDA device
+    of the rank under NCCL, or "cpu" under gloo (tests/test_bench_dist.py)."""
+
+    def __init__(self, world, device):
+        self.world, self.device = world, device
+
+    def _sync(self):
+        import torch
+        if str(self.device) != "cpu":
+            torch.cuda.synchronize(self.device)
+
+    def barrier(self):
+        import torch.distributed as dist
+        self._sync()
+        if self.world > 1:
+            dist.barrier()
+        self._sync()
+
+    def _reduce(self, v, op):
+        if self.world == 1:
+            return v
+        import torch
+        import torch.distributed as dist
+        t = torch.tensor([v], dtype=torch.float64, device=self.device)
+        dist.all_reduce(t, op=op)
+        return float(t.item())
+
+    def max(self, v):
+        import torch.distributed as dist
+        return self._reduce(v, dist.ReduceOp.MAX)
+
+    def sum(self, v):
+        import torch.distributed as dist
+        return self._reduce(v, dist.ReduceOp.SUM)
+
+    def job_value(self, units_local, ms_local):
+        """Whole-job throughput: units all ranks processed / the slowest rank's device time."""
+        ms_max = self.max(ms_local)
+        return self.sum(float(units_local)) / (ms_max * 1e-3), ms_max
+
+
 def run_b200(args):
     import torch
     import torch.distributed as dist
@@ -312,25 +356,8 @@ def run_b200(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     dev = torch.device("cuda", local_rank)
 
-    def barrier():
-        torch.cuda.synchronize(dev)
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize(dev)
-
-    def max_over_ranks(v):
-        if world == 1:
-            return v
-        t = torch.tensor([v], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
-
-    def sum_over_ranks(v):
-        if world == 1:
-            return v
-        t = torch.tensor([v], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        return float(t.item())
+    ranks = Ranks(world, dev)
+    barrier, max_over_ranks, sum_over_ranks = ranks.barrier, ranks.max, ranks.sum
 
     w = load_workload(args)
     rep = Replica(w, local_rank, flush=not args.no_flush)
