@@ -201,7 +201,7 @@ class Replica:
             self.step_device(t)
             n_int, _ = self.ctx.count_pairs()
             self.pairs_at_frame.append(n_int)
-            self.slots_at_frame.append(64 * self.ctx.list_count(1))
+            self.slots_at_frame.append(self.ctx.count_slots())
 
     def timed(self, step_fn, t0, nsteps):
         """Times nsteps steps starting at schedule position t0 with one CUDA-event pair per step on

@@ -146,6 +146,10 @@ int nb_measure_fp32_peak(nb_ctx*, double* fma_per_s);
  * that are force-field exclusions (*n_excluded; they contribute only the Ewald/RF correction).
  * Host outputs; either may be NULL.  Synchronises. */
 int nb_count_pairs(nb_ctx*, int64_t* n_interacting, int64_t* n_excluded);
+/* Atom-pair slots the force kernel evaluates over the current inner list (the paper's "raw" pair
+ * count, L167): the inner list is kept at half-j-cluster granularity (8 x 4 atoms = 32 slots per
+ * entry; cluster pairs that carry an exclusion mask stay whole, 64 slots).  Host output.  Synchronises. */
+int nb_count_slots(nb_ctx*, int64_t* slots);
 
 /* Per-stage device timing with CUDA events on the context's stream ("CUDA events
  * on the caller's stream").  Stage ids index the arrays of nb_timing_read. */

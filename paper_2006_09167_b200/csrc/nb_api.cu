@@ -285,6 +285,13 @@ extern "C" int nb_count_pairs(nb_ctx* c, int64_t* n_interacting, int64_t* n_excl
     return nbi_count_pairs(c, n_interacting, n_excluded);
 }
 
+extern "C" int nb_count_slots(nb_ctx* c, int64_t* slots)
+{
+    if (!c || !slots) return NB_ERR_ARG;
+    if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "no list yet (call nb_search)");
+    return nbi_count_slots(c, slots);
+}
+
 extern "C" int nb_timing_enable(nb_ctx* c, int on)
 {
     if (!c) return NB_ERR_ARG;

@@ -210,12 +210,13 @@ __global__ void __launch_bounds__(32, 16) k_force(ForceArgs A)
     const int2 cnt = make_int2(sg.z, sg.w);
     const int* __restrict__ il = A.il + sg.x;
     const int2* __restrict__ ilm = A.ilm + sg.y;
-    const int ns = cnt.x >> 2;
+    const int ns = cnt.x >> 3;             // unmasked steps: 8 half-clusters (4 atoms each) per step
+    const int g8 = lane >> 2, k4 = lane & 3;   // lane -> (half-cluster of the step, atom in it)
     // first list entries of both loops are requested before anything else is waited for
     int cj = 0, cj_n = 0;
     if (ns > 0) {
-        cj = il[g];
-        cj_n = il[4 * min(1, ns - 1) + g];
+        cj = il[g8] * 4 + k4;              // unmasked path: cj* hold this lane's j SLOT (4 * half-cluster + atom)
+        cj_n = il[8 * min(1, ns - 1) + g8] * 4 + k4;
     }
     int sx, sy, sz;
     nb_shift_vec(sid, sx, sy, sz);
@@ -236,8 +237,8 @@ __global__ void __launch_bounds__(32, 16) k_force(ForceArgs A)
     float4 xj = make_float4(0.f, 0.f, 0.f, 0.f);
     int tj = 0;
     if (ns > 0) {   // j data of the first unmasked step: in flight during the masked steps
-        xj = A.xq[cj * 8 + k];
-        tj = A.type_slot[cj * 8 + k];
+        xj = A.xq[cj];
+        tj = A.type_slot[cj];
     }
     __syncwarp();
 
@@ -256,7 +257,7 @@ __global__ void __launch_bounds__(32, 16) k_force(ForceArgs A)
         if (valid) red_add_v4(&A.f4[ce.x * 8 + k], -(fjx.x + fjx.y), -(fjy.x + fjy.y), -(fjz.x + fjz.y));
     }
 
-    // Cluster pairs without a mask: always full steps of 4 j-clusters.  ptxas schedules memory
+    // Cluster pairs without a mask, at half-cluster granularity: always full steps of 8 half-clusters.  ptxas schedules memory
     // operations whose consumer is an iteration away at the END of the step, so the j data of
     // step s+1 is loaded there; to make that load an L1 hit the lines are prefetched one step
     // earlier still (distance 2), and the list entries are read 3 steps ahead (indices clamped).
@@ -264,19 +265,19 @@ __global__ void __launch_bounds__(32, 16) k_force(ForceArgs A)
     float4 xj1 = xj;
     int tj1 = tj;
     if (ns > 0) {
-        cj2 = il[4 * min(2, ns - 1) + g];
-        cj3 = il[4 * min(3, ns - 1) + g];
-        xj1 = A.xq[cj_n * 8 + k];
-        tj1 = A.type_slot[cj_n * 8 + k];
+        cj2 = il[8 * min(2, ns - 1) + g8] * 4 + k4;
+        cj3 = il[8 * min(3, ns - 1) + g8] * 4 + k4;
+        xj1 = A.xq[cj_n];
+        tj1 = A.type_slot[cj_n];
     }
 #pragma unroll 2   // (unroll 3, the period of the rotation below, was measured slower)
     for (int s = 0; s < ns; s++) {
-        const int cj4 = il[4 * min(s + 4, ns - 1) + g];
-        const float4 x2 = A.xq[cj2 * 8 + k];
-        const int t2 = A.type_slot[cj2 * 8 + k];
+        const int cj4 = il[8 * min(s + 4, ns - 1) + g8] * 4 + k4;
+        const float4 x2 = A.xq[cj2];
+        const int t2 = A.type_slot[cj2];
         float2 fjx, fjy, fjz;
         pair_step<COUL, ENERGY, false>(K, ljw + tj, nt1, I, fix, fiy, fiz, elj, ecoul, xj, 0xffu, 0xffu, fjx, fjy, fjz, p3);
-        red_add_v4(&A.f4[cj * 8 + k], -(fjx.x + fjx.y), -(fjy.x + fjy.y), -(fjz.x + fjz.y));
+        red_add_v4(&A.f4[cj], -(fjx.x + fjx.y), -(fjy.x + fjy.y), -(fjz.x + fjz.y));
         cj = cj_n; xj = xj1; tj = tj1;
         cj_n = cj2; xj1 = x2; tj1 = t2;
         cj2 = cj3; cj3 = cj4;
@@ -462,6 +463,22 @@ __global__ void __launch_bounds__(256) k_count_pairs(ForceArgs A, unsigned long 
     }
 }
 
+// Atom-pair slots of the inner list as the force kernel evaluates it: 32 per real (non-dummy) half-cluster
+// entry, 64 per masked cluster pair.  One thread per segment; statistics only.
+__global__ void k_count_slots(const int4* __restrict__ seg, int nseg, const int* __restrict__ il, int nhalf_real,
+                              unsigned long long* __restrict__ out)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long n = 0;
+    if (i < nseg) {
+        const int4 sg = seg[i];
+        for (int e = 0; e < sg.z; e++) n += il[sg.x + e] < nhalf_real ? 32u : 0u;
+        n += 64ull * sg.w;
+    }
+    for (int d = 16; d > 0; d >>= 1) n += __shfl_xor_sync(0xffffffffu, n, d);
+    if ((threadIdx.x & 31) == 0 && n) atomicAdd(out, n);
+}
+
 template <int COUL, bool ENERGY>
 int launch_force(nb_ctx* c, const ForceArgs& A)
 {
@@ -565,6 +582,23 @@ int nbi_measure_fp32_peak(nb_ctx* c, double* fma_per_s)
     cudaEventDestroy(e1);
     out.release();
     *fma_per_s = (double)grid * 256 * iters * 64.0 / (best * 1e-3);
+    return NB_OK;
+}
+
+int nbi_count_slots(nb_ctx* c, int64_t* slots)
+{
+    cudaStream_t st = c->stream;
+    NB_CUDA(c, c->counters.ensure(8, st));
+    NB_CUDA(c, cudaMemsetAsync(c->counters.p, 0, 8 * sizeof(long long), st));
+    if (c->nseg_launch > 0) {
+        k_count_slots<<<(c->nseg_launch + 127) / 128, 128, 0, st>>>(c->seg.p, c->nseg_launch, c->il.p, 2 * c->nclusters,
+                                                                   (unsigned long long*)c->counters.p);
+        NB_LAUNCH_CHECK(c);
+    }
+    long long v = 0;
+    NB_CUDA(c, cudaMemcpyAsync(&v, c->counters.p, sizeof(v), cudaMemcpyDeviceToHost, st));
+    NB_CUDA(c, cudaStreamSynchronize(st));
+    *slots = v;
     return NB_OK;
 }
 

@@ -213,34 +213,30 @@ __host__ __device__ inline void nb_shift_vec(int id, int& sx, int& sy, int& sz)
 int nb_fail(nb_ctx* c, int code, const char* fmt, ...);
 
 #ifdef __CUDACC__
-#ifndef NB_TAIL_POLICY
-#define NB_TAIL_POLICY 1
-#endif
-// Closes an inner list segment of nu unmasked + nm masked entries (one warp; the entries must be
-// visible to the warp).  The (nu mod 4) unmasked entries left over: if they fit into the free
-// lanes of the masked steps that run anyway they go there (ref 0 = all-ones mask); otherwise the
-// unmasked list is filled up to a multiple of 4 with dummy clusters -- a full unmasked step is
-// cheaper than an extra masked one.
+// The compact inner list is kept at HALF j-cluster granularity (4 atoms): an unmasked entry is the
+// half-cluster index hc = 2*cj + half, whose atoms are the slots 4*hc .. 4*hc+3.  The prune kernel
+// keeps a half iff one of its atoms is within rlist_inner of the i-cluster, which skips about a
+// tenth of the atom-pair slots a whole-cluster list evaluates (the cluster-pair "split" of the
+// paper's GPU lists).  Masked entries {cj, mask ref} stay whole clusters.
+//
+// Closes a segment of nu unmasked half entries + nm masked entries (one warp): the unmasked count
+// is filled up to a multiple of 8 (one force-kernel step = 8 half-clusters) with dummy half-clusters.
 __device__ __forceinline__ void nb_ilist_finish(int nu, int nm, int salt, int lane, int cj_dummy,
                                                 int32_t* __restrict__ il, int2* __restrict__ ilm, int2* __restrict__ cnt)
 {
-    const int rem = nu & 3;
-    if (rem != 0 && (NB_TAIL_POLICY == 0 || (nm > 0 && (nm + rem + 3) / 4 == (nm + 3) / 4))) {
-        if (lane < rem) ilm[nm + lane] = make_int2(il[nu - rem + lane], 0);
-        nu -= rem;
-        nm += rem;
-    } else if (rem != 0) {
-        if (lane < 4 - rem) il[nu + lane] = cj_dummy + ((salt + lane) & (NB_NDUMMY - 1));
-        nu += 4 - rem;
+    const int rem = nu & 7;
+    if (rem != 0) {
+        if (lane < 8 - rem) il[nu + lane] = 2 * cj_dummy + ((salt + lane) & (2 * NB_NDUMMY - 1));
+        nu += 8 - rem;
     }
     if (lane == 0) *cnt = make_int2(nu, nm);
 }
 
 // Writes the compact inner list segment of (unit, i-cluster warp) from the unit's inner mask
-// words `bits_of(b)` (b = batch index relative to the unit).  Entries whose exclusion mask is
-// trivial for this i-cluster go to `il` (cj only), the others to `ilm` {cj, mask ref}; the
-// unmasked count is made a multiple of 4 (see below) so that the force kernel's unmasked steps
-// are always full.  One warp, all 32 lanes.
+// words `bits_of(b)` (b = batch index relative to the unit), keeping BOTH halves of every
+// cluster (used after a search: inner := outer).  Entries whose exclusion mask is trivial for
+// this i-cluster go to `il` (two half-cluster indices), the others to `ilm` {cj, mask ref}.
+// One warp, all 32 lanes.
 template <typename BitsOf>
 __device__ __forceinline__ void nb_ilist_write(BitsOf bits_of, int b0, int b1, int warp, int lane, int cj_dummy,
                                                const uint32_t* __restrict__ plane_excl, const int2* __restrict__ jl,
@@ -253,10 +249,11 @@ __device__ __forceinline__ void nb_ilist_write(BitsOf bits_of, int b0, int b1, i
         const unsigned eb = plane_excl[(size_t)b * 8 + warp] & bits, nb = bits & ~eb;
         if ((bits >> lane) & 1u) {
             const int2 e = jl[(size_t)b * 32 + lane];
-            if ((nb >> lane) & 1u) il[nu + __popc(nb & lt)] = e.x;
+            if ((nb >> lane) & 1u)
+                *reinterpret_cast<int2*>(&il[nu + 2 * __popc(nb & lt)]) = make_int2(2 * e.x, 2 * e.x + 1);
             else ilm[nm + __popc(eb & lt)] = e;
         }
-        nu += __popc(nb);
+        nu += 2 * __popc(nb);
         nm += __popc(eb);
     }
     __syncwarp();
@@ -290,4 +287,5 @@ int nbi_list_dump(nb_ctx* c, int which, int32_t* ci, int32_t* cj, int32_t* shift
                   int32_t* part);
 int nbi_measure_fp32_peak(nb_ctx* c, double* fma_per_s);   // nb_force.cu
 int nbi_count_pairs(nb_ctx* c, int64_t* n_interacting, int64_t* n_excluded);   // nb_force.cu
+int nbi_count_slots(nb_ctx* c, int64_t* slots);            // nb_force.cu
 int nbi_exclusive_scan(nb_ctx* c, const int32_t* in, int32_t* out, int64_t n, int32_t* total_dev);  // nb_list.cu

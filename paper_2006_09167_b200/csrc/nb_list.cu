@@ -327,8 +327,8 @@ __global__ void k_ilist_caps(const int4* __restrict__ units, int nunits, const u
         nu += __popc(bits & ~eb);
         nm += __popc(eb);
     }
-    capu[i] = (nu + 3) & ~3;
-    capm[i] = nm + 3;
+    capu[i] = (2 * nu + 7) & ~7;   // half-cluster entries, multiple of 8
+    capm[i] = nm;
 }
 
 // After a search, one block per work unit (launch order): inner := outer.
@@ -666,12 +666,12 @@ int nbi_search(nb_ctx* c, float rlist)
             const int* cu = c->h_caps.data();
             const int* cm = cu + nseg;
             int maxlen = 0;
-            for (int i = 0; i < nseg; i++) maxlen = std::max(maxlen, cu[i] + cm[i] - 3);
+            for (int i = 0; i < nseg; i++) maxlen = std::max(maxlen, cu[i] + 2 * cm[i]);
             std::vector<int32_t> start(maxlen + 2, 0), pos(nseg);
-            for (int i = 0; i < nseg; i++) start[maxlen - (cu[i] + cm[i] - 3) + 1]++;
+            for (int i = 0; i < nseg; i++) start[maxlen - (cu[i] + 2 * cm[i]) + 1]++;
             for (int l = 0; l <= maxlen; l++) start[l + 1] += start[l];
             c->nseg_launch = start[maxlen];   // everything before the length-0 bucket
-            for (int i = 0; i < nseg; i++) pos[i] = start[maxlen - (cu[i] + cm[i] - 3)]++;
+            for (int i = 0; i < nseg; i++) pos[i] = start[maxlen - (cu[i] + 2 * cm[i])]++;
             c->h_seg_sorted.resize(nseg);   // sorted position -> (unit launch position*8 + i-cluster)
             for (int i = 0; i < nseg; i++) c->h_seg_sorted[pos[i]] = i;
             NB_CUDA(c, c->seg_pos.ensure(nseg, st));

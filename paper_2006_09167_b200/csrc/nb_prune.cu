@@ -80,14 +80,15 @@ __device__ __forceinline__ void prune_step(const PruneArgs& A, const float2 (&xi
     const int cj = e.x, slot = e.y & 0x3fffffff;
     const bool found = prune_checks<DIAG>(xi, yi, zi, x, A.rl2, DIAG && cj == ci, k);
     const unsigned gm = __ballot_sync(0xffffffffu, found && valid);
-    const bool keep = k == 0 && ((gm >> (8 * g)) & 0xffu) != 0u;     // group leader of a surviving cluster pair
     const bool masked = (e.y >> 30) & 1;
-    const unsigned bu = __ballot_sync(0xffffffffu, keep && !masked), bm = __ballot_sync(0xffffffffu, keep && masked);
+    const bool keep = k == 0 && ((gm >> (8 * g)) & 0xffu) != 0u;              // leader of a surviving cluster pair
+    const bool keep_half = (lane & 3) == 0 && ((gm >> lane) & 0xfu) != 0u;    // leader of a surviving half (4 atoms)
+    const unsigned bu = __ballot_sync(0xffffffffu, keep_half && !masked), bm = __ballot_sync(0xffffffffu, keep && masked);
+    const unsigned lt = (1u << lane) - 1u;
+    if (keep_half && !masked) il[st.nu + __popc(bu & lt)] = 2 * cj + ((lane >> 2) & 1);
     if (keep) {
-        const unsigned lt = (1u << lane) - 1u;
         atomicOr(&res[slot >> 5], 1u << (slot & 31));
-        if (!masked) il[st.nu + __popc(bu & lt)] = cj;
-        else ilm[st.nm + __popc(bm & lt)] = make_int2(cj, A.jl[(size_t)b0 * 32 + slot].y);
+        if (masked) ilm[st.nm + __popc(bm & lt)] = make_int2(cj, A.jl[(size_t)b0 * 32 + slot].y);
     }
     st.nu += __popc(bu);
     st.nm += __popc(bm);

@@ -24,7 +24,7 @@ NB_SHIFT_CENTER = 13
 EXPORTS = ["nb_init", "nb_put_atoms", "nb_put_atoms_host", "nb_search", "nb_prune", "nb_forces",
            "nb_forces_host", "nb_free", "nb_last_error", "nb_get_layout", "nb_get_slots", "nb_list_count",
            "nb_list_dump", "nb_get_stats", "nb_measure_fp32_peak", "nb_count_pairs", "nb_timing_enable",
-           "nb_timing_read", "nb_timing_stages"]
+           "nb_timing_read", "nb_timing_stages", "nb_count_slots"]
 NB_T_NAMES = ["put", "grid", "search", "masks", "prune", "force", "reduce"]
 
 
@@ -190,6 +190,12 @@ class Context:
         a, b = C.c_int64(), C.c_int64()
         self._check(lib().nb_count_pairs(self._h, C.byref(a), C.byref(b)))
         return a.value, b.value
+
+    def count_slots(self):
+        """Atom-pair slots the force kernel evaluates over the inner list (raw pair count)."""
+        n = C.c_int64()
+        self._check(lib().nb_count_slots(self._h, C.byref(n)))
+        return n.value
 
     def timing_enable(self, on=True):
         self._check(lib().nb_timing_enable(self._h, C.c_int(int(on))))
