@@ -38,7 +38,7 @@ UNIT = "pairs/s"
 FLOP_PER_SLOT = {"ewald": 55.75, "rf": 36.75, "none": 31.75}
 # DRAM bytes of one force-kernel launch from the committed ncu --set full capture (profiles/r1c_force_full_cfg2.md);
 # the kernel is ALU-bound, its HBM traffic is ~0.2 % of what the HBM roofline would allow in the same time.
-NCU_DRAM_BYTES_PER_LAUNCH = {(2, "ewald"): 12.6e6}
+NCU_DRAM_BYTES_PER_LAUNCH = {(2, "ewald"): 14.8e6}
 N_SM, FP32_LANES_PER_SM = 148, 128   # B200_PROFILING.md: 148 SMs; 128 FP32 lanes/SM (4 SMSP x 32)
 
 
