@@ -6,15 +6,16 @@
 // Ewald correction on FMA hardware (L137); one kernel per combination of electrostatics and
 // energy/no-energy to avoid conditionals (L139).
 //
-// Thread mapping (differs from the paper's 8x4-per-warp tiles): a block is the
-// 8 i-clusters of one super-cluster working through one chunk of the joint j list; warp w owns
-// i-cluster w, whose 8 atoms sit in registers of every lane.  Lanes own j atoms: a step takes
-// the next 4 j-clusters whose mask bit w is set (32 j atoms) and every lane evaluates its j
-// atom against the 8 i atoms.  Consequences: no shuffle in the inner loop (the j force is
-// private to its lane and leaves with ONE vector atomic per j atom per cluster pair, i.e.
-// atomics at cluster granularity), no per-pair shared-memory load of i data, mask skipping
-// costs nothing (set bits are compacted, not tested one by one), and the i forces (8 x 3
-// registers) are reduced across lanes once per work unit.
+// Thread mapping (differs from the paper's 8x4-per-warp tiles): one thread
+// block = one warp = one i-cluster working through one segment of the compact inner list that the
+// prune kernel wrote for it.  The 8 i atoms sit in registers of every lane as 4 packed pairs.
+// Lanes own j atoms: an unmasked step takes the next 8 half j-clusters (4 atoms each, 32 j atoms),
+// a masked step 4 whole j-clusters with their exclusion masks; every lane evaluates its j atom
+// against the 8 i atoms, two at a time with packed FP32x2 instructions.  Consequences: no shuffle
+// in the inner loop (the j force is private to its lane and leaves with ONE vector atomic per j
+// atom per step, i.e. atomics at cluster granularity), no per-pair shared-memory load of i data,
+// no mask tests (the list holds survivors only), and the i forces (8 x 3 registers) are reduced
+// across lanes once per segment.
 #include "nb_internal.h"
 
 #include "ewald_corr_coeffs.h"
@@ -47,10 +48,6 @@ __device__ __forceinline__ void red_add_v4(float4* addr, float x, float y, float
 
 // Single-instruction MUFU forms: the arguments are clamped away from zero/denormals by the
 // caller (r^2 >= 1e-6 or distinct atoms, monic Q(r^2) >= 1/30), so the denormal fix-up code of rsqrtf()/__fdividef() is dead weight.
-__device__ __forceinline__ void prefetch_l1(const void* p)
-{
-    asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
-}
 __device__ __forceinline__ float rsqrt_fast(float x)
 {
     float y;

@@ -141,7 +141,7 @@ struct nb_ctx {
     // --- compact inner list (a6 -> a7): per (work unit, i-cluster) the j-clusters whose inner mask bit is set ---
     DevBuf<int32_t> il_off, ilm_off;           // [nunits*8] scan scratch: first entry of the segment in il / ilm
     DevBuf<int4> seg;                          // [nunits*8], one per (work unit, i-cluster), longest outer list first:
-                                               // {il offset, ilm offset, unmasked entries (multiple of 4), masked entries}
+                                               // {il offset, ilm offset, unmasked half-cluster entries (multiple of 8), masked entries}
     DevBuf<int32_t> unit_pos;                  // canonical unit index -> launch position (inverse of unit_order)
     DevBuf<int32_t> seg_pos;                   // [nunits*8] (unit launch position*8 + i-cluster) -> index into seg (longest first)
     DevBuf<int2> seg_ci;                       // [nunits*8] {i-cluster, shift id} of each seg entry
