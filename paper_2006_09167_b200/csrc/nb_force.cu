@@ -187,8 +187,8 @@ __device__ __forceinline__ void pair_step(const NbConst& K, const float4* __rest
 template <int COUL, bool ENERGY>
 __global__ void __launch_bounds__(32, 16) k_force(ForceArgs A)
 {
-    // Paired LJ table of this block: s_ljp[(w*4 + p)*nt1 + tj] = (-6c6, -6c6', 12c12, 12c12') of the
-    // i atoms 2p, 2p+1 of i-cluster w against j type tj: one LDS.128 feeds both packed operands.
+    // Paired LJ table of this block's i-cluster: s_ljp[p*nt1 + tj] = (-6c6, -6c6', 12c12, 12c12') of the
+    // i atoms 2p, 2p+1 against j type tj: one LDS.128 feeds both packed operands.
     extern __shared__ float4 s_ljp[];
     const NbConst& K = A.kc;
     const int lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7;
@@ -196,7 +196,6 @@ __global__ void __launch_bounds__(32, 16) k_force(ForceArgs A)
     const int2 sc = A.seg_ci[blockIdx.x];
     const int ci = sc.x, sid = sc.y, warp = ci & 7;
     const int nt1 = K.ntypes1;
-    // each warp builds its own part of the table: no block-level barrier
     float4* ljw = s_ljp;
     for (int i = lane; i < 4 * nt1; i += 32) {
         const int p = i / nt1, tj = i - p * nt1;
@@ -254,10 +253,10 @@ __global__ void __launch_bounds__(32, 16) k_force(ForceArgs A)
         if (valid) red_add_v4(&A.f4[ce.x * 8 + k], -(fjx.x + fjx.y), -(fjy.x + fjy.y), -(fjz.x + fjz.y));
     }
 
-    // Cluster pairs without a mask, at half-cluster granularity: always full steps of 8 half-clusters.  ptxas schedules memory
-    // operations whose consumer is an iteration away at the END of the step, so the j data of
-    // step s+1 is loaded there; to make that load an L1 hit the lines are prefetched one step
-    // earlier still (distance 2), and the list entries are read 3 steps ahead (indices clamped).
+    // Cluster pairs without a mask, at half-cluster granularity: always full steps of 8 half-clusters.
+    // ptxas schedules memory operations whose consumer is an iteration away at the END of a step,
+    // so the j data is requested TWO steps ahead into registers (xj: this step, xj1: next step, x2:
+    // the one after) and the list entries four steps ahead, indices clamped to the segment.
     int cj2 = 0, cj3 = 0;
     float4 xj1 = xj;
     int tj1 = tj;
