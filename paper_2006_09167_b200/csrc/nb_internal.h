@@ -150,8 +150,9 @@ struct nb_ctx {
     DevBuf<int32_t> il;                        // cj of cluster pairs without a mask for this i-cluster
     DevBuf<int2> ilm;                          // {cj, mask ref} of cluster pairs with a mask, plus each segment's tail
     // compact OUTER list (a3 -> a6): what the prune kernel streams; written once per search
-    DevBuf<int2> ol;                           // {cj, unit-local joint slot | masked << 30}; segment at il offset + ilm offset
-    DevBuf<int32_t> ol_cnt;                    // [nunits*8] entries per segment (index: unit launch position*8 + i-cluster)
+    DevBuf<int2> ol;                           // {cj, unit-local joint slot}; segment at il offset + ilm offset: the cluster pairs
+                                               // without a mask, then (from a multiple of 4 on) those with a mask
+    DevBuf<int2> ol_cnt;                       // [nunits*8] {unmasked, masked} entries per segment (index: unit launch position*8 + i-cluster)
     DevBuf<double> fshift;                     // [27*3] per-shift i-force sums (virial)
 
     // --- per-stage device timing (nb_timing_enable / nb_timing_read) ---

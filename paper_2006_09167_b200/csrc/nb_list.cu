@@ -337,7 +337,7 @@ __global__ void __launch_bounds__(256) k_ilist_build(const int4* __restrict__ un
                                                      const int* __restrict__ il_off, const int* __restrict__ ilm_off,
                                                      const int* __restrict__ seg_pos, int4* __restrict__ seg,
                                                      int2* __restrict__ seg_ci, int32_t* __restrict__ il,
-                                                     int2* __restrict__ ilm, int2* __restrict__ ol, int* __restrict__ ol_cnt,
+                                                     int2* __restrict__ ilm, int2* __restrict__ ol, int2* __restrict__ ol_cnt,
                                                      int cj_dummy)
 {
     const int4 u = units[blockIdx.x];   // units in launch order
@@ -349,18 +349,28 @@ __global__ void __launch_bounds__(256) k_ilist_build(const int4* __restrict__ un
         seg[s].y = om;
         seg_ci[s] = make_int2(u.w * 8 + warp, nb_half_shift_id(u.x - u.w * NB_NHALF));
     }
-    {   // compact outer list of this i-cluster: what the prune kernel streams
+    {   // compact outer list of this i-cluster, what the prune kernel streams: the cluster pairs
+        // without a mask first, then (from a multiple of 4 on) those with a mask
         int2* ols = ol + o + om;
         const unsigned lt = (1u << lane) - 1u;
-        int n = 0;
+        int nuo = 0, nmo = 0;
         for (int b = u.y; b < u.z; b++) {
             const unsigned bits = plane[(size_t)b * 8 + warp], eb = plane_excl[(size_t)b * 8 + warp] & bits;
-            if ((bits >> lane) & 1u)
-                ols[n + __popc(bits & lt)] =
-                    make_int2(jl[(size_t)b * 32 + lane].x, ((b - u.y) * 32 + lane) | (int)(((eb >> lane) & 1u) << 30));
-            n += __popc(bits);
+            nuo += __popc(bits & ~eb);
         }
-        if (lane == 0) ol_cnt[s0] = n;
+        const int mbase = (nuo + 3) & ~3;
+        nuo = 0;
+        for (int b = u.y; b < u.z; b++) {
+            const unsigned bits = plane[(size_t)b * 8 + warp], eb = plane_excl[(size_t)b * 8 + warp] & bits, nb = bits & ~eb;
+            if ((bits >> lane) & 1u) {
+                const int2 e = make_int2(jl[(size_t)b * 32 + lane].x, (b - u.y) * 32 + lane);
+                if ((nb >> lane) & 1u) ols[nuo + __popc(nb & lt)] = e;
+                else ols[mbase + nmo + __popc(eb & lt)] = e;
+            }
+            nuo += __popc(nb);
+            nmo += __popc(eb);
+        }
+        if (lane == 0) ol_cnt[s0] = make_int2(nuo, nmo);
     }
     nb_ilist_write([&](int b) { return plane[(size_t)(u.y + b) * 8 + warp]; }, u.y, u.z, warp, lane, cj_dummy, plane_excl, jl,
                    il + o, ilm + om, reinterpret_cast<int2*>(&seg[s]) + 1);

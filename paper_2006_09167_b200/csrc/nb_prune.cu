@@ -26,7 +26,7 @@ struct PruneArgs {
     const int2* jl;
     const uint32_t* plane_outer;
     const int2* ol;           // compact outer list (nb_list.cu k_ilist_build)
-    const int* ol_cnt;
+    const int2* ol_cnt;
     uint32_t* plane_inner;
     const float4* xq;
     float box[3];
@@ -70,28 +70,41 @@ struct PruneState {
     int nu, nm;
 };
 
-template <bool DIAG>
-__device__ __forceinline__ void prune_step(const PruneArgs& A, const float2 (&xi)[4], const float2 (&yi)[4],
-                                           const float2 (&zi)[4], const int2 e, const float4 x, const bool valid, const int ci,
-                                           const int b0, const int lane, unsigned* res, int32_t* il, int2* ilm,
-                                           PruneState& st)
+// One step over 4 cluster pairs WITHOUT a mask: a half j-cluster (4 atoms) survives iff one of its
+// atoms is within rlist_inner of an i atom; the survivors' half-cluster indices are appended to il.
+__device__ __forceinline__ void prune_step_unmasked(const PruneArgs& A, const float2 (&xi)[4], const float2 (&yi)[4],
+                                                    const float2 (&zi)[4], const int2 e, const float4 x, const bool valid,
+                                                    const int lane, unsigned* res, int32_t* il, PruneState& st)
+{
+    const bool found = prune_checks<false>(xi, yi, zi, x, A.rl2, false, 0);
+    const unsigned gm = __ballot_sync(0xffffffffu, found && valid);
+    unsigned hm = gm | (gm >> 1);
+    hm = (hm | (hm >> 2)) & 0x11111111u;          // bit 4h: half h of the step (lanes 4h..4h+3) has a survivor
+    if ((hm >> lane) & 1u) {                      // its leader lane (lane % 4 == 0)
+        il[st.nu + __popc(hm & ((1u << lane) - 1u))] = 2 * e.x + ((lane >> 2) & 1);
+        if ((lane & 4) == 0 || !((hm >> (lane - 4)) & 1u)) atomicOr(&res[e.y >> 5], 1u << (e.y & 31));   // once per cluster
+    }
+    st.nu += __popc(hm);
+}
+
+// One step over 4 cluster pairs WITH a mask (exclusions, or the zero-shift diagonal pair, which keeps
+// only atom pairs b > a): whole clusters, appended to ilm with their mask reference.
+__device__ __forceinline__ void prune_step_masked(const PruneArgs& A, const float2 (&xi)[4], const float2 (&yi)[4],
+                                                  const float2 (&zi)[4], const int2 e, const float4 x, const bool valid,
+                                                  const bool diag, const int b0, const int lane, unsigned* res, int2* ilm,
+                                                  PruneState& st)
 {
     const int g = lane >> 3, k = lane & 7;
-    const int cj = e.x, slot = e.y & 0x3fffffff;
-    const bool found = prune_checks<DIAG>(xi, yi, zi, x, A.rl2, DIAG && cj == ci, k);
+    const bool found = prune_checks<true>(xi, yi, zi, x, A.rl2, diag, k);
     const unsigned gm = __ballot_sync(0xffffffffu, found && valid);
-    const bool masked = (e.y >> 30) & 1;
-    const bool keep = k == 0 && ((gm >> (8 * g)) & 0xffu) != 0u;              // leader of a surviving cluster pair
-    const bool keep_half = (lane & 3) == 0 && ((gm >> lane) & 0xfu) != 0u;    // leader of a surviving half (4 atoms)
-    const unsigned bu = __ballot_sync(0xffffffffu, keep_half && !masked), bm = __ballot_sync(0xffffffffu, keep && masked);
-    const unsigned lt = (1u << lane) - 1u;
-    if (keep_half && !masked) il[st.nu + __popc(bu & lt)] = 2 * cj + ((lane >> 2) & 1);
-    if (keep) {
-        atomicOr(&res[slot >> 5], 1u << (slot & 31));
-        if (masked) ilm[st.nm + __popc(bm & lt)] = make_int2(cj, A.jl[(size_t)b0 * 32 + slot].y);
+    unsigned cm = gm | (gm >> 1);
+    cm |= cm >> 2;
+    cm = (cm | (cm >> 4)) & 0x01010101u;          // bit 8g: cluster pair g of the step survives
+    if ((cm >> lane) & 1u) {
+        atomicOr(&res[e.y >> 5], 1u << (e.y & 31));
+        ilm[st.nm + __popc(cm & ((1u << lane) - 1u))] = make_int2(e.x, A.jl[(size_t)b0 * 32 + e.y].y);
     }
-    st.nu += __popc(bu);
-    st.nm += __popc(bm);
+    st.nm += __popc(cm);
 }
 
 // One warp per block = one i-cluster of one work unit: streams its compact outer list segment.
@@ -106,17 +119,17 @@ __global__ void __launch_bounds__(32) k_prune(PruneArgs A)
     const int s0 = A.unit_pos[ucan] * 8 + warp;
     int4* sg = &A.seg[A.seg_pos[s0]];
     const int2 off = *reinterpret_cast<const int2*>(sg);
-    const int n = A.ol_cnt[s0];
+    const int2 n = A.ol_cnt[s0];            // {cluster pairs without a mask, with a mask}
     const int2* __restrict__ ol = A.ol + off.x + off.y;
     int32_t* il = A.il + off.x;
     int2* ilm = A.ilm + off.y;
-    const int ns = (n + 3) >> 2;
+    const int ns = (n.x + 3) >> 2;
     int2 ea = make_int2(ci, 0), eb = ea, ea2 = ea, eb2 = ea;
     if (ns > 0) {
-        ea = ol[min(g, n - 1)];
-        eb = ol[min(4 + g, n - 1)];
-        ea2 = ol[min(8 + g, n - 1)];
-        eb2 = ol[min(12 + g, n - 1)];
+        ea = ol[min(g, n.x - 1)];
+        eb = ol[min(4 + g, n.x - 1)];
+        ea2 = ol[min(8 + g, n.x - 1)];
+        eb2 = ol[min(12 + g, n.x - 1)];
     }
     int sx, sy, sz;
     nb_shift_vec(nb_half_shift_id(h), sx, sy, sz);
@@ -133,38 +146,30 @@ __global__ void __launch_bounds__(32) k_prune(PruneArgs A)
     if (lane < NB_MAX_UNIT_BATCHES) res[lane] = 0u;
     __syncwarp();
     PruneState st = {0, 0};
+    // cluster pairs with a mask: few (about one step per zero-shift segment), no pipeline
+    const int mbase = (n.x + 3) & ~3;
+    for (int s = 0; s < n.y; s += 4) {
+        const bool valid = s + g < n.y;
+        const int2 e = ol[mbase + min(s + g, n.y - 1)];
+        const float4 x = A.xq[e.x * 8 + k];
+        prune_step_masked(A, xi, yi, zi, e, x, valid, e.x == ci && h == 0, u.y, lane, res, ilm, st);
+    }
     if (ns > 0) {
         // two alternating register sets (a: even steps, b: odd steps); j coordinates two steps ahead,
         // list entries four steps ahead, indices clamped to the segment (as in the force kernel)
         float4 xa = A.xq[ea.x * 8 + k], xb = A.xq[eb.x * 8 + k];
         int s = 0;
-        // The joint list of a zero-shift element holds cj >= ci in ascending order, so the diagonal
-        // cluster pair (cj == ci), if listed, is in the first step of the segment: only that step
-        // needs the b > a predicate.
-        if (h == 0) {
-            prune_step<true>(A, xi, yi, zi, ea, xa, g < n, ci, u.y, lane, res, il, ilm, st);
-            ea = ea2;
-            xa = A.xq[ea.x * 8 + k];
-            ea2 = ol[min(4 * 4 + g, n - 1)];
-            if (ns > 1) {
-                prune_step<false>(A, xi, yi, zi, eb, xb, 4 + g < n, ci, u.y, lane, res, il, ilm, st);
-                eb = eb2;
-                xb = A.xq[eb.x * 8 + k];
-                eb2 = ol[min(4 * 5 + g, n - 1)];
-            }
-            s = 2;
-        }
         for (; s + 1 < ns; s += 2) {
-            prune_step<false>(A, xi, yi, zi, ea, xa, 4 * s + g < n, ci, u.y, lane, res, il, ilm, st);
+            prune_step_unmasked(A, xi, yi, zi, ea, xa, 4 * s + g < n.x, lane, res, il, st);
             ea = ea2;
             xa = A.xq[ea.x * 8 + k];
-            ea2 = ol[min(4 * (s + 4) + g, n - 1)];
-            prune_step<false>(A, xi, yi, zi, eb, xb, 4 * (s + 1) + g < n, ci, u.y, lane, res, il, ilm, st);
+            ea2 = ol[min(4 * (s + 4) + g, n.x - 1)];
+            prune_step_unmasked(A, xi, yi, zi, eb, xb, 4 * (s + 1) + g < n.x, lane, res, il, st);
             eb = eb2;
             xb = A.xq[eb.x * 8 + k];
-            eb2 = ol[min(4 * (s + 5) + g, n - 1)];
+            eb2 = ol[min(4 * (s + 5) + g, n.x - 1)];
         }
-        if (s < ns) prune_step<false>(A, xi, yi, zi, ea, xa, 4 * s + g < n, ci, u.y, lane, res, il, ilm, st);
+        if (s < ns) prune_step_unmasked(A, xi, yi, zi, ea, xa, 4 * s + g < n.x, lane, res, il, st);
     }
     __syncwarp();
     nb_ilist_finish(st.nu, st.nm, u.y * 8 + warp, lane, A.cj_dummy, il, ilm, reinterpret_cast<int2*>(sg) + 1);
