@@ -374,6 +374,24 @@ __global__ void __launch_bounds__(256) k_gather(int nslots, float4* __restrict__
     }
 }
 
+// Force-only gather, 4 consecutive slots per thread (nslots is a multiple of 64): the loads of a
+// thread are independent and issued together, which matters more than bytes at these sizes.
+__global__ void __launch_bounds__(256) k_gather4(int nquads, float4* __restrict__ f4, const int4* __restrict__ atom_of_slot4,
+                                                 float* __restrict__ f)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nquads) return;
+    const int4 a = atom_of_slot4[t];
+    float4* p = f4 + 4 * (size_t)t;
+    const float4 v0 = p[0], v1 = p[1], v2 = p[2], v3 = p[3];
+    const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+    p[0] = z; p[1] = z; p[2] = z; p[3] = z;
+    if (a.x >= 0) { f[3 * a.x] = v0.x; f[3 * a.x + 1] = v0.y; f[3 * a.x + 2] = v0.z; }
+    if (a.y >= 0) { f[3 * a.y] = v1.x; f[3 * a.y + 1] = v1.y; f[3 * a.y + 2] = v1.z; }
+    if (a.z >= 0) { f[3 * a.z] = v2.x; f[3 * a.z + 1] = v2.y; f[3 * a.z + 2] = v2.z; }
+    if (a.w >= 0) { f[3 * a.w] = v3.x; f[3 * a.w + 1] = v3.y; f[3 * a.w + 2] = v3.z; }
+}
+
 // Xi = -1/2 ( sum_i x_i (x) f_i + sum_s (s L) (x) S_s )   (reading A8)
 __global__ void k_virial_final(const double* __restrict__ xf, const double* __restrict__ fshift, float3 box,
                                double* __restrict__ virial)
@@ -544,7 +562,8 @@ int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial)
     if (virial)
         k_gather<true><<<nb, 256, 0, st>>>(c->nslots, c->f4.p, c->atom_of_slot.p, c->xq.p, f, xf);
     else
-        k_gather<false><<<nb, 256, 0, st>>>(c->nslots, c->f4.p, c->atom_of_slot.p, c->xq.p, f, xf);
+        k_gather4<<<(c->nslots / 4 + 255) / 256, 256, 0, st>>>(c->nslots / 4, c->f4.p,
+                                                              reinterpret_cast<const int4*>(c->atom_of_slot.p), f);
     NB_LAUNCH_CHECK(c);
     if (virial) {
         k_virial_final<<<1, 32, 0, st>>>(xf, c->fshift.p, make_float3(c->box[0], c->box[1], c->box[2]), virial);
