@@ -379,7 +379,9 @@ int nbi_grid(nb_ctx* c)
                                              c->sbb_lo.p, c->sbb_hi.p, make_float3(pb[0], pb[1], pb[2]),
                                              make_float3(pd[0], pd[1], pd[2]));
     NB_LAUNCH_CHECK(c);
-    {
+    if (c->dummy_at != (const void*)(c->xq.p + c->nslots) || c->dummy_box[0] != L[0] || c->dummy_box[1] != L[1] ||
+        c->dummy_box[2] != L[2]) {
+        // (rewritten only when the box or their place in the arrays has changed)
         // Dummy j-clusters (index nclusters .. nclusters + NB_NDUMMY - 1): padding-like atoms beyond the
         // padding lattice that interact with nothing.  The prune kernel may fill an inner list
         // segment up to a multiple of 8 half-clusters with them; the (zero) forces the force kernel adds to their
@@ -391,6 +393,8 @@ int nbi_grid(nb_ctx* c)
         NB_CUDA(c, cudaMemcpyAsync(c->xq.p + c->nslots, hx.data(), sizeof(float4) * hx.size(), cudaMemcpyHostToDevice, st));
         NB_CUDA(c, cudaMemcpyAsync(c->type_slot.p + c->nslots, ht.data(), sizeof(int32_t) * ht.size(), cudaMemcpyHostToDevice, st));
         NB_CUDA(c, cudaStreamSynchronize(st));
+        c->dummy_at = c->xq.p + c->nslots;
+        for (int k = 0; k < 3; k++) c->dummy_box[k] = L[k];
     }
     c->grid_box[0] = L[0];
     c->grid_box[1] = L[1];

@@ -132,10 +132,12 @@ struct nb_ctx {
     DevBuf<int32_t> unit_order;                // canonical unit index, longest first (force kernel launch order)
     // prune launch order: (canonical unit*8 + i-cluster), each rolling part longest list first; one
     // cached table per recently used nparts, rebuilt lazily after a search
-    struct PruneOrder { int nparts = 0; int64_t search = -1; DevBuf<int32_t> d; };
+    struct PruneOrder { int nparts = 0; int64_t search = -1; DevBuf<int32_t> d; std::vector<int32_t> h; };
     PruneOrder prune_orders[4];
     int prune_order_next = 0;
-    std::vector<int32_t> h_prune_order, h_unit_order, h_seg_sorted;   // host scratch / copies made at search time
+    std::vector<int32_t> h_unit_order, h_seg_sorted, h_seg_pos;   // host copies made at search time (sources of async uploads)
+    float dummy_box[3] = {0, 0, 0};            // box the dummy clusters were last written for
+    const void* dummy_at = nullptr;            // ... and where
     int nunits = 0;
 
     // --- compact inner list (a6 -> a7): per (work unit, i-cluster) the j-clusters whose inner mask bit is set ---

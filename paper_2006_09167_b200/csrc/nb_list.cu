@@ -677,7 +677,9 @@ int nbi_search(nb_ctx* c, float rlist)
             const int* cm = cu + nseg;
             int maxlen = 0;
             for (int i = 0; i < nseg; i++) maxlen = std::max(maxlen, cu[i] + 2 * cm[i]);
-            std::vector<int32_t> start(maxlen + 2, 0), pos(nseg);
+            std::vector<int32_t> start(maxlen + 2, 0);
+            std::vector<int32_t>& pos = c->h_seg_pos;   // member: source of an async upload
+            pos.resize(nseg);
             for (int i = 0; i < nseg; i++) start[maxlen - (cu[i] + 2 * cm[i]) + 1]++;
             for (int l = 0; l <= maxlen; l++) start[l + 1] += start[l];
             c->nseg_launch = start[maxlen];   // everything before the length-0 bucket
@@ -687,7 +689,6 @@ int nbi_search(nb_ctx* c, float rlist)
             NB_CUDA(c, c->seg_pos.ensure(nseg, st));
             NB_CUDA(c, c->seg_ci.ensure(nseg, st));
             NB_CUDA(c, cudaMemcpyAsync(c->seg_pos.p, pos.data(), sizeof(int) * nseg, cudaMemcpyHostToDevice, st));
-            NB_CUDA(c, cudaStreamSynchronize(st));
         }
         NB_CUDA(c, c->il.ensure((size_t)tot[0] + 4, st));
         NB_CUDA(c, c->ilm.ensure((size_t)tot[1] + 4, st));

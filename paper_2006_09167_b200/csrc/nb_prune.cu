@@ -200,14 +200,13 @@ int nbi_prune(nb_ctx* c, float rlist_inner, int part, int nparts)
             fill[p] = (int)(a * 8);
             for (long long i = a; i < b; i++) part_of[i] = p;
         }
-        c->h_prune_order.resize(nu * 8);
+        po->h.resize(nu * 8);
         for (long long t = 0; t < nu * 8; t++) {
             const int s0 = c->h_seg_sorted[t], ucan = c->h_unit_order[s0 >> 3];
-            c->h_prune_order[fill[part_of[ucan]]++] = ucan * 8 + (s0 & 7);
+            po->h[fill[part_of[ucan]]++] = ucan * 8 + (s0 & 7);
         }
         NB_CUDA(c, po->d.ensure(nu * 8, c->stream));
-        NB_CUDA(c, cudaMemcpyAsync(po->d.p, c->h_prune_order.data(), sizeof(int) * nu * 8, cudaMemcpyHostToDevice, c->stream));
-        NB_CUDA(c, cudaStreamSynchronize(c->stream));   // h_prune_order is reused
+        NB_CUDA(c, cudaMemcpyAsync(po->d.p, po->h.data(), sizeof(int) * nu * 8, cudaMemcpyHostToDevice, c->stream));
         po->nparts = nparts;
         po->search = c->st.search_count;
     }
