@@ -33,9 +33,9 @@ METRIC = "effective non-bonded pair interactions/s (cluster-pair step: put_atoms
 UNIT = "pairs/s"
 # FP32 work of the force kernel per atom-pair slot: what the unmasked F-only
 # step executes, counted in its SASS -- packed FFMA2 = 4 flop, FMUL2/FADD2 = 2, FFMA = 2,
-# FADD/FMUL/MUFU = 1 -- divided by the 256 slots of a warp step.  (SURVEY 8.4's estimate of the
+# FADD/FMUL/MUFU/compare/select = 1 -- divided by the 256 slots of a warp step.  (SURVEY 8.4's estimate of the
 # method's work was 62 / 40; the smaller executed count is the one used.)
-FLOP_PER_SLOT = {"ewald": 55.75, "rf": 36.75, "none": 31.75}
+FLOP_PER_SLOT = {"ewald": 54.75, "rf": 35.75, "none": 30.75}
 # DRAM bytes of one force-kernel launch from the committed ncu --set full capture (profiles/r1c_force_full_cfg2.md);
 # the kernel is ALU-bound, its HBM traffic is ~0.2 % of what the HBM roofline would allow in the same time.
 NCU_DRAM_BYTES_PER_LAUNCH = {(2, "ewald"): 14.8e6}

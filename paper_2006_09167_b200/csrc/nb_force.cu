@@ -54,12 +54,6 @@ __device__ __forceinline__ float rsqrt_fast(float x)
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
-__device__ __forceinline__ float fma_sat(float a, float b, float c)
-{
-    float y;
-    asm("fma.rn.sat.f32 %0, %1, %2, %3;" : "=f"(y) : "f"(a), "f"(b), "f"(c));
-    return y;
-}
 __device__ __forceinline__ float rcp_fast(float x)
 {
     float y;
@@ -118,18 +112,19 @@ __device__ __forceinline__ void pair_step(const NbConst& K, const float4* __rest
     for (int p = 0; p < 4; p++) {
         const float2 dx = add2(I.x[p], nxj), dy = add2(I.y[p], nyj), dz = add2(I.z[p], nzj);
         const float2 r2u = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
-        // A7: interact iff r^2 < rc^2 (strict).  MASKED steps select with predicates and clamp r^2 so
-        // that self pairs stay finite; unmasked steps have no r = 0 pairs (padding atoms sit at
-        // distinct finite positions, nb_grid.cu) and multiply by w = sat((rc^2 - r^2) 2^60), which
-        // is exactly 1 or 0 and costs FP32-pipe slots instead of the half-rate ALU pipe.
+        // A7: interact iff r^2 < rc^2 (strict), applied with compare + select on the ALU pipe, which
+        // has slack (the FP32 pipe is the bound; a saturating-FMA 0/1 factor there was measured 1 %
+        // slower).  MASKED steps also clamp r^2 so that self pairs stay finite; unmasked steps have no
+        // r = 0 pairs (padding atoms sit at distinct finite positions, nb_grid.cu).
         bool w0 = true, w1 = true;
-        float2 r2 = r2u, wc = f2(1.f);
+        float2 r2 = r2u;
         if (MASKED) {
             w0 = r2u.x < K.rc2 && ((cbyte >> (2 * p)) & 1u);
             w1 = r2u.y < K.rc2 && ((cbyte >> (2 * p + 1)) & 1u);
             r2 = f2(fmaxf(r2u.x, 1e-6f), fmaxf(r2u.y, 1e-6f));
         } else {
-            wc = f2(fma_sat(r2u.x, -K.cut_big, K.cut_rc2big), fma_sat(r2u.y, -K.cut_big, K.cut_rc2big));
+            w0 = r2u.x < K.rc2;
+            w1 = r2u.y < K.rc2;
         }
         const float2 rinv = f2(rsqrt_fast(r2.x), rsqrt_fast(r2.y));
         const float2 rinv2 = mul2(rinv, rinv);
@@ -153,8 +148,7 @@ __device__ __forceinline__ void pair_step(const NbConst& K, const float4* __rest
         } else {
             fs = mul2(rinv2, t1);                             // LJ only: charges are ignored
         }
-        if (MASKED) fs = f2(w0 ? fs.x : 0.f, w1 ? fs.y : 0.f);
-        else fs = mul2(fs, wc);
+        fs = f2(w0 ? fs.x : 0.f, w1 ? fs.y : 0.f);
         fix[p] = fma2(fs, dx, fix[p]);
         fiy[p] = fma2(fs, dy, fiy[p]);
         fiz[p] = fma2(fs, dz, fiz[p]);
@@ -176,8 +170,7 @@ __device__ __forceinline__ void pair_step(const NbConst& K, const float4* __rest
             } else {
                 vc = f2(0.f);
             }
-            const float2 vl = mul2(mul2(mf, vlj), wc);
-            vc = mul2(vc, wc);
+            const float2 vl = mul2(mf, vlj);
             elj += (w0 ? vl.x : 0.f) + (w1 ? vl.y : 0.f);
             ecoul += (w0 ? vc.x : 0.f) + (w1 ? vc.y : 0.f);
         }
@@ -534,8 +527,6 @@ int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial)
             if (k < 5) A.kc.ewp2[k] = make_float2((float)(b * b2 * bk * P[k] / qlead), (float)(b * b2 * bk * P[k] / qlead));
             A.kc.ewq2[k] = make_float2((float)(bk * Q[k] / qlead), (float)(bk * Q[k] / qlead));
         }
-        A.kc.cut_big = 1.152921504606846976e18f;              // 2^60: products with it are exact
-        A.kc.cut_rc2big = A.kc.rc2 * 1.152921504606846976e18f;
     }
     NB_CUDA(c, c->fshift.ensure(NB_NSHIFT * 3 + 9, st));
     A.fshift = c->fshift.p;

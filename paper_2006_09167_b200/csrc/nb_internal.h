@@ -65,7 +65,6 @@ struct NbConst {
     // Ewald correction fit as polynomials in r^2 (beta folded in), every coefficient duplicated
     // for the packed FFMA2 form: ewp2[k] = beta^(3+2k) P_k, ewq2[k] = beta^(2k) Q_k.
     float2 ewp2[5], ewq2[6];
-    float cut_big, cut_rc2big;   // 2^60 and rc^2 2^60: w = sat(rc2big - r2 big) is 1 inside the cut-off, else 0
 };
 
 struct nb_ctx {
