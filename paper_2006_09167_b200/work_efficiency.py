@@ -11,7 +11,7 @@ list) / (64 x listed cluster pairs).  Two cluster numbers are printed: the searc
 predicate, what the paper's CPU search produces) and the list after a prune at the same rlist (atom
 distances, the dual-list inner list).  The 1x1 reference is the ideal-gas ratio (rc / rlist)^3.
 The tolerance-based Verlet-buffer estimate of L159-L161 needs masses, temperature and constraints,
-which this path does not have: not built (DESIGN.md section 10).
+which this path does not have: not built (DESIGN.md section 11).
 """
 from __future__ import annotations
 
