@@ -137,6 +137,13 @@ int nb_list_count(nb_ctx*, int which, int64_t* n);
  * part: rolling part of the entry under the nparts of the last nb_prune (0 before any prune). */
 int nb_list_dump(nb_ctx*, int which, int32_t* ci, int32_t* cj, int32_t* shift, uint64_t* pairmask,
                  int32_t* part);
+/* Dumps the COMPACT inner list the force kernel streams (for parity tests; slow, synchronises).
+ * HOST arrays of *n entries, any may be NULL; call with all NULL to get *n.  Entry k: i-cluster ci[k],
+ * shift[k] (as in nb_list_dump), kind[k] = 0: entry[k] is a half j-cluster index 2*cj + half (atoms
+ * 4*entry .. 4*entry+3, a cluster pair without a mask, kept at half-cluster granularity);
+ * kind[k] = 1: entry[k] is a whole j-cluster cj whose pair with ci carries a mask.  Padding (dummy)
+ * entries are left out. */
+int nb_inner_dump(nb_ctx*, int64_t* n, int32_t* ci, int32_t* entry, int32_t* shift, int32_t* kind);
 int nb_get_stats(nb_ctx*, nb_stats* out);
 /* Measures the device's FP32 FMA issue peak with a register-resident FFMA chain kernel
  * (MEASURED_PEAKS.json has no FP32 entry).  Returns lane-FMA/s in *fma_per_s. */

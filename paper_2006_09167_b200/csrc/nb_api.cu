@@ -292,6 +292,13 @@ extern "C" int nb_count_slots(nb_ctx* c, int64_t* slots)
     return nbi_count_slots(c, slots);
 }
 
+extern "C" int nb_inner_dump(nb_ctx* c, int64_t* n, int32_t* ci, int32_t* entry, int32_t* shift, int32_t* kind)
+{
+    if (!c || !n) return NB_ERR_ARG;
+    if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "no list yet (call nb_search)");
+    return nbi_inner_dump(c, n, ci, entry, shift, kind);
+}
+
 extern "C" int nb_timing_enable(nb_ctx* c, int on)
 {
     if (!c) return NB_ERR_ARG;

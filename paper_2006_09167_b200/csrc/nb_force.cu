@@ -18,6 +18,8 @@
 // across lanes once per segment.
 #include "nb_internal.h"
 
+#include <algorithm>
+
 #include "ewald_corr_coeffs.h"
 
 namespace {
@@ -605,6 +607,43 @@ int nbi_count_slots(nb_ctx* c, int64_t* slots)
     NB_CUDA(c, cudaMemcpyAsync(&v, c->counters.p, sizeof(v), cudaMemcpyDeviceToHost, st));
     NB_CUDA(c, cudaStreamSynchronize(st));
     *slots = v;
+    return NB_OK;
+}
+
+int nbi_inner_dump(nb_ctx* c, int64_t* n, int32_t* ci, int32_t* entry, int32_t* shift, int32_t* kind)
+{
+    cudaStream_t st = c->stream;
+    const int ns = c->nseg_launch;
+    std::vector<int4> seg(std::max(ns, 1));
+    std::vector<int2> sci(std::max(ns, 1)), ilm(c->ilm_total + 1);
+    std::vector<int32_t> il(c->il_total + 1);
+    if (ns > 0) {
+        NB_CUDA(c, cudaMemcpyAsync(seg.data(), c->seg.p, sizeof(int4) * ns, cudaMemcpyDeviceToHost, st));
+        NB_CUDA(c, cudaMemcpyAsync(sci.data(), c->seg_ci.p, sizeof(int2) * ns, cudaMemcpyDeviceToHost, st));
+        if (c->il_total) NB_CUDA(c, cudaMemcpyAsync(il.data(), c->il.p, sizeof(int32_t) * c->il_total, cudaMemcpyDeviceToHost, st));
+        if (c->ilm_total) NB_CUDA(c, cudaMemcpyAsync(ilm.data(), c->ilm.p, sizeof(int2) * c->ilm_total, cudaMemcpyDeviceToHost, st));
+    }
+    NB_CUDA(c, cudaStreamSynchronize(st));
+    int64_t k = 0;
+    for (int s = 0; s < ns; s++) {
+        for (int e = 0; e < seg[s].z; e++) {
+            const int hc = il[seg[s].x + e];
+            if (hc >= 2 * c->nclusters) continue;   // dummy padding
+            if (ci) ci[k] = sci[s].x;
+            if (entry) entry[k] = hc;
+            if (shift) shift[k] = sci[s].y;
+            if (kind) kind[k] = 0;
+            k++;
+        }
+        for (int e = 0; e < seg[s].w; e++) {
+            if (ci) ci[k] = sci[s].x;
+            if (entry) entry[k] = ilm[seg[s].y + e].x;
+            if (shift) shift[k] = sci[s].y;
+            if (kind) kind[k] = 1;
+            k++;
+        }
+    }
+    *n = k;
     return NB_OK;
 }
 

@@ -146,6 +146,7 @@ struct nb_ctx {
     DevBuf<int32_t> unit_pos;                  // canonical unit index -> launch position (inverse of unit_order)
     DevBuf<int32_t> seg_pos;                   // [nunits*8] (unit launch position*8 + i-cluster) -> index into seg (longest first)
     DevBuf<int2> seg_ci;                       // [nunits*8] {i-cluster, shift id} of each seg entry
+    size_t il_total = 0, ilm_total = 0;        // allocated extents of il / ilm in use (sum of segment capacities)
     int nseg_launch = 0;                       // seg entries with a non-empty outer list (= force kernel grid)
     std::vector<int32_t> h_caps;               // host scratch
     DevBuf<int32_t> il;                        // cj of cluster pairs without a mask for this i-cluster
@@ -290,4 +291,5 @@ int nbi_list_dump(nb_ctx* c, int which, int32_t* ci, int32_t* cj, int32_t* shift
 int nbi_measure_fp32_peak(nb_ctx* c, double* fma_per_s);   // nb_force.cu
 int nbi_count_pairs(nb_ctx* c, int64_t* n_interacting, int64_t* n_excluded);   // nb_force.cu
 int nbi_count_slots(nb_ctx* c, int64_t* slots);            // nb_force.cu
+int nbi_inner_dump(nb_ctx* c, int64_t* n, int32_t* ci, int32_t* entry, int32_t* shift, int32_t* kind);   // nb_force.cu
 int nbi_exclusive_scan(nb_ctx* c, const int32_t* in, int32_t* out, int64_t n, int32_t* total_dev);  // nb_list.cu

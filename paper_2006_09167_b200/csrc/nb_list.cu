@@ -690,6 +690,8 @@ int nbi_search(nb_ctx* c, float rlist)
             NB_CUDA(c, c->seg_ci.ensure(nseg, st));
             NB_CUDA(c, cudaMemcpyAsync(c->seg_pos.p, pos.data(), sizeof(int) * nseg, cudaMemcpyHostToDevice, st));
         }
+        c->il_total = (size_t)tot[0];
+        c->ilm_total = (size_t)tot[1];
         NB_CUDA(c, c->il.ensure((size_t)tot[0] + 4, st));
         NB_CUDA(c, c->ilm.ensure((size_t)tot[1] + 4, st));
         NB_CUDA(c, c->ol.ensure((size_t)tot[0] + (size_t)tot[1] + 4, st));

@@ -24,7 +24,7 @@ NB_SHIFT_CENTER = 13
 EXPORTS = ["nb_init", "nb_put_atoms", "nb_put_atoms_host", "nb_search", "nb_prune", "nb_forces",
            "nb_forces_host", "nb_free", "nb_last_error", "nb_get_layout", "nb_get_slots", "nb_list_count",
            "nb_list_dump", "nb_get_stats", "nb_measure_fp32_peak", "nb_count_pairs", "nb_timing_enable",
-           "nb_timing_read", "nb_timing_stages", "nb_count_slots"]
+           "nb_timing_read", "nb_timing_stages", "nb_count_slots", "nb_inner_dump"]
 NB_T_NAMES = ["put", "grid", "search", "masks", "prune", "force", "reduce"]
 
 
@@ -196,6 +196,16 @@ class Context:
         n = C.c_int64()
         self._check(lib().nb_count_slots(self._h, C.byref(n)))
         return n.value
+
+    def inner_dump(self):
+        """The compact inner list the force kernel streams: numpy arrays ci, entry, shift id, kind
+        (0: entry = half j-cluster index 2*cj + half; 1: entry = whole j-cluster with a mask)."""
+        n = C.c_int64()
+        null = C.c_void_p(0)
+        self._check(lib().nb_inner_dump(self._h, C.byref(n), null, null, null, null))
+        arr = [np.zeros(max(n.value, 1), dtype=np.int32) for _ in range(4)]
+        self._check(lib().nb_inner_dump(self._h, C.byref(n), *[_hptr(a) for a in arr]))
+        return tuple(a[: n.value] for a in arr)
 
     def timing_enable(self, on=True):
         self._check(lib().nb_timing_enable(self._h, C.c_int(int(on))))

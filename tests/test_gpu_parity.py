@@ -319,6 +319,59 @@ def test_full_size_configs_in_bench_schedule(which):
         assert rel_rms(d.forces(), r.f) <= TOL_F
 
 
+@pytest.mark.parametrize("which", ["cfg0", "rect_rf", "lj"])
+def test_half_cluster_inner_list(which):
+    """The compact inner list the force kernel streams is kept at half-j-cluster granularity (DESIGN.md
+    section 5).  Layout-independent check in fp64 on the library's own slot table, with a 1e-6 nm guard band
+    around rlist_inner (the kernel decides in fp32): COMPLETE -- every atom pair closer than rlist_inner
+    is covered by a listed half-cluster of the other atom's cluster or by a masked cluster pair -- and
+    MINIMAL -- every listed half has an atom within rlist_inner of the i-cluster; the cluster pairs it
+    spans are exactly the inner list of nb_list_dump."""
+    w = {"cfg0": W.config0, "lj": lambda: W.lj_fluid(12, rc=0.9),
+         "rect_rf": lambda: W.small_water(150, 2.0, seed=21, rc=0.8, rlist_outer=0.9, rlist_inner=0.84,
+                                          box_scale=(1.0, 1.1, 1.25), coulomb="rf")}[which]()
+    d = Driver(w)
+    d.put()
+    d.ctx.search(w.rlist_outer)
+    for x, part, nparts in ((None, 0, 1), (w.positions_at(40), 0, 2), (w.positions_at(40), 1, 2)):
+        d.put(x)
+        d.ctx.prune(w.rlist_inner, part, nparts)
+    aos, xq = d.slots()
+    box = np.asarray(w.box, dtype=np.float64)
+    ci, ent, sid, kind = d.ctx.inner_dump()
+    svec = d.nb.shift_vectors(sid).astype(np.int64)
+    half = kind == 0
+    skey = LC.shift_id(svec)
+    hkeys = set(zip(ci[half].tolist(), ent[half].tolist(), skey[half].tolist()))
+    mkeys = set(zip(ci[~half].tolist(), ent[~half].tolist(), skey[~half].tolist()))
+    assert len(hkeys) == int(half.sum()) and len(mkeys) == int((~half).sum())      # no duplicates
+    # complete
+    si, sj, sp, _ = LC.close_atom_pairs(aos, xq, box, w.rlist_inner - 1e-6)
+    ka, kb = LC.shift_id(sp), LC.shift_id(-sp)
+    missing = 0
+    for a, b, k1, k2 in zip(si.tolist(), sj.tolist(), ka.tolist(), kb.tolist()):
+        if ((a // 8, b // 4, k1) in hkeys or (b // 8, a // 4, k2) in hkeys or (a // 8, b // 8, k1) in mkeys
+                or (b // 8, a // 8, k2) in mkeys):
+            continue
+        missing += 1
+    assert missing == 0 and si.size > 1000
+    # minimal: every listed half has a real atom within rlist_inner (+ guard) of a real atom of ci
+    x = np.asarray(xq, dtype=np.float64).reshape(-1, 4)[:, :3]
+    real = np.asarray(aos) >= 0
+    hci, hent, hs = ci[half], ent[half], svec[half]
+    xi = x[hci[:, None] * 8 + np.arange(8)[None, :]] + (hs * box)[:, None, :]           # [n,8,3], shift on the i side
+    xj = x[hent[:, None] * 4 + np.arange(4)[None, :]]                                   # [n,4,3]
+    d2 = ((xi[:, :, None, :] - xj[:, None, :, :]) ** 2).sum(-1)
+    ok = real[hci[:, None] * 8 + np.arange(8)[None, :]][:, :, None] & real[hent[:, None] * 4 + np.arange(4)[None, :]][:, None, :]
+    dmin = np.sqrt(np.where(ok, d2, np.inf).min(axis=(1, 2)))
+    assert (dmin < w.rlist_inner + 1e-6).all()
+    # same cluster pairs as the bit-plane inner list
+    dci, dcj, dsv, _, _ = d.dump(1)
+    planes = set(zip(dci.tolist(), dcj.tolist(), LC.shift_id(dsv).tolist()))
+    spanned = {(a, e // 2, k) for a, e, k in hkeys} | mkeys
+    assert spanned == planes
+
+
 def test_work_efficiency_table_against_oracle():
     """SURVEY 8.1 (f3), Fig. 5 definition: the table's numerator is the oracle's count of atom pairs
     within rc (interacting + excluded), its denominator 64 x the listed cluster pairs; the efficiency falls
