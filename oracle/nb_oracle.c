@@ -44,6 +44,9 @@ typedef struct {
     double beta;         /* Ewald splitting parameter, 1/nm */
     double eps_rf;       /* <= 0 means infinity */
     double epsfac;       /* 1/(4 pi eps0), kJ mol^-1 nm e^-2 (A2: 138.935458) */
+    double rc_vdw;       /* twin cut-offs (PME load balancing scales only the electrostatics
+                            cut-off): LJ interacts iff r < rc_vdw <= rc, its potential shift is taken at rc_vdw;
+                            <= 0 means rc_vdw = rc (single cut-off, reading A19) */
 } oracle_params;
 
 #define TWO_OVER_SQRT_PI 1.1283791670955125738961589031215
@@ -79,7 +82,7 @@ static void rf_constants(const oracle_params* p, double* krf, double* crf)
 }
 
 /*
- * One pair at distance r < rc (S:8.3.1 table).  qq = q_i*q_j (without epsfac).
+ * One pair at distance r < rc (S:8.3.1 table; LJ only below rc_vdw).  qq = q_i*q_j (without epsfac).
  * Outputs: energies V_lj, V_c (kJ/mol) and RADIAL forces F_lj, F_c = -dV/dr
  * (positive = repulsive).  excluded != 0 selects the exclusion-correction rows
  * (A4: no LJ; Ewald: -A erf(beta r)/r without shift (A5); RF: A (k_rf r^2 - c_rf)).
@@ -89,12 +92,13 @@ void oracle_pair(const oracle_params* p, double r, double qq, double c6, double 
 {
     double A = p->epsfac * qq;
     double rc = p->rc;
+    double rcv = p->rc_vdw > 0.0 ? p->rc_vdw : rc;     /* LJ cut-off (twin cut-offs), strict like A7 */
     *V_lj = 0.0; *F_lj = 0.0;
-    if (!excluded) {
+    if (!excluded && r * r < rcv * rcv) {
         double r2 = r * r, r6 = r2 * r2 * r2, r12 = r6 * r6;
         *V_lj = c12 / r12 - c6 / r6;
         if (p->lj_shift) {
-            double rc6 = rc * rc * rc * rc * rc * rc;
+            double rc6 = rcv * rcv * rcv * rcv * rcv * rcv;
             *V_lj -= c12 / (rc6 * rc6) - c6 / rc6;
         }
         *F_lj = 12.0 * c12 / (r12 * r) - 6.0 * c6 / (r6 * r);
@@ -502,6 +506,95 @@ long long oracle_lists(int nclusters, int C, const int32_t* atom_of_slot, const 
                                 out_mask[k] = pair_mask(C, atom_of_slot, excl_off, excl_idx, ci, cj, s);
                             }
                             k++;
+                        }
+            }
+            if (!pass) cnt[ci + 1] = k;
+        }
+        if (!pass) {
+            for (int c = 0; c < nclusters; c++) cnt[c + 1] += cnt[c];
+            total = cnt[nclusters];
+        }
+    }
+    free(lo); free(hi); free(nv); free(cnt);
+    return total;
+}
+
+/*
+ * The inner list at HALF j-cluster granularity (DESIGN.md section 5 "compact inner list"; the
+ * paper's "splitting j-clusters" while pruning: the search's cluster pairs are "pruned
+ * into" narrower ones).  This is the list the force kernel streams, so it gets its own definition:
+ *
+ *   for every canonical triple (ci,cj,s) of S_outer (bb predicate, as in oracle_lists):
+ *     - if its pair mask is NOT trivial (some pair of real atoms is excluded, or the triple is the
+ *       zero-shift diagonal ci == cj): the WHOLE cluster pair is kept iff inner_test() holds
+ *       -> one entry {ci, cj, s, kind 1};
+ *     - else, for each half h in {0,1} of cj (atoms h*C/2 .. h*C/2 + C/2 - 1): the half is kept iff
+ *       some real atom of the half is within fl32(rlist_inner^2) of some real atom of ci (A12 order)
+ *       -> one entry {ci, 2*cj + h, s, kind 0}.
+ *
+ * Same enumeration, sub-range rule, return value and output order (ci, cj, s, then kind-0 halves
+ * in h order) as oracle_lists.  Pins: tests/test_oracle_lists.py (numpy recomputation on a layout
+ * the test makes up, union-of-halves == inner flag of oracle_lists, completeness by k-d tree).
+ */
+long long oracle_half_lists(int nclusters, int C, const int32_t* atom_of_slot, const float* xq, const float* box,
+                            float rlist_outer, float rlist_inner, const int32_t* excl_off, const int32_t* excl_idx,
+                            int c_begin, int c_end, long long cap, int32_t* out_ci, int32_t* out_entry,
+                            int8_t* out_s /*[cap*3]*/, uint8_t* out_kind)
+{
+    float* lo = (float*)malloc(sizeof(float) * 3 * (size_t)nclusters);
+    float* hi = (float*)malloc(sizeof(float) * 3 * (size_t)nclusters);
+    int32_t* nv = (int32_t*)malloc(sizeof(int32_t) * (size_t)nclusters);
+    oracle_cluster_bb(nclusters, C, atom_of_slot, xq, lo, hi, nv);
+    float ro2 = rlist_outer * rlist_outer, ri2 = rlist_inner * rlist_inner;   /* fl32(r*r) */
+    const int H = C / 2;
+    long long total = 0;
+    long long* cnt = (long long*)calloc((size_t)nclusters + 1, sizeof(long long));
+    for (int pass = 0; pass < 2; pass++) {
+#pragma omp parallel for schedule(dynamic, 8)
+        for (int ci = 0; ci < nclusters; ci++) {
+            if (nv[ci] == 0) continue;
+            long long k = pass ? cnt[ci] : 0;
+            for (int cj = 0; cj < nclusters; cj++) {
+                if (nv[cj] == 0) continue;
+                if (!((ci >= c_begin && ci < c_end) || (cj >= c_begin && cj < c_end))) continue;
+                for (int sx = -1; sx <= 1; sx++)
+                    for (int sy = -1; sy <= 1; sy++)
+                        for (int sz = -1; sz <= 1; sz++) {
+                            int s[3] = { sx, sy, sz };
+                            if (!canonical(ci, cj, s)) continue;
+                            if (!(bb_dist2(lo + 3 * ci, hi + 3 * ci, lo + 3 * cj, hi + 3 * cj, s, box) < ro2)) continue;
+                            /* trivial mask: every pair of real atoms interacts */
+                            uint64_t m = pair_mask(C, atom_of_slot, excl_off, excl_idx, ci, cj, s), full = 0;
+                            for (int a = 0; a < C; a++)
+                                for (int b = 0; b < C; b++)
+                                    if (atom_of_slot[ci * C + a] >= 0 && atom_of_slot[cj * C + b] >= 0)
+                                        full |= (uint64_t)1 << (a * C + b);
+                            if (m != full) {
+                                if (inner_test(C, atom_of_slot, xq, box, ci, cj, s, ri2)) {
+                                    if (pass && k < cap) {
+                                        out_ci[k] = ci; out_entry[k] = cj; out_kind[k] = 1;
+                                        out_s[3 * k] = (int8_t)sx; out_s[3 * k + 1] = (int8_t)sy; out_s[3 * k + 2] = (int8_t)sz;
+                                    }
+                                    k++;
+                                }
+                                continue;
+                            }
+                            for (int h = 0; h < 2; h++) {
+                                int keep = 0;
+                                for (int a = 0; a < C && !keep; a++) {
+                                    if (atom_of_slot[ci * C + a] < 0) continue;
+                                    for (int b = h * H; b < (h + 1) * H; b++) {
+                                        if (atom_of_slot[cj * C + b] < 0) continue;
+                                        if (atom_dist2(xq + 4 * (ci * C + a), xq + 4 * (cj * C + b), s, box) < ri2) { keep = 1; break; }
+                                    }
+                                }
+                                if (!keep) continue;
+                                if (pass && k < cap) {
+                                    out_ci[k] = ci; out_entry[k] = 2 * cj + h; out_kind[k] = 0;
+                                    out_s[3 * k] = (int8_t)sx; out_s[3 * k + 1] = (int8_t)sy; out_s[3 * k + 2] = (int8_t)sz;
+                                }
+                                k++;
+                            }
                         }
             }
             if (!pass) cnt[ci + 1] = k;

@@ -19,7 +19,7 @@ _lib = None
 class _Params(C.Structure):
     _fields_ = [("coulomb", C.c_int32), ("lj_shift", C.c_int32), ("coul_shift", C.c_int32),
                 ("ntypes", C.c_int32), ("rc", C.c_double), ("beta", C.c_double),
-                ("eps_rf", C.c_double), ("epsfac", C.c_double)]
+                ("eps_rf", C.c_double), ("epsfac", C.c_double), ("rc_vdw", C.c_double)]
 
 
 EPSFAC = 138.935458  # reading A2
@@ -35,11 +35,12 @@ class Params:
     epsfac: float = EPSFAC
     lj_shift: bool = True
     coul_shift: bool = True
+    rc_vdw: float = 0.0  # twin cut-offs: LJ cut-off <= rc; <= 0: same as rc
 
     def c(self) -> _Params:
         return _Params({"ewald": 0, "rf": 1, "none": 2}[self.coulomb], int(self.lj_shift), int(self.coul_shift),
                        int(self.ntypes), float(self.rc), float(self.beta), float(self.eps_rf),
-                       float(self.epsfac))
+                       float(self.epsfac), float(self.rc_vdw))
 
 
 def lib():
@@ -177,3 +178,47 @@ def lists(atom_of_slot, xq, box, rlist_outer, rlist_inner, excl_off, excl_idx, c
             break
         cap = int(n)
     return ListResult(*bufs)
+
+
+@dataclasses.dataclass
+class HalfListResult:
+    ci: np.ndarray  # int32 [n]
+    entry: np.ndarray  # int32 [n]   kind 0: 2*cj + half;  kind 1: cj
+    s: np.ndarray  # int8 [n,3]   shift of ci, as in ListResult
+    kind: np.ndarray  # uint8 [n]  0 = half j-cluster of a cluster pair with a trivial mask, 1 = whole masked cluster pair
+
+    def keys(self) -> np.ndarray:
+        """Unique int64 key per entry (ci, entry, shift, kind)."""
+        sid = (self.s[:, 0].astype(np.int64) + 1) * 9 + (self.s[:, 1].astype(np.int64) + 1) * 3 \
+            + (self.s[:, 2].astype(np.int64) + 1)
+        return (self.ci.astype(np.int64) << 38) | (self.entry.astype(np.int64) << 9) | (sid << 1) | self.kind.astype(np.int64)
+
+
+def half_lists(atom_of_slot, xq, box, rlist_outer, rlist_inner, excl_off, excl_idx, cluster_size=8,
+               c_begin=0, c_end=None) -> HalfListResult:
+    """The inner list at half-j-cluster granularity (oracle_half_lists) on the exported layout."""
+    aos = np.ascontiguousarray(atom_of_slot, dtype=np.int32)
+    xq32 = np.ascontiguousarray(xq, dtype=np.float32).reshape(-1, 4)
+    b32 = np.ascontiguousarray(box, dtype=np.float32)
+    eo = np.ascontiguousarray(excl_off, dtype=np.int32)
+    ei = np.ascontiguousarray(excl_idx, dtype=np.int32)
+    if ei.size == 0:
+        ei = np.zeros(1, dtype=np.int32)
+    ncl = aos.shape[0] // cluster_size
+    if c_end is None:
+        c_end = ncl
+    lib().oracle_half_lists.restype = C.c_longlong
+    cap = 0
+    for _ in range(2):
+        ci = np.zeros(max(cap, 1), dtype=np.int32)
+        ent = np.zeros(max(cap, 1), dtype=np.int32)
+        s = np.zeros((max(cap, 1), 3), dtype=np.int8)
+        kind = np.zeros(max(cap, 1), dtype=np.uint8)
+        n = lib().oracle_half_lists(C.c_int(ncl), C.c_int(cluster_size), _ptr(aos), _ptr(xq32), _ptr(b32),
+                                    C.c_float(rlist_outer), C.c_float(rlist_inner), _ptr(eo), _ptr(ei),
+                                    C.c_int(c_begin), C.c_int(c_end), C.c_longlong(cap), _ptr(ci), _ptr(ent),
+                                    _ptr(s), _ptr(kind))
+        if n <= cap:
+            return HalfListResult(ci[:n], ent[:n], s[:n], kind[:n])
+        cap = int(n)
+    raise RuntimeError("oracle_half_lists: count changed between passes")

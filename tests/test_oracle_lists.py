@@ -134,3 +134,123 @@ def test_canonicalise_roundtrip():
     assert a.tolist() == [2, 5, 7] and b.tolist() == [5, 2, 7]
     assert t.tolist() == [[0, 0, 0], [1, 0, -1], [0, 0, 0]]
     assert mt.tolist() == [1 << (2 * 8 + 1), 1 << (4 * 8 + 3), 5]
+
+
+# ---------------------------------------------------------------- fp32 recomputation in numpy (reading A12)
+def _fma32(a, b, c):
+    """fmaf for float32 arrays: the product of two float32 is exact in float64; the sum is rounded to
+    float64 and then to float32 (a double rounding could differ from fmaf only when the float64 sum
+    lands exactly on a float32 midpoint, ~1e-9 per operation; inputs are seeded, so deterministic)."""
+    return (a.astype(np.float64) * b.astype(np.float64) + c.astype(np.float64)).astype(np.float32)
+
+
+def _cluster_bbs(aos, xq, C=8):
+    x = np.where((aos >= 0)[:, None], xq[:, :3], np.nan).reshape(-1, C, 3)
+    with np.errstate(all="ignore"):
+        return np.nanmin(x, axis=1).astype(np.float32), np.nanmax(x, axis=1).astype(np.float32)
+
+
+def _all_canonical_triples(ncl):
+    ci, cj, sx, sy, sz = np.meshgrid(np.arange(ncl), np.arange(ncl), *[np.arange(-1, 2)] * 3, indexing="ij")
+    ci, cj = ci.ravel(), cj.ravel()
+    s = np.stack([sx.ravel(), sy.ravel(), sz.ravel()], axis=1)
+    lex = np.where(s[:, 0] != 0, s[:, 0], np.where(s[:, 1] != 0, s[:, 1], s[:, 2]))
+    keep = (lex > 0) | ((lex == 0) & (cj >= ci))
+    return ci[keep], cj[keep], s[keep]
+
+
+def _bb_dist2_np(lo, hi, ci, cj, s, box):
+    sL = (s.astype(np.float32) * box[None, :].astype(np.float32))          # exact: s in {-1,0,1}
+    a = (sL + lo[ci]).astype(np.float32) - hi[cj]                            # fmaf(s,L,lo_i) - hi_j
+    b = lo[cj] - (sL + hi[ci]).astype(np.float32)                            # lo_j - fmaf(s,L,hi_i)
+    g = np.maximum(np.maximum(a, b), np.float32(0)).astype(np.float32)
+    return _fma32(g[:, 2], g[:, 2], _fma32(g[:, 1], g[:, 1], (g[:, 0] * g[:, 0]).astype(np.float32)))
+
+
+def _atom_d2_np(xq, slots_i, slots_j, s, box):
+    """[n, len(slots_i[0]), len(slots_j[0])] float32 distances d = x_a + s L - x_b in the A12 order."""
+    sL = (s.astype(np.float32) * box[None, :].astype(np.float32))
+    xi = (xq[slots_i, :3] + sL[:, None, :]).astype(np.float32)               # fmaf(s, L, x_a): s L exact
+    d = (xi[:, :, None, :] - xq[slots_j, :3][:, None, :, :]).astype(np.float32)
+    return _fma32(d[..., 2], d[..., 2], _fma32(d[..., 1], d[..., 1], (d[..., 0] * d[..., 0]).astype(np.float32)))
+
+
+def test_bb_predicate_is_exact_both_ways(small):
+    """Pin against OVER-listing as well as under-listing at C = 8: over ALL canonical (ci, cj, s) of a
+    test-made layout, listed <=> D2_bb < fl32(r^2) with D2_bb recomputed in numpy float32.  A lo/hi mix-up,
+    a shift on the wrong side or a wrong sign in the gap changes the listed set."""
+    w = small
+    aos, xq = _simple_layout(w)
+    res = O.lists(aos, xq, w.box, w.rlist_outer, w.rlist_inner, w.excl_off, w.excl_idx)
+    lo, hi = _cluster_bbs(aos, xq)
+    ncl = aos.size // 8
+    ci, cj, s = _all_canonical_triples(ncl)
+    d2 = _bb_dist2_np(lo, hi, ci, cj, s, w.box)
+    r2 = np.float32(w.rlist_outer) * np.float32(w.rlist_outer)
+    want = d2 < r2
+    listed = np.isin(LC.triple_keys(ci, cj, s), res.keys())
+    assert want.sum() > 500 and (~want).sum() > 500
+    assert np.array_equal(listed, want)
+    # the band around the threshold is populated on both sides: the comparison really is decided there
+    near = np.abs(np.sqrt(d2.astype(np.float64)) - w.rlist_outer) < 0.05
+    assert (want & near).sum() > 20 and (~want & near).sum() > 20
+
+
+def test_half_lists_against_numpy(small):
+    """oracle_half_lists recomputed in numpy float32 on a test-made layout: whole masked cluster pairs and
+    surviving halves of the unmasked ones, bit-exact as sets; halves are consistent with the inner flag
+    of oracle_lists; every atom pair within rlist_inner is covered; every listed half has a close pair."""
+    w = small
+    aos, xq = _simple_layout(w)
+    res = O.lists(aos, xq, w.box, w.rlist_outer, w.rlist_inner, w.excl_off, w.excl_idx)
+    hl = O.half_lists(aos, xq, w.box, w.rlist_outer, w.rlist_inner, w.excl_off, w.excl_idx)
+    assert np.unique(hl.keys()).size == hl.keys().size
+    valid = (aos >= 0).reshape(-1, 8)
+    full = np.zeros(res.ci.size, dtype=np.uint64)
+    for a in range(8):
+        for b in range(8):
+            full |= (valid[res.ci, a] & valid[res.cj, b]).astype(np.uint64) << np.uint64(a * 8 + b)
+    masked = res.pairmask != full
+    diag = (res.ci == res.cj) & (res.s == 0).all(axis=1)
+    assert masked[diag].all() and masked.sum() > diag.sum()           # water: intramolecular exclusions too
+    ri2 = np.float32(w.rlist_inner) * np.float32(w.rlist_inner)
+    si = res.ci[:, None] * 8 + np.arange(8)[None, :]
+    sj = res.cj[:, None] * 8 + np.arange(8)[None, :]
+    d2 = _atom_d2_np(xq, si, sj, res.s.astype(np.int64), w.box)       # [n, 8, 8]
+    ok = valid[res.ci][:, :, None] & valid[res.cj][:, None, :]
+    close = (d2 < ri2) & ok
+    upper = np.triu(np.ones((8, 8), bool), 1)                          # diagonal cluster pair: b > a only
+    close_m = np.where(diag[:, None, None], close & upper[None], close)
+    want = set()
+    sid = LC.shift_id(res.s)
+    for k in range(res.ci.size):
+        if masked[k]:
+            if close_m[k].any():
+                want.add((int(res.ci[k]), int(res.cj[k]), int(sid[k]), 1))
+        else:
+            for h in range(2):
+                if close[k][:, 4 * h:4 * h + 4].any():
+                    want.add((int(res.ci[k]), 2 * int(res.cj[k]) + h, int(sid[k]), 0))
+    got = set(zip(hl.ci.tolist(), hl.entry.tolist(), LC.shift_id(hl.s).tolist(), hl.kind.tolist()))
+    assert got == want and sum(1 for g in got if g[3] == 0) > 300 and sum(1 for g in got if g[3] == 1) > 20
+    # consistency with oracle_lists: the cluster pairs spanned by the entries are exactly the inner triples
+    spanned = {(c, e // 2 if kd == 0 else e, k) for c, e, k, kd in got}
+    inner = set(zip(res.ci[res.inner].tolist(), res.cj[res.inner].tolist(), sid[res.inner].tolist()))
+    assert spanned == inner
+    # strictly finer than whole clusters: some surviving unmasked cluster pairs keep one half only
+    unm = [(c, e // 2, k) for c, e, k, kd in got if kd == 0]
+    assert len(unm) > len(set(unm)) > 0.55 * len(unm)
+    # completeness in fp64, layout-independent (k-d tree): every atom pair closer than rlist_inner is covered
+    pi, pj, sp, _ = LC.close_atom_pairs(aos, xq, w.box, w.rlist_inner - 1e-6)
+    ka, kb = LC.shift_id(sp), LC.shift_id(-sp)
+    miss = 0
+    for a, b, k1, k2 in zip(pi.tolist(), pj.tolist(), ka.tolist(), kb.tolist()):
+        if not ((a // 8, b // 4, k1, 0) in got or (b // 8, a // 4, k2, 0) in got
+                or (a // 8, b // 8, k1, 1) in got or (b // 8, a // 8, k2, 1) in got):
+            miss += 1
+    assert miss == 0 and pi.size > 1000
+    # sub-range enumeration = selection of the full one
+    part = O.half_lists(aos, xq, w.box, w.rlist_outer, w.rlist_inner, w.excl_off, w.excl_idx, c_begin=3, c_end=6)
+    cj_full = np.where(hl.kind == 0, hl.entry // 2, hl.entry)
+    sel = ((hl.ci >= 3) & (hl.ci < 6)) | ((cj_full >= 3) & (cj_full < 6))
+    assert np.array_equal(np.sort(hl.keys()[sel]), np.sort(part.keys()))
