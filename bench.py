@@ -9,9 +9,12 @@ One "step" is one MD step of the whole hot path on the synthetic water box, in t
 schedule: every step stages new coordinates
 (nb_put_atoms) and computes forces (nb_forces); every nstlist-th step first rebuilds the grid and
 the outer pair list (nb_search) and prunes it fully; every other step prunes one rolling part of
-the outer list (nb_prune) before the forces.  So K = nstlist steps contain every row of SURVEY 8(a)
-in the proportions the method prescribes.  `value` = effective pair interactions (non-excluded
-atom pairs with r < rc, the paper's "effective" throughput, L167-L173) per second.
+the outer list (nb_prune) before the forces.  Whatever --steps is, BOTH kinds of step are timed in
+the same run: K inner steps and S = max(3, ceil(K/nstlist)) search steps (the schedule is restarted
+S times), and ms_per_step = (mean search step + (nstlist-1) * mean inner step) / nstlist is the cost
+of a step in the proportions the method prescribes -- every row of SURVEY 8(a) is inside it.
+`value` = effective pair interactions (non-excluded atom pairs with r < rc, the paper's "effective"
+throughput, L167-L173) per second = mean pairs per step / ms_per_step.
 
 N > 1 (torchrun): the path does not shard ("replicas only"): every rank runs an
 independent replica on its own GPU, no data-path collective; value = sum over ranks / max time.
@@ -36,10 +39,42 @@ UNIT = "pairs/s"
 # FADD/FMUL/MUFU/compare/select = 1 -- divided by the 256 slots of a warp step.  (SURVEY 8.4's estimate of the
 # method's work was 62 / 40; the smaller executed count is the one used.)
 FLOP_PER_SLOT = {"ewald": 54.75, "rf": 35.75, "none": 30.75}
-# DRAM bytes of one force-kernel launch from the committed ncu --set full capture (profiles/r1c_force_full_cfg2.md);
-# the kernel is ALU-bound, its HBM traffic is ~0.2 % of what the HBM roofline would allow in the same time.
-NCU_DRAM_BYTES_PER_LAUNCH = {(2, "ewald"): 14.8e6}
 N_SM, FP32_LANES_PER_SM = 148, 128   # B200_PROFILING.md: 148 SMs; 128 FP32 lanes/SM (4 SMSP x 32)
+HBM_FALLBACK_GBS = 6650.0            # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+PRUNE_FLOP_PER_CHECK = 8             # 3 sub + 1 mul + 2 fma (= 5 more flop) per atom-pair distance check
+GRID_BYTES_PER_ATOM = 120            # algorithmic bytes of (a2) per atom
+
+
+def measured_hbm_gbs():
+    """(GB/s, source): the driver-measured copy bandwidth, else the profiling guide's fallback."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(kernel, config, coulomb):
+    """DRAM bytes per launch of `kernel` ("force" / "prune") from the NEWEST committed ncu --set full summary
+    under profiles/ for this workload (dram__bytes_read.sum + dram__bytes_write.sum of its first captured
+    launch), or (None, reason).  Nothing is hard-coded: a summary that is not there gives null."""
+    import glob
+    import re
+    tag = f"cfg{config}" + ("_rf" if coulomb == "rf" else "")
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", f"r*_{kernel}_full_{tag}.md")))
+    if not files:
+        return None, f"no profiles/r*_{kernel}_full_{tag}.md committed for this workload"
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    total, found = 0.0, 0
+    with open(files[-1]) as fh:
+        for line in fh:
+            m = re.match(r"\| `dram__bytes_(read|write)\.sum` \| (\w+) \| ([0-9.eE+-]+) \|", line)
+            if m and m.group(2) in scale:
+                total += float(m.group(3)) * scale[m.group(2)]
+                found += 1
+    if found < 2:
+        return None, f"{os.path.basename(files[-1])} has no dram__bytes rows"
+    return total, "profiles/" + os.path.basename(files[-1])
 
 
 def parse_args():
@@ -57,6 +92,9 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-flush", action="store_true", help="do not flush L2 between timed steps")
+    ap.add_argument("--prune", default="overlapped", choices=["plain", "overlapped"],
+                    help="rolling prune on the caller's stream before the force kernel (plain) or on the library's second "
+                         "stream next to it (overlapped, PAPER.md L193)")
     return ap.parse_args()
 
 
@@ -132,7 +170,7 @@ class ClockSampler(threading.Thread):
 class Replica:
     """One box on one GPU, driven through the Python binding of the C ABI."""
 
-    def __init__(self, w, device_index, flush):
+    def __init__(self, w, device_index, flush, overlapped=False):
         import numpy as np
         import torch
         from paper_2006_09167_b200 import nb
@@ -159,6 +197,14 @@ class Replica:
         self.flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device=self.dev) if flush else None
         self.pairs_at_frame = None
         self.slots_at_frame = None
+        self.overlapped = overlapped
+
+    def _rolling_prune(self, fr):
+        w, c = self.w, self.ctx
+        if self.overlapped:
+            c.prune_overlapped(w.rlist_inner, fr % w.nparts, w.nparts)   # next to the force kernel (L193)
+        else:
+            c.prune(w.rlist_inner, fr % w.nparts, w.nparts)              # rolling part (L193)
 
     def step_device(self, t):
         """Inputs already in HBM (the `value` leg)."""
@@ -171,7 +217,7 @@ class Replica:
             c.prune(w.rlist_inner, 0, 1)           # first use of a fresh list: full prune
             c.forces(self.f_dev, self.e_dev, self.v_dev)   # energies + virial once per list lifetime
         else:
-            c.prune(w.rlist_inner, fr % w.nparts, w.nparts)   # rolling part (L193)
+            self._rolling_prune(fr)
             c.forces(self.f_dev, None, None)
 
     def step_host(self, t):
@@ -185,7 +231,7 @@ class Replica:
             c.prune(w.rlist_inner, 0, 1)
             c.forces_host(self.f_host.numpy(), self.e_host.numpy(), self.v_host.numpy())
         else:
-            c.prune(w.rlist_inner, fr % w.nparts, w.nparts)
+            self._rolling_prune(fr)
             c.forces_host(self.f_host.numpy(), None, None)
 
     def flush(self):
@@ -203,23 +249,50 @@ class Replica:
             self.pairs_at_frame.append(n_int)
             self.slots_at_frame.append(self.ctx.count_slots())
 
-    def timed(self, step_fn, t0, nsteps):
-        """Times nsteps steps starting at schedule position t0 with one CUDA-event pair per step on
-        the stream the library launches on; returns (total ms, effective pairs, slots)."""
+    @staticmethod
+    def schedule(nstlist, k_inner):
+        """Schedule positions of the timed region: S = max(3, ceil(K/nstlist)) list lifetimes are started (a
+        search step at position 0 each) and K inner steps follow them, spread evenly; every step is timed."""
+        n_search = max(3, -(-k_inner // max(nstlist - 1, 1)))
+        per = [k_inner // n_search + (1 if i < k_inner % n_search else 0) for i in range(n_search)]
+        pos = []
+        for n in per:
+            pos.append(0)
+            pos.extend(1 + (j % max(nstlist - 1, 1)) for j in range(n))
+        return pos
+
+    def timed(self, step_fn, positions):
+        """Times the steps at the given schedule positions with one CUDA-event pair per step on the stream
+        the library launches on.  Returns {"search"/"inner": (ms, steps, effective pairs, slots)}."""
         torch = self.torch
         stream = torch.cuda.current_stream(self.dev)
-        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(nsteps)]
-        pairs = slots = 0
-        for i in range(nsteps):
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in positions]
+        for i, t in enumerate(positions):
             self.flush()
             ev[i][0].record(stream)
-            step_fn(t0 + i)
+            step_fn(t)
             ev[i][1].record(stream)
-            fr = (t0 + i) % self.w.nstlist
-            pairs += self.pairs_at_frame[fr]
-            slots += self.slots_at_frame[fr]
         torch.cuda.synchronize(self.dev)
-        return sum(a.elapsed_time(b) for a, b in ev), pairs, slots
+        out = {"search": [0.0, 0, 0, 0], "inner": [0.0, 0, 0, 0]}
+        for (a, b), t in zip(ev, positions):
+            fr = t % self.w.nstlist
+            o = out["search" if fr == 0 else "inner"]
+            o[0] += a.elapsed_time(b)
+            o[1] += 1
+            o[2] += self.pairs_at_frame[fr]
+            o[3] += self.slots_at_frame[fr]
+        return out
+
+
+def schedule_mean(pop, nstlist):
+    """(ms per step, pairs per step, slots per step) of the method's schedule -- one search step and
+    nstlist-1 inner steps per list lifetime -- from the two timed populations."""
+    s, i = pop["search"], pop["inner"]
+    if i[1] == 0:
+        return s[0] / s[1], s[2] / s[1], s[3] / s[1]
+    wts, wti = 1.0 / nstlist, (nstlist - 1.0) / nstlist
+    return (wts * s[0] / s[1] + wti * i[0] / i[1], wts * s[2] / s[1] + wti * i[2] / i[1],
+            wts * s[3] / s[1] + wti * i[3] / i[1])
 
 
 def cpu_baseline(w, budget_s=12.0):
@@ -243,8 +316,9 @@ def cpu_baseline(w, budget_s=12.0):
 
 def run_reference(args):
     """--impl reference: the oracle on the host cores, same metric/unit.  Each step is one oracle
-    force evaluation of a water box made by the same recipe at the same density, sized so that the
-    whole --steps/--warmup run ends within a few minutes (a bounded sample of the workload)."""
+    force+energy+virial evaluation of the BENCHED workload itself (same seeded box as the b200 arm);
+    only when the whole --steps/--warmup run would not end within a few minutes is a smaller box of
+    the same recipe/density/cut-offs evaluated instead, and the line says which."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
@@ -267,16 +341,23 @@ def run_reference(args):
         r = O.forces(w.x, w.q, w.type, w.box, w.lj_c6c12, w.excl_off, w.excl_idx, p, method="cells")
         return time.perf_counter() - t0, r.npairs
 
-    min_side = int(3.0 * full.rc * workloads.MOLECULES_PER_NM3 ** (1.0 / 3.0)) + 2   # >= 3 cells of rc per axis
-    probe = make(min_side)
-    evaluate(probe)
-    dt, _ = evaluate(probe)
-    per_mol = dt / min_side ** 3
-    nside = min_side
-    full_side = round((full.natoms / 3) ** (1.0 / 3.0))
-    while nside + 1 <= full_side and per_mol * (nside + 1) ** 3 * nsteps <= budget:
-        nside += 1
-    w = probe if nside == min_side else make(nside)
+    evaluate(full)                       # (pages the library and the box in)
+    dt_full, _ = evaluate(full)
+    if dt_full * nsteps <= budget:
+        w, which = full, "the benched workload itself"
+    else:
+        min_side = int(3.0 * full.rc * workloads.MOLECULES_PER_NM3 ** (1.0 / 3.0)) + 2   # >= 3 cells of rc per axis
+        probe = make(min_side)
+        evaluate(probe)
+        dt, _ = evaluate(probe)
+        per_mol = dt / min_side ** 3
+        nside = min_side
+        full_side = round((full.natoms / 3) ** (1.0 / 3.0))
+        while nside + 1 <= full_side and per_mol * (nside + 1) ** 3 * nsteps <= budget:
+            nside += 1
+        w = probe if nside == min_side else make(nside)
+        which = (f"a {w.natoms}-atom water box of the same recipe/density/cut-offs (the {full.natoms}-atom workload would "
+                 f"take {dt_full * nsteps:.0f} s for {nsteps} evaluations, over the {budget:.0f} s budget)")
     for _ in range(args.warmup):
         evaluate(w)
     spent, npairs = 0.0, 0
@@ -285,12 +366,12 @@ def run_reference(args):
         spent += dt
         npairs += n
     value = npairs / spent
-    sample = (f"each step = one oracle_forces_cells evaluation (fp64, force+energy+virial) of a {w.natoms}-atom "
-              f"water box, same recipe/density/cut-offs as the workload ({full.natoms} atoms)")
+    sample = f"each step = one oracle_forces_cells evaluation (fp64, force+energy+virial) of {which}"
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * spent / max(args.steps, 1),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(full, args, {"reference_sample_atoms": w.natoms}),
+            "config": workload_config(full, args, {"reference_sample_atoms": w.natoms,
+                                                   "reference_sample": "full workload" if w is full else "sized sample"}),
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -360,12 +441,14 @@ def run_b200(args):
     barrier, max_over_ranks, sum_over_ranks = ranks.barrier, ranks.max, ranks.sum
 
     w = load_workload(args)
-    rep = Replica(w, local_rank, flush=not args.no_flush)
+    rep = Replica(w, local_rank, flush=not args.no_flush, overlapped=args.prune == "overlapped" and w.nparts <= 32)
     ctx = rep.ctx
     fma_peak = ctx.measure_fp32_peak()          # lane-FMA/s of a register-resident FFMA chain, this GPU, now
     rep.count_pass()                            # untimed: per-frame pair and slot counts (also warms everything up)
     W = max(args.warmup, 3)
     K = args.steps
+    positions = Replica.schedule(w.nstlist, K)  # K inner steps + S >= 3 search steps, all timed
+    S = sum(1 for t in positions if t == 0)
 
     # ---------------- device-resident leg: `value` ----------------
     for i in range(W):
@@ -373,8 +456,8 @@ def run_b200(args):
     # Inside the timed region only the force kernel (the roofline's kernel) carries an event pair:
     # every timed stage costs two event records per call (~3 us of stream time per stage and step;
     # with all seven stages timed the step was 13-26 % longer).  The other stages are timed in a
-    # second pass over the same K steps that does not count towards `value`.
-    force_bit = 1 << nb.NB_T_NAMES.index("force")
+    # second pass over the same steps that does not count towards `value`.
+    force_bit = (1 << nb.NB_T_NAMES.index("force")) | (1 << nb.NB_T_NAMES.index("force_energy"))
     ctx.timing_stages(force_bit)
     ctx.timing_enable(True)
     ctx.timing_read(reset=True)
@@ -382,21 +465,26 @@ def run_b200(args):
     barrier()
     sampler = ClockSampler(local_rank)
     sampler.start()
-    ms, pairs, slots = rep.timed(rep.step_device, W, K)
+    pop = rep.timed(rep.step_device, positions)
     barrier()
     clocks = sampler.result()
     stages = ctx.timing_read(reset=True)
-    launches1 = ctx.get_stats()["kernel_launches"]
+    st1 = ctx.get_stats()
+    launches = st1["kernel_launches"] - launches0 - 3   # get_stats itself launches three counting kernels
+    # second pass, plain prune (the stage timer brackets launches on the caller's stream): the other stages
     ctx.timing_stages(0xFFFFFFFF & ~force_bit)
-    rep.timed(rep.step_device, W, K)
+    was_overlapped, rep.overlapped = rep.overlapped, False
+    rep.timed(rep.step_device, positions)
+    rep.overlapped = was_overlapped
     stages_other = ctx.timing_read(reset=True)
-    stages = {k: (stages[k] if k == "force" else stages_other[k]) for k in stages}
+    stages = {k: (stages[k] if k in ("force", "force_energy") else stages_other[k]) for k in stages}
     ctx.timing_stages(0xFFFFFFFF)
     ctx.timing_enable(False)
-    launches = launches1 - launches0 - 1   # get_stats itself launches one counting kernel
-    ms_max = max_over_ranks(ms)
-    pairs_all = sum_over_ranks(float(pairs))
-    value = pairs_all / (ms_max * 1e-3)
+    ms_step, pairs_step, slots_step = schedule_mean(pop, w.nstlist)
+    ms_step_max = max_over_ranks(ms_step)
+    value = sum_over_ranks(float(pairs_step)) / (ms_step_max * 1e-3)
+    ms_search = max_over_ranks(pop["search"][0] / max(pop["search"][1], 1))
+    ms_inner = max_over_ranks(pop["inner"][0] / max(pop["inner"][1], 1))
 
     # ---------------- host-buffer leg: `e2e` ----------------
     e2e = None
@@ -404,50 +492,92 @@ def run_b200(args):
         for i in range(W):
             rep.step_host(i)
         barrier()
-        ms_h, pairs_h, _ = rep.timed(rep.step_host, W, K)
+        pop_h = rep.timed(rep.step_host, positions)
         barrier()
+        ms_h, pairs_h, _ = schedule_mean(pop_h, w.nstlist)
         ms_h_max = max_over_ranks(ms_h)
         n = w.natoms
-        n_energy_steps = sum(1 for i in range(W, W + K) if i % w.nstlist == 0)
         e2e = {"value": sum_over_ranks(float(pairs_h)) / (ms_h_max * 1e-3), "unit": UNIT,
-               "h2d_bytes_per_step": n * 12 + n * 8 * n_energy_steps / max(K, 1),   # x every step; q, type on search steps
-               "d2h_bytes_per_step": n * 12 + (11 * 8 * n_energy_steps) / max(K, 1),
-               "ms_per_step": ms_h_max / max(K, 1)}
+               "h2d_bytes_per_step": n * 12 + n * 8 / w.nstlist,        # x every step; q, type on search steps
+               "d2h_bytes_per_step": n * 12 + 11 * 8 / w.nstlist,       # f every step; energies + virial on search steps
+               "ms_per_step": ms_h_max, "ms_search_step": pop_h["search"][0] / max(pop_h["search"][1], 1),
+               "ms_inner_step": pop_h["inner"][0] / max(pop_h["inner"][1], 1)}
 
-    # ---------------- roofline of the dominant kernel (force kernel, FP32 ALU bound) ----------------
-    f_ms, f_n = stages["force"]
+    # ---------------- rooflines ----------------
     sm_max = clocks["sm_max_mhz"] or 1965
     peak_tflops = N_SM * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    hbm_gbs, hbm_src = measured_hbm_gbs()
+    per_stage_us = {k: (1e3 * v[0] / v[1] if v[1] else None) for k, v in stages.items()}
+    # dominant kernel: the force kernel (FP32 ALU bound), F-only flavour of the inner steps
+    f_ms, f_n = stages["force"]
     flop_slot = FLOP_PER_SLOT[w.coulomb]
-    slots_per_launch = slots / max(K, 1)
+    slots_per_launch = pop["inner"][3] / max(pop["inner"][1], 1)
     force_us = 1e3 * f_ms / max(f_n, 1)
     achieved = flop_slot * slots_per_launch / (force_us * 1e-6) / 1e12 if f_n else 0.0
+    workload_is_config = args.lj_rc <= 0 and args.water_nside <= 0
+    traffic, traffic_src = ncu_traffic("force", args.config, w.coulomb) if workload_is_config else (None, "not a BASELINE config")
     roofline = {"bound": "alu", "kernel": "k_force (a7)", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-                "frac": achieved / peak_tflops, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((args.config, w.coulomb)) if args.lj_rc <= 0 and args.water_nside <= 0 else None,
-                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one k_force launch, ncu --set full "
-                                  "(profiles/, latest force_full summary); null = not captured for this workload",
+                "frac": achieved / peak_tflops, "traffic": traffic,
+                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one k_force launch, ncu --set full: " + traffic_src,
                 "peak_source": f"derived: {N_SM} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x {sm_max} MHz (clocks.max.sm); "
                                "MEASURED_PEAKS.json has no FP32 entry",
                 "measured_ffma_chain_tflops": 2 * fma_peak / 1e12,
                 "frac_of_measured_ffma_chain": achieved / (2 * fma_peak / 1e12),
-                "flop_per_slot": flop_slot, "slots_per_launch": slots_per_launch, "kernel_us": force_us}
+                "flop_per_slot": flop_slot, "slots_per_launch": slots_per_launch, "kernel_us": force_us,
+                "kernel_us_is": "mean of the F-only launches (the inner steps) inside the timed region; the F+E+virial launches of "
+                                "the search steps are stage_us.force_energy"}
 
+    line = None
     if rank == 0:
-        st = ctx.get_stats()
-        per_stage_us = {k: (1e3 * v[0] / v[1] if v[1] else None) for k, v in stages.items()}
+        st = st1
+        # prune kernel (a6): one rolling part per inner step; arithmetic = 64 distance checks per outer cluster pair
+        n_outer, n_half = st["n_pairs_outer"], slots_step / 32.0
+        p_us = per_stage_us["prune"]
+        prune_launch_pairs = n_outer * (S + (pop["inner"][1]) / w.nparts) / max(S + pop["inner"][1], 1)   # mean over full + rolling launches
+        prune_flop = prune_launch_pairs * 64 * PRUNE_FLOP_PER_CHECK
+        prune_bytes = prune_launch_pairs * 4 + st["nslots"] * 16 + (prune_launch_pairs / max(n_outer, 1)) * n_half * 4
+        ptraffic, ptraffic_src = ncu_traffic("prune", args.config, w.coulomb) if workload_is_config else (None, "not a BASELINE config")
+        roofline_prune = None
+        if p_us:
+            roofline_prune = {"kernel": "k_prune (a6)", "kernel_us": p_us,
+                              "kernel_us_is": "mean over the timed launches: S full prunes and K rolling parts (plain-prune pass)",
+                              "bound": "alu", "achieved": prune_flop / (p_us * 1e-6) / 1e12, "peak": peak_tflops, "unit": "TFLOP/s",
+                              "frac": prune_flop / (p_us * 1e-6) / 1e12 / peak_tflops,
+                              "flop_per_check": PRUNE_FLOP_PER_CHECK, "checks_per_launch": prune_launch_pairs * 64,
+                              "hbm": {"achieved": prune_bytes / (p_us * 1e-6) / 1e9, "peak": hbm_gbs, "unit": "GB/s",
+                                      "frac": prune_bytes / (p_us * 1e-6) / 1e9 / hbm_gbs, "peak_source": hbm_src,
+                                      "algorithmic_bytes_per_launch": prune_bytes,
+                                      "bytes_are": "4 B per outer cluster pair read + xq once (16 B/slot) + 4 B per surviving half entry written",
+                                      "traffic": ptraffic, "traffic_source": ptraffic_src}}
+        # gridding (a2): HBM-side algorithmic bytes, and what the launch count alone costs
+        g_us = per_stage_us["grid"]
+        roofline_grid = None
+        if g_us:
+            gbytes = GRID_BYTES_PER_ATOM * w.natoms
+            roofline_grid = {"kernels": "k_bin, k_col_scan, k_col_scatter, k_col_layout, k_grid_tail (a2)", "stage_us": g_us,
+                             "bound": "hbm", "bytes_per_atom": GRID_BYTES_PER_ATOM, "achieved": gbytes / (g_us * 1e-6) / 1e9,
+                             "peak": hbm_gbs, "unit": "GB/s", "frac": gbytes / (g_us * 1e-6) / 1e9 / hbm_gbs, "peak_source": hbm_src,
+                             "launches": 5, "launch_floor_us": 5 * 2.5,
+                             "note": "latency- and sort-bound at these sizes: five dependent launches (~2.5 us each) and a "
+                                     "per-column shared-memory sort; once per nstlist steps"}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-                "ms_per_step": ms_max / max(K, 1), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "ms_per_step": ms_step_max, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic",
                 "config": workload_config(w, args, {"l2": "flushed between timed steps (256 MiB fill)" if not args.no_flush
-                                                    else "not flushed"}),
+                                                    else "not flushed", "prune": "overlapped" if rep.overlapped else "plain"}),
+                "schedule": {"timed_inner_steps": pop["inner"][1], "timed_search_steps": S, "ms_inner_step": ms_inner,
+                             "ms_search_step": ms_search,
+                             "ms_per_step_is": "(ms_search_step + (nstlist-1) * ms_inner_step) / nstlist"},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
-                "raw_pairs_per_s_per_gpu": slots / (ms * 1e-3),
-                "work_efficiency": pairs / max(slots, 1),
+                "roofline_prune": roofline_prune, "roofline_grid": roofline_grid,
+                "raw_pairs_per_s_per_gpu": slots_step / (ms_step * 1e-3),
+                "work_efficiency": pairs_step / max(slots_step, 1),
                 "stage_us": per_stage_us,
-                "stage_share_of_step": {k: v[0] / ms for k, v in stages.items()},
-                "stage_timing": "force: event pair inside the timed region; other stages: second pass over the same steps",
+                "stage_share_of_step": {k: ((v / w.nstlist if k in ("grid", "search", "masks") else v) / (1e3 * ms_step) if v else None)
+                                        for k, v in per_stage_us.items()},
+                "stage_timing": "force: event pair inside the timed region; other stages: second pass over the same steps with the plain prune",
                 "list": {k: st[k] for k in ("nsuper", "n_sci_entries", "n_joint_outer", "n_pairs_outer", "n_pairs_inner",
-                                            "n_excl_masks", "n_work_units")}}
+                                            "n_excl_masks", "n_work_units", "list_grow_retries")}}
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(w)
         print(json.dumps(line))

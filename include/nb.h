@@ -14,8 +14,9 @@
  *  - Every call returns NB_OK or a negative NB_ERR_* code; nothing throws or exits.
  *    nb_last_error() gives a message for the last failure on that context.
  *  - All work is enqueued on the stream given in nb_params and returns without
- *    synchronising, except nb_search (reads list sizes back to size buffers) and the
- *    introspection / _host calls.
+ *    synchronising, except nb_search (one synchronisation at its end to read the list sizes
+ *    back) and the introspection / _host calls.  Every call switches to the context's device
+ *    and restores the caller's current device before returning.
  *  - Call order: nb_init -> nb_put_atoms -> nb_search -> { nb_put_atoms -> [nb_prune] ->
  *    nb_forces }* -> nb_put_atoms -> nb_search ...; violations return NB_ERR_STATE.
  *  - Units: nm, kJ/mol, e.  Rectangular periodic boxes only.  natoms, types, charges'
@@ -67,6 +68,9 @@ typedef struct {
     int32_t coul_modifier;           /* Ewald only; reaction-field always carries its own constant c_rf */
     int32_t device;                  /* CUDA ordinal */
     void* stream;                    /* cudaStream_t (NULL = legacy default stream) */
+    float rc_vdw;                    /* twin cut-offs (PME load balancing scales only the electrostatics
+                                        cut-off): LJ interacts iff r^2 < rc_vdw^2 and its potential shift is taken at rc_vdw;
+                                        0 -> rc (single cut-off); otherwise 0 < rc_vdw <= rc */
 } nb_params;
 
 /* Counters for the last calls; all device work they describe has completed when
@@ -80,15 +84,17 @@ typedef struct {
     int64_t n_pairs_inner;           /* cluster pairs with the inner mask bit set (after pruning) */
     int64_t n_excl_masks;            /* joint entries carrying a non-trivial exclusion mask */
     int64_t n_work_units;            /* list chunks scheduled by the force/prune kernels (L199-L201) */
-    int64_t slots_last_forces;       /* atom-pair slots evaluated by the last nb_forces = 64 * n_pairs_inner */
+    int64_t slots_last_forces;       /* atom-pair slots the force kernel evaluates over the current inner list (= nb_count_slots):
+                                        32 per surviving half j-cluster, 64 per masked cluster pair; 0 before the first nb_forces */
     int64_t kernel_launches;         /* kernels launched by this context so far */
     int64_t search_count, prune_count, force_count;
-    int32_t list_grow_retries;
+    int32_t list_grow_retries;       /* searches repeated because a list buffer sized from the previous search was too small */
     float ewald_beta;
 } nb_stats;
 
 /* Creates a context.  Copies the LJ table and exclusions.  NB_ERR_ARG on bad sizes,
- * an exclusion index out of range, rc <= 0, or (beta*rc)^2 > 12. */
+ * an exclusion index out of range, a self entry or an entry (i,j) without its mirror (j,i),
+ * rc <= 0, or (beta*rc)^2 > 12. */
 int nb_init(const nb_params* p, nb_ctx** out);
 
 /* (a1) Coordinate staging.  x [dev] natoms*3 fp32, q [dev] natoms,
@@ -103,7 +109,10 @@ int nb_put_atoms_host(nb_ctx*, const float* x, const float* q, const int32_t* ty
 /* (a2)-(a5) Gridding into clusters (L129-L131), bounding-box pair search with interaction
  * masks (L131-L133, L187), exclusion masks (L135), list splitting/sorting (L199-L201).
  * Sets inner list := outer list.  NB_ERR_CUTOFF unless rc <= rlist_outer <= min(L)/2;
- * NB_ERR_BOX for a non-positive box.  Synchronises (reads list sizes). */
+ * NB_ERR_BOX for a non-positive box; NB_ERR_ARG if an atom type is outside [0, ntypes).
+ * All of it runs on the device; list buffers are sized from the previous search with head-room and
+ * the stream is synchronised ONCE, at the end, to read the list sizes back (the first search of a
+ * context, and a search whose list outgrew the buffers, synchronise stage by stage). */
 int nb_search(nb_ctx*, float rlist_outer);
 
 /* (a6) Dynamic pruning (L187-L193): recomputes the inner interaction mask of rolling part
@@ -111,6 +120,14 @@ int nb_search(nb_ctx*, float rlist_outer);
  * iff some atom pair is closer than rlist_inner.  Needs rc <= rlist_inner <= rlist_outer,
  * 0 <= part < nparts; nparts = 1 prunes everything. */
 int nb_prune(nb_ctx*, float rlist_inner, int part, int nparts);
+/* Same prune, scheduled "between force computations" so that it overlaps other work:
+ * the kernel runs on a second stream of the library, concurrently with whatever the caller enqueues
+ * next (the nb_forces of the same step), reads the coordinates of the last nb_put_atoms, and writes
+ * the part into a second copy of the inner list.  The part switches to the new list at the NEXT
+ * nb_put_atoms (which waits for the prune): the nb_forces calls before it still use the previous
+ * list of that part, those after it the new one.  The list therefore serves one step longer than
+ * with nb_prune: choose rlist_inner - rc for nparts + 1 steps of motion.  nparts <= 32. */
+int nb_prune_overlapped(nb_ctx*, float rlist_inner, int part, int nparts);
 
 /* (a7)-(a8) Forces over the inner list.  f [dev] natoms*3 fp32 in the caller's atom order,
  * overwritten.  energies [dev] double[2] = {E_lj, E_coul} (kJ/mol) or NULL for the force-only
@@ -119,6 +136,13 @@ int nb_prune(nb_ctx*, float rlist_inner, int part, int nparts);
 int nb_forces(nb_ctx*, float* f, double* energies, double* virial);
 /* Same with host pointers; synchronises before returning. */
 int nb_forces_host(nb_ctx*, float* f, double* energies, double* virial);
+/* First use of a freshly searched list ("Initial pruning is done the first time the
+ * list is processed by a special version of the kernel (using warp collectives for low extra cost),
+ * and the pruned list is reused for consecutive MD steps"): ONE kernel walks the OUTER list, computes
+ * the forces (and energies / virial, as nb_forces) and writes the whole inner list for rlist_inner from
+ * the distances it evaluates anyway.  Equivalent to nb_prune(rlist_inner, 0, 1) followed by nb_forces:
+ * same inner list bit for bit, forces equal up to summation order.  Same argument rules as nb_prune / nb_forces. */
+int nb_forces_prune(nb_ctx*, float rlist_inner, float* f, double* energies, double* virial);
 
 void nb_free(nb_ctx*);
 const char* nb_last_error(const nb_ctx*);
@@ -141,9 +165,10 @@ int nb_list_dump(nb_ctx*, int which, int32_t* ci, int32_t* cj, int32_t* shift, u
  * HOST arrays of *n entries, any may be NULL; call with all NULL to get *n.  Entry k: i-cluster ci[k],
  * shift[k] (as in nb_list_dump), kind[k] = 0: entry[k] is a half j-cluster index 2*cj + half (atoms
  * 4*entry .. 4*entry+3, a cluster pair without a mask, kept at half-cluster granularity);
- * kind[k] = 1: entry[k] is a whole j-cluster cj whose pair with ci carries a mask.  Padding (dummy)
- * entries are left out. */
-int nb_inner_dump(nb_ctx*, int64_t* n, int32_t* ci, int32_t* entry, int32_t* shift, int32_t* kind);
+ * kind[k] = 1: entry[k] is a whole j-cluster cj whose pair with ci carries a mask; part[k]: rolling
+ * part of the entry under the nparts of the last prune call.  Padding (dummy) entries are left out.
+ * An overlapped prune still in flight is joined first. */
+int nb_inner_dump(nb_ctx*, int64_t* n, int32_t* ci, int32_t* entry, int32_t* shift, int32_t* kind, int32_t* part);
 int nb_get_stats(nb_ctx*, nb_stats* out);
 /* Measures the device's FP32 FMA issue peak with a register-resident FFMA chain kernel
  * (MEASURED_PEAKS.json has no FP32 entry).  Returns lane-FMA/s in *fma_per_s. */
@@ -165,9 +190,10 @@ enum { NB_T_PUT = 0,      /* (a1) nb_put_atoms: copies + cluster-order refresh *
        NB_T_SEARCH = 2,   /* (a3)+(a5) pair search count/fill passes, unit table upload */
        NB_T_MASKS = 3,    /* (a4) exclusion masks, (a5) compact inner list set-up and its launch order (+ list statistics) */
        NB_T_PRUNE = 4,    /* (a6) prune kernel */
-       NB_T_FORCE = 5,    /* (a7) force kernel alone */
+       NB_T_FORCE = 5,    /* (a7) force kernel alone, force-only flavour */
        NB_T_REDUCE = 6,   /* (a8) gather to caller order, virial/energy finalisation */
-       NB_T_NKINDS = 7 };
+       NB_T_FORCE_ENERGY = 7,   /* (a7) force kernel alone, force + energy (+ virial) flavour */
+       NB_T_NKINDS = 8 };
 /* on != 0: record an event pair around every stage from now on.  Off by default. */
 int nb_timing_enable(nb_ctx*, int on);
 /* Restricts the timing to the stages whose bit (1u << NB_T_*) is set in stage_mask (default: all).

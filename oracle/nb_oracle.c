@@ -490,9 +490,10 @@ long long oracle_lists(int nclusters, int C, const int32_t* atom_of_slot, const 
         for (int ci = 0; ci < nclusters; ci++) {
             if (nv[ci] == 0) continue;
             long long k = pass ? cnt[ci] : 0;
-            for (int cj = 0; cj < nclusters; cj++) {
+            /* first OR second cluster in [c_begin, c_end): all cj for a ci inside the range, else the cj inside it */
+            const int ci_in = (ci >= c_begin && ci < c_end);
+            for (int cj = ci_in ? 0 : c_begin; cj < (ci_in ? nclusters : (c_end < nclusters ? c_end : nclusters)); cj++) {
                 if (nv[cj] == 0) continue;
-                if (!((ci >= c_begin && ci < c_end) || (cj >= c_begin && cj < c_end))) continue;
                 for (int sx = -1; sx <= 1; sx++)
                     for (int sy = -1; sy <= 1; sy++)
                         for (int sz = -1; sz <= 1; sz++) {
@@ -554,9 +555,10 @@ long long oracle_half_lists(int nclusters, int C, const int32_t* atom_of_slot, c
         for (int ci = 0; ci < nclusters; ci++) {
             if (nv[ci] == 0) continue;
             long long k = pass ? cnt[ci] : 0;
-            for (int cj = 0; cj < nclusters; cj++) {
+            /* first OR second cluster in [c_begin, c_end): all cj for a ci inside the range, else the cj inside it */
+            const int ci_in = (ci >= c_begin && ci < c_end);
+            for (int cj = ci_in ? 0 : c_begin; cj < (ci_in ? nclusters : (c_end < nclusters ? c_end : nclusters)); cj++) {
                 if (nv[cj] == 0) continue;
-                if (!((ci >= c_begin && ci < c_end) || (cj >= c_begin && cj < c_end))) continue;
                 for (int sx = -1; sx <= 1; sx++)
                     for (int sy = -1; sy <= 1; sy++)
                         for (int sz = -1; sz <= 1; sz++) {

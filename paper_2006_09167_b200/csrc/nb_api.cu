@@ -22,6 +22,22 @@ int nb_fail(nb_ctx* c, int code, const char* fmt, ...)
 
 static bool finite_pos(float v) { return v > 0.f && isfinite(v); }
 
+// Every entry point runs on the context's device whatever device is current in the calling thread,
+// and leaves the caller's current device as it found it.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const nb_ctx* c)
+    {
+        if (!c) return;
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != c->prm.device) switched = cudaSetDevice(c->prm.device) == cudaSuccess;
+    }
+    ~DeviceGuard()
+    {
+        if (switched) cudaSetDevice(prev);
+    }
+};
+
 extern "C" int nb_init(const nb_params* p, nb_ctx** out)
 {
     if (!p || !out) return NB_ERR_ARG;
@@ -29,7 +45,10 @@ extern "C" int nb_init(const nb_params* p, nb_ctx** out)
     if (p->natoms <= 0 || p->ntypes <= 0 || p->ntypes > NB_MAX_TYPES || !p->lj_c6c12 || !finite_pos(p->rc)) return NB_ERR_ARG;
     if (p->coulomb != NB_COUL_EWALD && p->coulomb != NB_COUL_RF && p->coulomb != NB_COUL_NONE) return NB_ERR_ARG;
     if (p->excl_off && p->excl_off[p->natoms] > 0 && !p->excl_idx) return NB_ERR_ARG;
+    int prev_device = -1;
+    cudaGetDevice(&prev_device);
     if (cudaSetDevice(p->device) != cudaSuccess) return NB_ERR_CUDA;
+    struct Restore { int d; ~Restore() { if (d >= 0) cudaSetDevice(d); } } restore{prev_device};
     nb_ctx* c = new (std::nothrow) nb_ctx();
     if (!c) return NB_ERR_NOMEM;
     c->err[0] = 0;
@@ -63,14 +82,19 @@ extern "C" int nb_init(const nb_params* p, nb_ctx** out)
     NbConst& K = c->kc;
     memset(&K, 0, sizeof(K));
     K.rc2 = p->rc * p->rc;
+    if (p->rc_vdw < 0.f || p->rc_vdw > p->rc || !isfinite(p->rc_vdw))
+        return nb_fail(c, NB_ERR_ARG, "rc_vdw = %g must be 0 (= rc) or in (0, rc = %g]", p->rc_vdw, p->rc);
+    const double rcv = p->rc_vdw > 0.f ? (double)p->rc_vdw : rc;   // twin cut-offs: LJ below rc_vdw only
+    c->twin = p->rc_vdw > 0.f && p->rc_vdw < p->rc;
+    K.rcv2 = c->twin ? p->rc_vdw * p->rc_vdw : K.rc2;
     K.epsfac = (float)epsfac;
     K.beta = (float)beta; K.beta2 = (float)(beta * beta); K.beta3 = (float)(beta * beta * beta);
     K.ewald_shift = (p->coulomb == NB_COUL_EWALD && p->coul_modifier == NB_MOD_POTSHIFT) ? (float)(erfc(beta * rc) / rc) : 0.f;
     double krf = (p->eps_rf <= 0.f || isinf(p->eps_rf)) ? 1.0 / (2.0 * rc * rc * rc)
                                                          : ((double)p->eps_rf - 1.0) / ((2.0 * p->eps_rf + 1.0) * rc * rc * rc);   // reading A6
     K.krf = (float)krf; K.two_krf = (float)(2.0 * krf); K.crf = (float)(1.0 / rc + krf * rc * rc);
-    K.lj_sh6 = p->lj_modifier == NB_MOD_POTSHIFT ? (float)pow(rc, -6.0) : 0.f;
-    K.lj_sh12 = p->lj_modifier == NB_MOD_POTSHIFT ? (float)pow(rc, -12.0) : 0.f;
+    K.lj_sh6 = p->lj_modifier == NB_MOD_POTSHIFT ? (float)pow(rcv, -6.0) : 0.f;
+    K.lj_sh12 = p->lj_modifier == NB_MOD_POTSHIFT ? (float)pow(rcv, -12.0) : 0.f;
     K.ntypes1 = p->ntypes + 1;
     c->beta = (float)beta;
     c->beta_d = beta;
@@ -97,6 +121,14 @@ extern "C" int nb_init(const nb_params* p, nb_ctx** out)
             if (p->excl_idx[k] < 0 || p->excl_idx[k] >= n || p->excl_idx[k] == i)
                 return nb_fail(c, NB_ERR_ARG, "exclusion %d of atom %d is out of range or a self entry", k, i);
     }
+    // symmetric: the mask kernel walks each excluded pair from its lower index only
+    for (int i = 0; i < n; i++)
+        for (int k = eo[i]; k < eo[i + 1]; k++) {
+            const int j = p->excl_idx[k];
+            bool mirrored = false;
+            for (int m = eo[j]; m < eo[j + 1] && !mirrored; m++) mirrored = p->excl_idx[m] == i;
+            if (!mirrored) return nb_fail(c, NB_ERR_ARG, "exclusion (%d,%d) has no mirror entry (%d,%d)", i, j, j, i);
+        }
     NB_CUDA(c, c->excl_off.ensure(n + 1, st));
     NB_CUDA(c, c->excl_idx.ensure(c->nexcl + 1, st));
     NB_CUDA(c, cudaMemcpyAsync(c->excl_off.p, eo, sizeof(int32_t) * (n + 1), cudaMemcpyHostToDevice, st));
@@ -104,6 +136,10 @@ extern "C" int nb_init(const nb_params* p, nb_ctx** out)
     NB_CUDA(c, c->x.ensure((size_t)3 * n, st));
     NB_CUDA(c, c->q.ensure(n, st));
     NB_CUDA(c, c->type.ensure(n, st));
+    NB_CUDA(c, cudaMalloc((void**)&c->tot_dev, sizeof(NbTotals)));
+    NB_CUDA(c, cudaMallocHost((void**)&c->tot_host, sizeof(NbTotals)));
+    memset(c->tot_host, 0, sizeof(NbTotals));
+    NB_CUDA(c, cudaMemsetAsync(c->tot_dev, 0, sizeof(NbTotals), st));
     NB_CUDA(c, cudaStreamSynchronize(st));   // host staging vectors go out of scope
     return NB_OK;
 }
@@ -111,6 +147,7 @@ extern "C" int nb_init(const nb_params* p, nb_ctx** out)
 static int put_atoms_common(nb_ctx* c, const float* x, const float* q, const int32_t* type, const float box[3], cudaMemcpyKind kind)
 {
     if (!c) return NB_ERR_ARG;
+    DeviceGuard guard(c);
     if (!x || !box) return nb_fail(c, NB_ERR_ARG, "nb_put_atoms: null argument");
     if ((!q || !type) && !c->have_atoms)
         return nb_fail(c, NB_ERR_ARG, "nb_put_atoms: q and type may be NULL only after a call that passed them");
@@ -118,6 +155,9 @@ static int put_atoms_common(nb_ctx* c, const float* x, const float* q, const int
         if (!finite_pos(box[k])) return nb_fail(c, NB_ERR_BOX, "box[%d] = %g is not positive", k, box[k]);
     cudaStream_t st = c->stream;
     const int n = c->natoms;
+    // an overlapped prune reads the coordinates this call overwrites: join it; its part flips to the new list here
+    int rcp = nbi_commit_pending(c);
+    if (rcp != NB_OK) return rcp;
     NbStageTimer tm(c, NB_T_PUT);
     const bool device = kind == cudaMemcpyDeviceToDevice;
     if (!device) {
@@ -154,6 +194,7 @@ extern "C" int nb_put_atoms_host(nb_ctx* c, const float* x, const float* q, cons
 extern "C" int nb_search(nb_ctx* c, float rlist_outer)
 {
     if (!c) return NB_ERR_ARG;
+    DeviceGuard guard(c);
     if (!c->have_atoms) return nb_fail(c, NB_ERR_STATE, "nb_search before nb_put_atoms");
     const float minL = fminf(c->box[0], fminf(c->box[1], c->box[2]));
     if (!(rlist_outer >= c->prm.rc) || !(rlist_outer <= 0.5f * minL))
@@ -162,28 +203,57 @@ extern "C" int nb_search(nb_ctx* c, float rlist_outer)
     return nbi_search(c, rlist_outer);
 }
 
-extern "C" int nb_prune(nb_ctx* c, float rlist_inner, int part, int nparts)
+static int prune_checks(nb_ctx* c, float rlist_inner, int part, int nparts)
 {
-    if (!c) return NB_ERR_ARG;
     if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "nb_prune without a valid list (call nb_search)");
     if (nparts < 1 || part < 0 || part >= nparts) return nb_fail(c, NB_ERR_ARG, "nb_prune: part %d of %d", part, nparts);
     if (!(rlist_inner >= c->prm.rc) || !(rlist_inner <= c->rlist_outer))
         return nb_fail(c, NB_ERR_CUTOFF, "rlist_inner = %g must satisfy rc = %g <= rlist_inner <= rlist_outer = %g", rlist_inner, c->prm.rc, c->rlist_outer);
-    return nbi_prune(c, rlist_inner, part, nparts);
+    return NB_OK;
+}
+
+extern "C" int nb_prune(nb_ctx* c, float rlist_inner, int part, int nparts)
+{
+    if (!c) return NB_ERR_ARG;
+    DeviceGuard guard(c);
+    int rc = prune_checks(c, rlist_inner, part, nparts);
+    return rc != NB_OK ? rc : nbi_prune(c, rlist_inner, part, nparts);
+}
+
+extern "C" int nb_prune_overlapped(nb_ctx* c, float rlist_inner, int part, int nparts)
+{
+    if (!c) return NB_ERR_ARG;
+    DeviceGuard guard(c);
+    int rc = prune_checks(c, rlist_inner, part, nparts);
+    return rc != NB_OK ? rc : nbi_prune_overlapped(c, rlist_inner, part, nparts);
 }
 
 extern "C" int nb_forces(nb_ctx* c, float* f, double* energies, double* virial)
 {
     if (!c) return NB_ERR_ARG;
+    DeviceGuard guard(c);
     if (!f) return nb_fail(c, NB_ERR_ARG, "nb_forces: f is null");
     if (virial && !energies) return nb_fail(c, NB_ERR_ARG, "nb_forces: virial needs energies (same kernel flavour)");
     if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "nb_forces without a valid list (call nb_search)");
     return nbi_forces(c, f, energies, virial);
 }
 
+extern "C" int nb_forces_prune(nb_ctx* c, float rlist_inner, float* f, double* energies, double* virial)
+{
+    if (!c) return NB_ERR_ARG;
+    DeviceGuard guard(c);
+    if (!f) return nb_fail(c, NB_ERR_ARG, "nb_forces_prune: f is null");
+    if (virial && !energies) return nb_fail(c, NB_ERR_ARG, "nb_forces_prune: virial needs energies (same kernel flavour)");
+    int rc = prune_checks(c, rlist_inner, 0, 1);
+    if (rc != NB_OK) return rc;
+    if ((rc = nbi_commit_pending(c)) != NB_OK) return rc;
+    return nbi_forces(c, f, energies, virial, rlist_inner);
+}
+
 extern "C" int nb_forces_host(nb_ctx* c, float* f, double* energies, double* virial)
 {
     if (!c) return NB_ERR_ARG;
+    DeviceGuard guard(c);
     if (!f) return nb_fail(c, NB_ERR_ARG, "nb_forces_host: f is null");
     cudaStream_t st = c->stream;
     NB_CUDA(c, c->stage_f.ensure((size_t)3 * c->natoms, st));
@@ -200,21 +270,31 @@ extern "C" int nb_forces_host(nb_ctx* c, float* f, double* energies, double* vir
 extern "C" void nb_free(nb_ctx* c)
 {
     if (!c) return;
+    DeviceGuard guard(c);
+    if (c->side_stream) cudaStreamSynchronize(c->side_stream);
     cudaStreamSynchronize(c->stream);
+    if (c->side_stream) cudaStreamDestroy(c->side_stream);
+    if (c->ev_main) cudaEventDestroy(c->ev_main);
+    if (c->ev_side) cudaEventDestroy(c->ev_side);
+    if (c->tot_dev) cudaFree(c->tot_dev);
+    if (c->tot_host) cudaFreeHost(c->tot_host);
     for (auto& r : c->tim_open) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
     for (auto e : c->tim_pool) cudaEventDestroy(e);
     c->x.release(); c->q.release(); c->type.release();
     c->stage_x.release(); c->stage_q.release(); c->stage_f.release(); c->stage_type.release(); c->stage_ev.release();
     c->excl_off.release(); c->excl_idx.release(); c->ljtab.release();
     c->col_count.release(); c->col_atom_off.release(); c->col_sc_off.release(); c->atom_col.release();
-    c->atom_rank.release(); c->col_atoms.release(); c->grid_totals.release(); c->image.release(); c->xw_atom.release();
+    c->atom_rank.release(); c->col_atoms.release(); c->image.release(); c->xw_atom.release();
     c->xq.release(); c->type_slot.release(); c->atom_of_slot.release(); c->slot_of_atom.release();
     c->bb_lo.release(); c->bb_hi.release(); c->sbb_lo.release(); c->sbb_hi.release(); c->f4.release();
     c->ent_count.release(); c->ent_jbegin.release(); c->jl.release(); c->imask_outer.release();
     c->plane_outer.release(); c->plane_inner.release(); c->plane_excl.release(); c->batch_ent.release(); c->scan_tmp.release();
     c->scan_blk.release(); c->excl_masks.release(); c->counters.release(); c->units_canon.release();
-    c->units_sorted.release(); c->fshift.release(); c->unit_order.release(); for (auto& po : c->prune_orders) po.d.release();
-    c->il_off.release(); c->ilm_off.release(); c->seg.release(); c->unit_pos.release(); c->seg_pos.release(); c->seg_ci.release(); c->il.release(); c->ilm.release(); c->ol.release(); c->ol_cnt.release();
+    c->fshift.release(); c->unit_nsplit.release(); c->unit_off.release(); c->sort_hist.release(); c->seg_len.release();
+    for (auto& po : c->prune_orders) po.d.release();
+    c->il_off.release(); c->ilm_off.release(); c->seg_of_s0.release(); c->segd.release(); c->ol_cnt.release();
+    c->olu.release(); c->olm.release(); c->ljrow.release();
+    for (int b = 0; b < 2; b++) { c->seg_cnt[b].release(); c->il[b].release(); c->ilm[b].release(); }
     delete c;
 }
 
@@ -222,6 +302,7 @@ extern "C" const char* nb_last_error(const nb_ctx* c) { return c ? c->err : "nul
 
 extern "C" int nb_get_layout(nb_ctx* c, int32_t* cluster_size, int32_t* nclusters, int32_t* nsuper, int32_t* nslots)
 {
+    DeviceGuard guard(c);
     if (!c) return NB_ERR_ARG;
     if (!c->have_grid) return nb_fail(c, NB_ERR_STATE, "no grid yet (call nb_search)");
     if (cluster_size) *cluster_size = NB_C;
@@ -233,6 +314,7 @@ extern "C" int nb_get_layout(nb_ctx* c, int32_t* cluster_size, int32_t* ncluster
 
 extern "C" int nb_get_slots(nb_ctx* c, int32_t* atom_of_slot, float* xq)
 {
+    DeviceGuard guard(c);
     if (!c) return NB_ERR_ARG;
     if (!c->have_grid) return nb_fail(c, NB_ERR_STATE, "no grid yet (call nb_search)");
     if (atom_of_slot) NB_CUDA(c, cudaMemcpyAsync(atom_of_slot, c->atom_of_slot.p, sizeof(int32_t) * c->nslots, cudaMemcpyDeviceToDevice, c->stream));
@@ -243,6 +325,7 @@ extern "C" int nb_get_slots(nb_ctx* c, int32_t* atom_of_slot, float* xq)
 
 extern "C" int nb_list_count(nb_ctx* c, int which, int64_t* n)
 {
+    DeviceGuard guard(c);
     if (!c || !n) return NB_ERR_ARG;
     if (which != 0 && which != 1) return nb_fail(c, NB_ERR_ARG, "which must be 0 (outer) or 1 (inner)");
     if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "no list yet (call nb_search)");
@@ -251,6 +334,7 @@ extern "C" int nb_list_count(nb_ctx* c, int which, int64_t* n)
 
 extern "C" int nb_list_dump(nb_ctx* c, int which, int32_t* ci, int32_t* cj, int32_t* shift, uint64_t* pairmask, int32_t* part)
 {
+    DeviceGuard guard(c);
     if (!c) return NB_ERR_ARG;
     if (which != 0 && which != 1) return nb_fail(c, NB_ERR_ARG, "which must be 0 (outer) or 1 (inner)");
     if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "no list yet (call nb_search)");
@@ -259,14 +343,18 @@ extern "C" int nb_list_dump(nb_ctx* c, int which, int32_t* ci, int32_t* cj, int3
 
 extern "C" int nb_get_stats(nb_ctx* c, nb_stats* out)
 {
+    DeviceGuard guard(c);
     if (!c || !out) return NB_ERR_ARG;
     NB_CUDA(c, cudaStreamSynchronize(c->stream));
     if (c->have_list) {
         int64_t n = 0;
-        int rc = nbi_list_count(c, 1, &n);
+        int rc = nbi_list_stats(c);
         if (rc != NB_OK) return rc;
+        if ((rc = nbi_list_count(c, 1, &n)) != NB_OK) return rc;
         c->st.n_pairs_inner = n;
-        c->st.slots_last_forces = c->st.force_count ? n * 64 : 0;
+        int64_t slots = 0;
+        if ((rc = nbi_count_slots(c, &slots)) != NB_OK) return rc;
+        c->st.slots_last_forces = c->st.force_count ? slots : 0;
     }
     *out = c->st;
     return NB_OK;
@@ -274,12 +362,14 @@ extern "C" int nb_get_stats(nb_ctx* c, nb_stats* out)
 
 extern "C" int nb_measure_fp32_peak(nb_ctx* c, double* fma_per_s)
 {
+    DeviceGuard guard(c);
     if (!c || !fma_per_s) return NB_ERR_ARG;
     return nbi_measure_fp32_peak(c, fma_per_s);
 }
 
 extern "C" int nb_count_pairs(nb_ctx* c, int64_t* n_interacting, int64_t* n_excluded)
 {
+    DeviceGuard guard(c);
     if (!c) return NB_ERR_ARG;
     if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "no list yet (call nb_search)");
     return nbi_count_pairs(c, n_interacting, n_excluded);
@@ -287,16 +377,18 @@ extern "C" int nb_count_pairs(nb_ctx* c, int64_t* n_interacting, int64_t* n_excl
 
 extern "C" int nb_count_slots(nb_ctx* c, int64_t* slots)
 {
+    DeviceGuard guard(c);
     if (!c || !slots) return NB_ERR_ARG;
     if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "no list yet (call nb_search)");
     return nbi_count_slots(c, slots);
 }
 
-extern "C" int nb_inner_dump(nb_ctx* c, int64_t* n, int32_t* ci, int32_t* entry, int32_t* shift, int32_t* kind)
+extern "C" int nb_inner_dump(nb_ctx* c, int64_t* n, int32_t* ci, int32_t* entry, int32_t* shift, int32_t* kind, int32_t* part)
 {
+    DeviceGuard guard(c);
     if (!c || !n) return NB_ERR_ARG;
     if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "no list yet (call nb_search)");
-    return nbi_inner_dump(c, n, ci, entry, shift, kind);
+    return nbi_inner_dump(c, n, ci, entry, shift, kind, part);
 }
 
 extern "C" int nb_timing_enable(nb_ctx* c, int on)
@@ -315,6 +407,7 @@ extern "C" int nb_timing_stages(nb_ctx* c, unsigned stage_mask)
 
 extern "C" int nb_timing_read(nb_ctx* c, double* ms, int64_t* count, int reset)
 {
+    DeviceGuard guard(c);
     if (!c) return NB_ERR_ARG;
     NB_CUDA(c, cudaStreamSynchronize(c->stream));
     for (auto& r : c->tim_open) {

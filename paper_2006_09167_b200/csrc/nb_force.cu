@@ -25,17 +25,28 @@
 namespace {
 
 struct ForceArgs {
-    const int4* units;          // work units {entry slot, batch begin, batch end, sci}: launch order (k_force), canonical (k_count_pairs)
+    const int4* units;          // work units {entry slot, batch begin, batch end, sci}, canonical order (k_count_pairs)
     const int2* jl;
     const uint32_t* plane;
     const float4* xq;
     const int* type_slot;
-    const float2* ljtab;
+    const float4* ljrow;        // paired LJ rows per i-cluster (k_ljrows)
     const unsigned long long* masks;
-    const int4* seg;            // compact inner list, see nb_internal.h
-    const int2* seg_ci;
-    const int* il;
-    const int2* ilm;
+    const int4* segd;           // compact inner list, see nb_internal.h
+    const int2* seg_cnt[2];
+    const int* il[2];
+    const int2* ilm[2];
+    unsigned bufmask;           // which inner buffer each rolling part lives in (nb_prune_overlapped), 0 = all in buffer 0
+    int nparts, nunits;
+    // the fused first prune (k_force<..., PRUNE = true>): outer list in, inner list (buffer 0) out
+    const int2* ol_cnt;
+    const int* olu;
+    const int2* olm;
+    int32_t* il_w;
+    int2* ilm_w;
+    int2* seg_cnt_w;
+    float rl2;                  // fl32(rlist_inner^2), reading A12
+    int cj_dummy;
     float4* f4;
     double* fshift;     // [27*3]
     double* energies;   // [2]
@@ -101,19 +112,28 @@ struct IAtoms {
 // table, stride `ljs` float4 between i-atom pairs) against the 8 i atoms, two at a time.
 // MASKED: cbyte/mbyte carry the lane's 8 "counted"/"interacts" bits (reading A4: an excluded pair
 // keeps the Ewald/RF correction, loses LJ and the 1/r part).
+// TWIN: twin cut-offs, LJ only below rc_vdw <= rc.
+// PRUNE: the fused first prune; returns whether some counted pair of this lane's j atom is
+// within rlist_inner, decided on the same r^2 (the exact A12 arithmetic: I holds fmaf(s, L, x_a), and
+// x_a' + (-x_b) = x_a' - x_b, fma2(dz,dz, fma2(dy,dy, dx*dx)) round like the oracle's scalar forms).
 // Returns the NEGATED j force in (fjx, fjy, fjz) pairs (sum the halves and negate).
-template <int COUL, bool ENERGY, bool MASKED>
-__device__ __forceinline__ void pair_step(const NbConst& K, const float4* __restrict__ ljj, const int ljs, const IAtoms& I,
+template <int COUL, bool ENERGY, bool MASKED, bool TWIN, bool PRUNE>
+__device__ __forceinline__ bool pair_step(const NbConst& K, const float4* __restrict__ ljj, const int ljs, const IAtoms& I,
                                           float2 (&fix)[4], float2 (&fiy)[4], float2 (&fiz)[4], float& elj, float& ecoul,
                                           const float4 xj, unsigned cbyte, unsigned mbyte, float2& fjx, float2& fjy,
-                                          float2& fjz, const float2 p3)
+                                          float2& fjz, const float2 p3, const float rl2)
 {
     const float2 nxj = f2(-xj.x), nyj = f2(-xj.y), nzj = f2(-xj.z), qj = f2(xj.w);
     fjx = f2(0.f); fjy = f2(0.f); fjz = f2(0.f);
+    bool found = false;
 #pragma unroll
     for (int p = 0; p < 4; p++) {
         const float2 dx = add2(I.x[p], nxj), dy = add2(I.y[p], nyj), dz = add2(I.z[p], nzj);
         const float2 r2u = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+        if (PRUNE) {
+            if (MASKED) found = found || (r2u.x < rl2 && ((cbyte >> (2 * p)) & 1u)) || (r2u.y < rl2 && ((cbyte >> (2 * p + 1)) & 1u));
+            else found = found || r2u.x < rl2 || r2u.y < rl2;
+        }
         // A7: interact iff r^2 < rc^2 (strict), applied with compare + select on the ALU pipe, which
         // has slack (the FP32 pipe is the bound; a saturating-FMA 0/1 factor there was measured 1 %
         // slower).  MASKED steps also clamp r^2 so that self pairs stay finite; unmasked steps have no
@@ -133,7 +153,9 @@ __device__ __forceinline__ void pair_step(const NbConst& K, const float4* __rest
         const float4 c = ljj[p * ljs];                        // (-6 c6_a, -6 c6_b, 12 c12_a, 12 c12_b)
         const float2 nc6 = f2(c.x, c.y), c12 = f2(c.z, c.w);
         const float2 rinv6 = mul2(mul2(rinv2, rinv2), rinv2);
-        const float2 flj = mul2(fma2(c12, rinv6, nc6), rinv6);
+        float2 flj = mul2(fma2(c12, rinv6, nc6), rinv6);
+        const bool v0 = !TWIN || r2u.x < K.rcv2, v1 = !TWIN || r2u.y < K.rcv2;   // LJ cut-off (twin cut-offs)
+        if (TWIN) flj = f2(v0 ? flj.x : 0.f, v1 ? flj.y : 0.f);
         const float2 qq = mul2(I.q[p], qj);                   // epsfac folded into the i charge
         float2 t1 = COUL == NB_COUL_NONE ? flj : fma2(qq, rinv, flj);   // (F_lj + A/r) r
         float2 mf = f2(1.f);
@@ -173,41 +195,55 @@ __device__ __forceinline__ void pair_step(const NbConst& K, const float4* __rest
                 vc = f2(0.f);
             }
             const float2 vl = mul2(mf, vlj);
-            elj += (w0 ? vl.x : 0.f) + (w1 ? vl.y : 0.f);
+            elj += (w0 && v0 ? vl.x : 0.f) + (w1 && v1 ? vl.y : 0.f);
             ecoul += (w0 ? vc.x : 0.f) + (w1 ? vc.y : 0.f);
         }
     }
+    return found;
 }
 
-template <int COUL, bool ENERGY>
-__global__ void __launch_bounds__(32, 16) k_force(ForceArgs A)
+// PRUNE = false: the inner list (half j-clusters, 8 per step; masked cluster pairs, 4 per step).
+// PRUNE = true: the fused first prune of a freshly searched list: the same kernel walks
+// the OUTER list (whole j-clusters, 4 per step), evaluates the forces, and writes the inner list from
+// the r^2 values it has anyway -- one ballot per step, as in nb_prune.cu's kernel.
+template <int COUL, bool ENERGY, bool TWIN, bool PRUNE>
+__global__ void __launch_bounds__(32, PRUNE ? 8 : 16) k_force(ForceArgs A)
 {
     // Paired LJ table of this block's i-cluster: s_ljp[p*nt1 + tj] = (-6c6, -6c6', 12c12, 12c12') of the
     // i atoms 2p, 2p+1 against j type tj: one LDS.128 feeds both packed operands.
     extern __shared__ float4 s_ljp[];
     const NbConst& K = A.kc;
     const int lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7;
-    const int4 sg = A.seg[blockIdx.x];
-    const int2 sc = A.seg_ci[blockIdx.x];
-    const int ci = sc.x, sid = sc.y, warp = ci & 7;
+    const int4 sd = A.segd[blockIdx.x];
+    const int buf = PRUNE ? 0 : nb_seg_buf(sd.w, A.bufmask, A.nparts, A.nunits);
+    // PRUNE: outer counts {cluster pairs without a mask, with a mask}; else inner {half entries, masked pairs}
+    const int2 cnt = PRUNE ? A.ol_cnt[blockIdx.x] : A.seg_cnt[buf][blockIdx.x];
+    const int ci = sd.z & 0x3ffffff, sid = sd.z >> 26, warp = ci & 7;
     const int nt1 = K.ntypes1;
     float4* ljw = s_ljp;
-    for (int i = lane; i < 4 * nt1; i += 32) {
-        const int p = i / nt1, tj = i - p * nt1;
-        const int ta = A.type_slot[ci * 8 + 2 * p], tb = A.type_slot[ci * 8 + 2 * p + 1];
-        const float2 ca = A.ljtab[ta * nt1 + tj], cb = A.ljtab[tb * nt1 + tj];
-        ljw[i] = make_float4(-ca.x, -cb.x, ca.y, cb.y);
-    }
-    const int2 cnt = make_int2(sg.z, sg.w);
-    const int* __restrict__ il = A.il + sg.x;
-    const int2* __restrict__ ilm = A.ilm + sg.y;
-    const int ns = cnt.x >> 3;             // unmasked steps: 8 half-clusters (4 atoms each) per step
-    const int g8 = lane >> 2, k4 = lane & 3;   // lane -> (half-cluster of the step, atom in it)
+    // the rows were paired at search time (types do not change between searches): one coalesced load
+    for (int i = lane; i < 4 * nt1; i += 32) ljw[i] = A.ljrow[(size_t)ci * 4 * nt1 + i];
+    const int* __restrict__ il = (PRUNE ? A.olu : A.il[buf]) + sd.x;
+    const int2* __restrict__ ilm = (PRUNE ? A.olm : A.ilm[buf]) + sd.y;
+    int32_t* il_w = PRUNE ? A.il_w + sd.x : nullptr;
+    int2* ilm_w = PRUNE ? A.ilm_w + sd.y : nullptr;
+    int nu_w = 0, nm_w = 0;
+    // unmasked steps: 8 half-clusters (4 atoms each) per step; PRUNE: 4 whole clusters per step
+    const int ns = PRUNE ? (cnt.x + 3) >> 2 : cnt.x >> 3;
+    const int g8 = PRUNE ? g : lane >> 2, k4 = PRUNE ? k : lane & 3;   // lane -> (entry of the step, atom in it)
+    constexpr int EPS = PRUNE ? 4 : 8, APE = PRUNE ? 8 : 4;          // entries per step, atoms per entry
+    // PRUNE: the last step may be partly filled; its spare lanes take a dummy cluster (far from everything:
+    // no force, no survivor; nb_grid.cu)
+    auto entry = [&](int s) {
+        if (!PRUNE) return il[EPS * s + g8];
+        const int idx = EPS * s + g8, v = il[min(idx, max(cnt.x - 1, 0))];
+        return idx < cnt.x ? v : A.cj_dummy;
+    };
     // first list entries of both loops are requested before anything else is waited for
     int cj = 0, cj_n = 0;
     if (ns > 0) {
-        cj = il[g8] * 4 + k4;              // unmasked path: cj* hold this lane's j SLOT (4 * half-cluster + atom)
-        cj_n = il[8 * min(1, ns - 1) + g8] * 4 + k4;
+        cj = entry(0) * APE + k4;              // unmasked path: cj* hold this lane's j SLOT
+        cj_n = entry(min(1, ns - 1)) * APE + k4;
     }
     int sx, sy, sz;
     nb_shift_vec(sid, sx, sy, sz);
@@ -233,8 +269,8 @@ __global__ void __launch_bounds__(32, 16) k_force(ForceArgs A)
     }
     __syncwarp();
 
-    // Cluster pairs with exclusion / self / diagonal masks, and possibly the segment's tail (ref 0 =
-    // all ones).  (Software-pipelining this loop like the unmasked one was measured slower.)
+    // Cluster pairs with exclusion / self / diagonal masks.  (Software-pipelining this loop like the
+    // unmasked one was measured slower.)
     for (int s = 0; s < cnt.y; s += 4) {
         const bool valid = s + g < cnt.y;
         const int2 ce = valid ? ilm[s + g] : make_int2(ci, 0);
@@ -244,34 +280,55 @@ __global__ void __launch_bounds__(32, 16) k_force(ForceArgs A)
         const unsigned cbyte = valid ? (unsigned)(mm.y >> (8 * k)) & 0xffu : 0u;
         const unsigned mbyte = (unsigned)(mm.x >> (8 * k)) & cbyte;
         float2 fjx, fjy, fjz;
-        pair_step<COUL, ENERGY, true>(K, ljw + tm, nt1, I, fix, fiy, fiz, elj, ecoul, xm, cbyte, mbyte, fjx, fjy, fjz, p3);
+        const bool found = pair_step<COUL, ENERGY, true, TWIN, PRUNE>(K, ljw + tm, nt1, I, fix, fiy, fiz, elj, ecoul, xm, cbyte,
+                                                                      mbyte, fjx, fjy, fjz, p3, A.rl2);
         if (valid) red_add_v4(&A.f4[ce.x * 8 + k], -(fjx.x + fjx.y), -(fjy.x + fjy.y), -(fjz.x + fjz.y));
+        if (PRUNE) {   // surviving cluster pairs of the step keep their {cj, mask ref}
+            const unsigned gm = __ballot_sync(0xffffffffu, found);
+            unsigned cm = gm | (gm >> 1);
+            cm |= cm >> 2;
+            cm = (cm | (cm >> 4)) & 0x01010101u;
+            if ((cm >> lane) & 1u) ilm_w[nm_w + __popc(cm & ((1u << lane) - 1u))] = ce;
+            nm_w += __popc(cm);
+        }
     }
 
-    // Cluster pairs without a mask, at half-cluster granularity: always full steps of 8 half-clusters.
-    // ptxas schedules memory operations whose consumer is an iteration away at the END of a step,
-    // so the j data is requested TWO steps ahead into registers (xj: this step, xj1: next step, x2:
-    // the one after) and the list entries four steps ahead, indices clamped to the segment.
+    // Cluster pairs without a mask: always full steps of 8 half-clusters (PRUNE: 4 clusters, the last step
+    // possibly partly filled).  ptxas schedules memory operations whose consumer is an iteration away at the
+    // END of a step, so the j data is requested TWO steps ahead into registers (xj: this step, xj1: next
+    // step, x2: the one after) and the list entries four steps ahead, indices clamped to the segment.
     int cj2 = 0, cj3 = 0;
     float4 xj1 = xj;
     int tj1 = tj;
     if (ns > 0) {
-        cj2 = il[8 * min(2, ns - 1) + g8] * 4 + k4;
-        cj3 = il[8 * min(3, ns - 1) + g8] * 4 + k4;
+        cj2 = entry(min(2, ns - 1)) * APE + k4;
+        cj3 = entry(min(3, ns - 1)) * APE + k4;
         xj1 = A.xq[cj_n];
         tj1 = A.type_slot[cj_n];
     }
 #pragma unroll 2   // (unroll 3, the period of the rotation below, was measured slower)
     for (int s = 0; s < ns; s++) {
-        const int cj4 = il[8 * min(s + 4, ns - 1) + g8] * 4 + k4;
+        const int cj4 = entry(min(s + 4, ns - 1)) * APE + k4;
         const float4 x2 = A.xq[cj2];
         const int t2 = A.type_slot[cj2];
         float2 fjx, fjy, fjz;
-        pair_step<COUL, ENERGY, false>(K, ljw + tj, nt1, I, fix, fiy, fiz, elj, ecoul, xj, 0xffu, 0xffu, fjx, fjy, fjz, p3);
+        const bool found = pair_step<COUL, ENERGY, false, TWIN, PRUNE>(K, ljw + tj, nt1, I, fix, fiy, fiz, elj, ecoul, xj, 0xffu,
+                                                                       0xffu, fjx, fjy, fjz, p3, A.rl2);
         red_add_v4(&A.f4[cj], -(fjx.x + fjx.y), -(fjy.x + fjy.y), -(fjz.x + fjz.y));
+        if (PRUNE) {
+            const unsigned gm = __ballot_sync(0xffffffffu, found);
+            unsigned hm = gm | (gm >> 1);
+            hm = (hm | (hm >> 2)) & 0x11111111u;   // bit 4h: half h of the step (lanes 4h..4h+3) has a survivor
+            if ((hm >> lane) & 1u) il_w[nu_w + __popc(hm & ((1u << lane) - 1u))] = (cj >> 2);   // slot/4 = 2*cj + half
+            nu_w += __popc(hm);
+        }
         cj = cj_n; xj = xj1; tj = tj1;
         cj_n = cj2; xj1 = x2; tj1 = t2;
         cj2 = cj3; cj3 = cj4;
+    }
+    if (PRUNE) {
+        __syncwarp();
+        nb_ilist_finish(nu_w, nm_w, sd.x + ci, lane, A.cj_dummy, il_w, ilm_w, &A.seg_cnt_w[blockIdx.x]);
     }
 
     float fi[24];
@@ -323,6 +380,20 @@ __global__ void __launch_bounds__(32, 16) k_force(ForceArgs A)
         fi[2] += __shfl_xor_sync(0xffffffffu, fi[2], d);
     }
     if ((lane & 3) == 0) red_add_v4(&A.f4[ci * 8 + (lane >> 2)], fi[0], fi[1], fi[2]);
+}
+
+// Paired LJ rows per i-cluster, written once per search (types are fixed between searches):
+// ljrow[(ci*4 + p)*nt1 + tj] = (-6c6, -6c6', 12c12, 12c12') of the i atoms 2p, 2p+1 of cluster ci against
+// j type tj -- what the force kernel's prologue copies to shared memory with one coalesced load.
+__global__ void k_ljrows(int nrows, int nt1, const int* __restrict__ type_slot, const float2* __restrict__ ljtab,
+                         float4* __restrict__ ljrow)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nrows) return;
+    const int tj = i % nt1, cp = i / nt1;   // cp = ci*4 + p
+    const int ta = type_slot[cp * 2], tb = type_slot[cp * 2 + 1];
+    const float2 ca = ljtab[ta * nt1 + tj], cb = ljtab[tb * nt1 + tj];
+    ljrow[i] = make_float4(-ca.x, -cb.x, ca.y, cb.y);
 }
 
 // (a8) gather to the caller's atom order; leaves the accumulator zeroed for the next call.
@@ -474,51 +545,107 @@ __global__ void __launch_bounds__(256) k_count_pairs(ForceArgs A, unsigned long 
 
 // Atom-pair slots of the inner list as the force kernel evaluates it: 32 per real (non-dummy) half-cluster
 // entry, 64 per masked cluster pair.  One thread per segment; statistics only.
-__global__ void k_count_slots(const int4* __restrict__ seg, int nseg, const int* __restrict__ il, int nhalf_real,
-                              unsigned long long* __restrict__ out)
+__global__ void k_count_slots(ForceArgs A, int nseg, int nhalf_real, unsigned long long* __restrict__ out)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     unsigned long long n = 0;
     if (i < nseg) {
-        const int4 sg = seg[i];
-        for (int e = 0; e < sg.z; e++) n += il[sg.x + e] < nhalf_real ? 32u : 0u;
-        n += 64ull * sg.w;
+        const int4 sd = A.segd[i];
+        const int buf = nb_seg_buf(sd.w, A.bufmask, A.nparts, A.nunits);
+        const int2 cnt = A.seg_cnt[buf][i];
+        for (int e = 0; e < cnt.x; e++) n += A.il[buf][sd.x + e] < nhalf_real ? 32u : 0u;
+        n += 64ull * cnt.y;
     }
     for (int d = 16; d > 0; d >>= 1) n += __shfl_xor_sync(0xffffffffu, n, d);
     if ((threadIdx.x & 31) == 0 && n) atomicAdd(out, n);
 }
 
-template <int COUL, bool ENERGY>
+template <int COUL, bool ENERGY, bool TWIN, bool PRUNE>
 int launch_force(nb_ctx* c, const ForceArgs& A)
 {
     const size_t smem = sizeof(float4) * 4 * (size_t)c->kc.ntypes1;   // paired LJ table of one i-cluster, 64 B per type
     if (smem > 48 * 1024)
-        NB_CUDA(c, cudaFuncSetAttribute(k_force<COUL, ENERGY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_force<COUL, ENERGY><<<c->nseg_launch, 32, smem, c->stream>>>(A);
+        NB_CUDA(c, cudaFuncSetAttribute(k_force<COUL, ENERGY, TWIN, PRUNE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_force<COUL, ENERGY, TWIN, PRUNE><<<c->nseg_launch, 32, smem, c->stream>>>(A);
     NB_LAUNCH_CHECK(c);
     return NB_OK;
 }
 
+// One instantiation per combination of electrostatics, energy / no energy, single / twin cut-off and
+// plain / fused-prune ("separate kernels are used for different combinations ... to avoid conditionals").
+template <int COUL, bool ENERGY, bool TWIN>
+int launch_force_p(nb_ctx* c, const ForceArgs& A, bool prune)
+{
+    return prune ? launch_force<COUL, ENERGY, TWIN, true>(c, A) : launch_force<COUL, ENERGY, TWIN, false>(c, A);
+}
+template <int COUL, bool ENERGY>
+int launch_force_t(nb_ctx* c, const ForceArgs& A, bool twin, bool prune)
+{
+    return twin ? launch_force_p<COUL, ENERGY, true>(c, A, prune) : launch_force_p<COUL, ENERGY, false>(c, A, prune);
+}
+template <int COUL>
+int launch_force_e(nb_ctx* c, const ForceArgs& A, bool energy, bool twin, bool prune)
+{
+    return energy ? launch_force_t<COUL, true>(c, A, twin, prune) : launch_force_t<COUL, false>(c, A, twin, prune);
+}
+
 }  // namespace
 
-int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial)
+static void fill_force_args(nb_ctx* c, ForceArgs& A)
 {
-    cudaStream_t st = c->stream;
-    ForceArgs A;
-    A.units = c->units_sorted.p;
+    memset(&A, 0, sizeof(A));
+    A.units = c->units_canon.p;
     A.jl = c->jl.p;
     A.plane = c->plane_inner.p;
-    A.seg = c->seg.p;
-    A.seg_ci = c->seg_ci.p;
-    A.il = c->il.p;
-    A.ilm = c->ilm.p;
+    A.segd = c->segd.p;
+    for (int b = 0; b < 2; b++) {
+        A.seg_cnt[b] = c->seg_cnt[b].p;
+        A.il[b] = c->il[b].p;
+        A.ilm[b] = c->ilm[b].p;
+    }
+    A.bufmask = c->bufmask;
+    A.nparts = c->buf_nparts;
+    A.nunits = c->nunits;
     A.xq = c->xq.p;
     A.type_slot = c->type_slot.p;
-    A.ljtab = c->ljtab.p;
+    A.ljrow = c->ljrow.p;
     A.masks = c->excl_masks.p;
     A.f4 = c->f4.p;
     A.kc = c->kc;
     for (int k = 0; k < 3; k++) A.kc.box[k] = c->box[k];
+}
+
+int nbi_ljrows(nb_ctx* c)
+{
+    const int nt1 = c->kc.ntypes1, nrows = c->nclusters_max * 4 * nt1;
+    NB_CUDA(c, c->ljrow.ensure(nrows, c->stream));
+    k_ljrows<<<(nrows + 255) / 256, 256, 0, c->stream>>>(nrows, nt1, c->type_slot.p, c->ljtab.p, c->ljrow.p);
+    NB_LAUNCH_CHECK(c);
+    return NB_OK;
+}
+
+// rlist_inner > 0: the fused first prune (nb_forces_prune): walk the outer list, write the whole inner list.
+int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial, float rlist_inner)
+{
+    cudaStream_t st = c->stream;
+    const bool prune = rlist_inner > 0.f;
+    if (prune) {
+        int rcp = nbi_consolidate(c);   // everything is (re)written into inner buffer 0
+        if (rcp != NB_OK) return rcp;
+        c->last_nparts = 1;
+        c->planes_dirty = true;
+        c->st.prune_count++;
+    }
+    ForceArgs A;
+    fill_force_args(c, A);
+    A.ol_cnt = c->ol_cnt.p;
+    A.olu = c->olu.p;
+    A.olm = c->olm.p;
+    A.il_w = c->il[0].p;
+    A.ilm_w = c->ilm[0].p;
+    A.seg_cnt_w = c->seg_cnt[0].p;
+    A.rl2 = rlist_inner * rlist_inner;
+    A.cj_dummy = c->nclusters_max;
     {
         const double P[5] = {NB_EWC_P0, NB_EWC_P1, NB_EWC_P2, NB_EWC_P3, NB_EWC_P4};
         const double Q[6] = {NB_EWC_Q0, NB_EWC_Q1, NB_EWC_Q2, NB_EWC_Q3, NB_EWC_Q4, NB_EWC_Q5};
@@ -540,23 +667,23 @@ int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial)
     }
     int rc = NB_OK;
     if (c->nunits > 0 && c->nseg_launch > 0) {
-        NbStageTimer tm(c, NB_T_FORCE);
-        if (c->prm.coulomb == NB_COUL_EWALD)
-            rc = energy ? launch_force<NB_COUL_EWALD, true>(c, A) : launch_force<NB_COUL_EWALD, false>(c, A);
-        else if (c->prm.coulomb == NB_COUL_RF)
-            rc = energy ? launch_force<NB_COUL_RF, true>(c, A) : launch_force<NB_COUL_RF, false>(c, A);
-        else
-            rc = energy ? launch_force<NB_COUL_NONE, true>(c, A) : launch_force<NB_COUL_NONE, false>(c, A);
+        NbStageTimer tm(c, energy ? NB_T_FORCE_ENERGY : NB_T_FORCE);
+        const bool twin = c->twin;
+        if (c->prm.coulomb == NB_COUL_EWALD) rc = launch_force_e<NB_COUL_EWALD>(c, A, energy, twin, prune);
+        else if (c->prm.coulomb == NB_COUL_RF) rc = launch_force_e<NB_COUL_RF>(c, A, energy, twin, prune);
+        else rc = launch_force_e<NB_COUL_NONE>(c, A, energy, twin, prune);
         if (rc != NB_OK) return rc;
     }
     double* xf = c->fshift.p + NB_NSHIFT * 3;
-    const int nb = (c->nslots + 255) / 256;
+    // (the slots between the actual and the bounded number of super-clusters hold no atoms: atom_of_slot = -1)
+    const int nslots = c->nslots_max;
+    const int nb = (nslots + 255) / 256;
     NbStageTimer tm(c, NB_T_REDUCE);
     if (virial)
-        k_gather<true><<<nb, 256, 0, st>>>(c->nslots, c->f4.p, c->atom_of_slot.p, c->xq.p, f, xf);
+        k_gather<true><<<nb, 256, 0, st>>>(nslots, c->f4.p, c->atom_of_slot.p, c->xq.p, f, xf);
     else
-        k_gather4<<<(c->nslots / 4 + 255) / 256, 256, 0, st>>>(c->nslots / 4, c->f4.p,
-                                                              reinterpret_cast<const int4*>(c->atom_of_slot.p), f);
+        k_gather4<<<(nslots / 4 + 255) / 256, 256, 0, st>>>(nslots / 4, c->f4.p,
+                                                           reinterpret_cast<const int4*>(c->atom_of_slot.p), f);
     NB_LAUNCH_CHECK(c);
     if (virial) {
         k_virial_final<<<1, 32, 0, st>>>(xf, c->fshift.p, make_float3(c->box[0], c->box[1], c->box[2]), virial);
@@ -596,10 +723,14 @@ int nbi_measure_fp32_peak(nb_ctx* c, double* fma_per_s)
 int nbi_count_slots(nb_ctx* c, int64_t* slots)
 {
     cudaStream_t st = c->stream;
+    int rc = nbi_commit_pending(c);
+    if (rc != NB_OK) return rc;
     NB_CUDA(c, c->counters.ensure(8, st));
     NB_CUDA(c, cudaMemsetAsync(c->counters.p, 0, 8 * sizeof(long long), st));
     if (c->nseg_launch > 0) {
-        k_count_slots<<<(c->nseg_launch + 127) / 128, 128, 0, st>>>(c->seg.p, c->nseg_launch, c->il.p, 2 * c->nclusters,
+        ForceArgs A;
+        fill_force_args(c, A);
+        k_count_slots<<<(c->nseg_launch + 127) / 128, 128, 0, st>>>(A, c->nseg_launch, 2 * c->nclusters_max,
                                                                    (unsigned long long*)c->counters.p);
         NB_LAUNCH_CHECK(c);
     }
@@ -610,36 +741,51 @@ int nbi_count_slots(nb_ctx* c, int64_t* slots)
     return NB_OK;
 }
 
-int nbi_inner_dump(nb_ctx* c, int64_t* n, int32_t* ci, int32_t* entry, int32_t* shift, int32_t* kind)
+int nbi_inner_dump(nb_ctx* c, int64_t* n, int32_t* ci, int32_t* entry, int32_t* shift, int32_t* kind, int32_t* part)
 {
     cudaStream_t st = c->stream;
-    const int ns = c->nseg_launch;
-    std::vector<int4> seg(std::max(ns, 1));
-    std::vector<int2> sci(std::max(ns, 1)), ilm(c->ilm_total + 1);
-    std::vector<int32_t> il(c->il_total + 1);
+    int rc = nbi_commit_pending(c);
+    if (rc != NB_OK) return rc;
+    const int ns = c->nseg_launch, nbuf = c->have_buf1 ? 2 : 1;
+    std::vector<int4> segd(std::max(ns, 1));
+    std::vector<int2> cnt[2], ilm[2];
+    std::vector<int32_t> il[2];
+    for (int b = 0; b < nbuf; b++) {
+        cnt[b].resize(std::max(ns, 1));
+        il[b].resize(c->il_total + 1);
+        ilm[b].resize(c->ilm_total + 1);
+    }
     if (ns > 0) {
-        NB_CUDA(c, cudaMemcpyAsync(seg.data(), c->seg.p, sizeof(int4) * ns, cudaMemcpyDeviceToHost, st));
-        NB_CUDA(c, cudaMemcpyAsync(sci.data(), c->seg_ci.p, sizeof(int2) * ns, cudaMemcpyDeviceToHost, st));
-        if (c->il_total) NB_CUDA(c, cudaMemcpyAsync(il.data(), c->il.p, sizeof(int32_t) * c->il_total, cudaMemcpyDeviceToHost, st));
-        if (c->ilm_total) NB_CUDA(c, cudaMemcpyAsync(ilm.data(), c->ilm.p, sizeof(int2) * c->ilm_total, cudaMemcpyDeviceToHost, st));
+        NB_CUDA(c, cudaMemcpyAsync(segd.data(), c->segd.p, sizeof(int4) * ns, cudaMemcpyDeviceToHost, st));
+        for (int b = 0; b < nbuf; b++) {
+            NB_CUDA(c, cudaMemcpyAsync(cnt[b].data(), c->seg_cnt[b].p, sizeof(int2) * ns, cudaMemcpyDeviceToHost, st));
+            if (c->il_total) NB_CUDA(c, cudaMemcpyAsync(il[b].data(), c->il[b].p, sizeof(int32_t) * c->il_total, cudaMemcpyDeviceToHost, st));
+            if (c->ilm_total) NB_CUDA(c, cudaMemcpyAsync(ilm[b].data(), c->ilm[b].p, sizeof(int2) * c->ilm_total, cudaMemcpyDeviceToHost, st));
+        }
     }
     NB_CUDA(c, cudaStreamSynchronize(st));
     int64_t k = 0;
     for (int s = 0; s < ns; s++) {
-        for (int e = 0; e < seg[s].z; e++) {
-            const int hc = il[seg[s].x + e];
-            if (hc >= 2 * c->nclusters) continue;   // dummy padding
-            if (ci) ci[k] = sci[s].x;
+        const int4 sd = segd[s];
+        const int b = c->bufmask ? (int)((c->bufmask >> nb_part_of_unit(sd.w, c->buf_nparts, c->nunits)) & 1u) : 0;
+        const int sci = sd.z & 0x3ffffff, sid = sd.z >> 26;
+        const int prt = nb_part_of_unit(sd.w, std::max(c->last_nparts, 1), std::max(c->nunits, 1));
+        for (int e = 0; e < cnt[b][s].x; e++) {
+            const int hc = il[b][sd.x + e];
+            if (hc >= 2 * c->nclusters_max) continue;   // dummy padding
+            if (ci) ci[k] = sci;
             if (entry) entry[k] = hc;
-            if (shift) shift[k] = sci[s].y;
+            if (shift) shift[k] = sid;
             if (kind) kind[k] = 0;
+            if (part) part[k] = prt;
             k++;
         }
-        for (int e = 0; e < seg[s].w; e++) {
-            if (ci) ci[k] = sci[s].x;
-            if (entry) entry[k] = ilm[seg[s].y + e].x;
-            if (shift) shift[k] = sci[s].y;
+        for (int e = 0; e < cnt[b][s].y; e++) {
+            if (ci) ci[k] = sci;
+            if (entry) entry[k] = ilm[b][sd.y + e].x;
+            if (shift) shift[k] = sid;
             if (kind) kind[k] = 1;
+            if (part) part[k] = prt;
             k++;
         }
     }
@@ -650,15 +796,10 @@ int nbi_inner_dump(nb_ctx* c, int64_t* n, int32_t* ci, int32_t* entry, int32_t* 
 int nbi_count_pairs(nb_ctx* c, int64_t* n_interacting, int64_t* n_excluded)
 {
     cudaStream_t st = c->stream;
+    int rc = nbi_rebuild_inner_planes(c);
+    if (rc != NB_OK) return rc;
     ForceArgs A;
-    memset(&A, 0, sizeof(A));
-    A.units = c->units_canon.p;
-    A.jl = c->jl.p;
-    A.plane = c->plane_inner.p;
-    A.xq = c->xq.p;
-    A.masks = c->excl_masks.p;
-    A.kc = c->kc;
-    for (int k = 0; k < 3; k++) A.kc.box[k] = c->box[k];
+    fill_force_args(c, A);
     NB_CUDA(c, c->counters.ensure(8, st));
     NB_CUDA(c, cudaMemsetAsync(c->counters.p, 0, 8 * sizeof(long long), st));
     if (c->nunits > 0) {

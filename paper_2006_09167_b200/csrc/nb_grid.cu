@@ -21,39 +21,53 @@ __device__ __forceinline__ uint32_t float_orderable(float v)
 
 // One thread per atom: wrap into the box (image fixed until the next search), column index,
 // rank inside the column (arrival order; the later sort makes the layout deterministic).
-__global__ void k_bin(int n, const float* __restrict__ x, const float* __restrict__ q, float3 box, int ncx,
-                      int ncy, float inv_cx, float inv_cy, char4* __restrict__ image,
+// The column counters are few (a hundred for 100k atoms) and consecutive atoms mostly share a column,
+// so the lanes of a warp that hit the same column send ONE atomic (match_any + popc ranks).
+__global__ void k_bin(int n, const float* __restrict__ x, const float* __restrict__ q, const int* __restrict__ type,
+                      int ntypes, float3 box, int ncx, int ncy, float inv_cx, float inv_cy, char4* __restrict__ image,
                       float4* __restrict__ xw_atom, int* __restrict__ atom_col, int* __restrict__ atom_rank,
-                      int* __restrict__ col_count)
+                      int* __restrict__ col_count, NbTotals* __restrict__ tot)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    float L[3] = {box.x, box.y, box.z};
-    float w[3];
-    int img[3];
+    const int lane = threadIdx.x & 31;
+    int col = -1;
+    if (i < n) {
+        float L[3] = {box.x, box.y, box.z};
+        float w[3];
+        int img[3];
 #pragma unroll
-    for (int k = 0; k < 3; k++) {
-        float v = x[3 * i + k];
-        float kf = floorf(v / L[k]);
-        float t = __fmaf_rn(-kf, L[k], v);
-        if (t < 0.f) { kf -= 1.f; t = __fmaf_rn(-kf, L[k], v); }
-        else if (t >= L[k]) { kf += 1.f; t = __fmaf_rn(-kf, L[k], v); }
-        kf = fminf(fmaxf(kf, -127.f), 127.f);
-        w[k] = __fmaf_rn(-kf, L[k], v);
-        img[k] = (int)kf;
+        for (int k = 0; k < 3; k++) {
+            float v = x[3 * i + k];
+            float kf = floorf(v / L[k]);
+            float t = __fmaf_rn(-kf, L[k], v);
+            if (t < 0.f) { kf -= 1.f; t = __fmaf_rn(-kf, L[k], v); }
+            else if (t >= L[k]) { kf += 1.f; t = __fmaf_rn(-kf, L[k], v); }
+            kf = fminf(fmaxf(kf, -127.f), 127.f);
+            w[k] = __fmaf_rn(-kf, L[k], v);
+            img[k] = (int)kf;
+        }
+        int cx = min(ncx - 1, max(0, (int)floorf(w[0] * inv_cx)));
+        int cy = min(ncy - 1, max(0, (int)floorf(w[1] * inv_cy)));
+        col = cx * ncy + cy;
+        image[i] = make_char4((signed char)img[0], (signed char)img[1], (signed char)img[2], 0);
+        xw_atom[i] = make_float4(w[0], w[1], w[2], q[i]);
+        atom_col[i] = col;
+        const int t = type[i];
+        if (t < 0 || t >= ntypes) tot->bad_type = 1;   // reported as NB_ERR_ARG at the end of the search
     }
-    int cx = min(ncx - 1, max(0, (int)floorf(w[0] * inv_cx)));
-    int cy = min(ncy - 1, max(0, (int)floorf(w[1] * inv_cy)));
-    int col = cx * ncy + cy;
-    image[i] = make_char4((signed char)img[0], (signed char)img[1], (signed char)img[2], 0);
-    xw_atom[i] = make_float4(w[0], w[1], w[2], q[i]);
-    atom_col[i] = col;
-    atom_rank[i] = atomicAdd(&col_count[col], 1);
+    const unsigned peers = __match_any_sync(0xffffffffu, col);
+    if (col >= 0) {
+        const int leader = __ffs(peers) - 1;
+        int base = 0;
+        if (lane == leader) base = atomicAdd(&col_count[col], __popc(peers));
+        base = __shfl_sync(peers, base, leader);
+        atom_rank[i] = base + __popc(peers & ((1u << lane) - 1u));
+    }
 }
 
 // Single block: exclusive scans over columns of the atom count and of the super-cluster count.
 __global__ void k_col_scan(int ncol, const int* __restrict__ col_count, int* __restrict__ col_atom_off,
-                           int* __restrict__ col_sc_off, int* __restrict__ totals)
+                           int* __restrict__ col_sc_off, NbTotals* __restrict__ totals)
 {
     __shared__ int s_a[1024], s_s[1024];
     __shared__ int carry_a, carry_s, maxc;
@@ -86,8 +100,8 @@ __global__ void k_col_scan(int ncol, const int* __restrict__ col_count, int* __r
     if (t == 0) {
         col_atom_off[ncol] = carry_a;
         col_sc_off[ncol] = carry_s;
-        totals[0] = carry_s;
-        totals[1] = maxc;
+        totals->nsc = carry_s;
+        totals->max_col = maxc;
     }
 }
 
@@ -146,13 +160,17 @@ k_col_layout(int ncy, const int* __restrict__ col_atom_off, const int* __restric
              const int* __restrict__ type, int pad_type, int np2_max, float4* __restrict__ xq,
              int* __restrict__ type_slot, int* __restrict__ atom_of_slot, int* __restrict__ slot_of_atom,
              float4* __restrict__ bb_lo, float4* __restrict__ bb_hi, float4* __restrict__ sbb_lo,
-             float4* __restrict__ sbb_hi, float3 pad_base, float3 pad_step)
+             float4* __restrict__ sbb_hi, float3 pad_base, float3 pad_step, NbTotals* __restrict__ tot)
 {
     extern __shared__ unsigned long long s_keys[];
     __shared__ SlabScratch s_slab[8];
     int col = blockIdx.x;
     int a0 = col_atom_off[col], n = col_atom_off[col + 1] - a0;
     if (n == 0) return;
+    if (n > np2_max) {   // the sort buffer was sized from the previous search: say so, the host repeats the search
+        if (threadIdx.x == 0) atomicOr(&tot->overflow, NB_OVF_COL);
+        return;
+    }
     int np2 = 1;
     while (np2 < n) np2 <<= 1;
     for (int i = threadIdx.x; i < np2; i += blockDim.x) {
@@ -252,6 +270,30 @@ k_col_layout(int ncy, const int* __restrict__ col_atom_off, const int* __restric
     }
 }
 
+// Arrays are sized and kernels launched for nsc_max = natoms/64 + columns super-clusters, a bound the
+// host knows without reading anything back; the super-clusters between the actual count and the
+// bound are written as empty ones (no atoms, no bounding box: they are never listed).
+__global__ void k_grid_tail(int nsc_max, const NbTotals* __restrict__ tot, int pad_type, float4* __restrict__ xq,
+                            int* __restrict__ type_slot, int* __restrict__ atom_of_slot, float4* __restrict__ bb_lo,
+                            float4* __restrict__ bb_hi, float4* __restrict__ sbb_lo, float4* __restrict__ sbb_hi,
+                            float3 pad_base, float3 pad_step)
+{
+    const int slot = tot->nsc * NB_SC_ATOMS + blockIdx.x * blockDim.x + threadIdx.x;
+    if (slot >= nsc_max * NB_SC_ATOMS) return;
+    const int e = slot & 63, sc = slot >> 6;
+    xq[slot] = make_float4(pad_base.x - pad_step.x * (float)e, pad_base.y - pad_step.y * (float)(sc & 63), pad_base.z, 0.f);
+    type_slot[slot] = pad_type;
+    atom_of_slot[slot] = -1;
+    if ((e & 7) == 0) {
+        bb_lo[slot >> 3] = make_float4(1e30f, 1e30f, 1e30f, 0.f);
+        bb_hi[slot >> 3] = make_float4(-1e30f, -1e30f, -1e30f, 0.f);
+    }
+    if (e == 0) {
+        sbb_lo[sc] = make_float4(1e30f, 1e30f, 1e30f, -1.f);
+        sbb_hi[sc] = make_float4(-1e30f, -1e30f, -1e30f, 0.f);
+    }
+}
+
 // (a1) refresh of the cluster-ordered coordinates from caller-order x with the stored image.
 __global__ void k_refresh_xq(int n, const float* __restrict__ x, const float* __restrict__ q,
                              const char4* __restrict__ image, const int* __restrict__ slot_of_atom, float3 box,
@@ -323,6 +365,10 @@ int nbi_grid(nb_ctx* c)
     c->ncol = c->ncx * c->ncy;
     c->inv_cx = (float)(c->ncx / (double)L[0]);
     c->inv_cy = (float)(c->ncy / (double)L[1]);
+    // sum over columns of ceil(count/64) <= natoms/64 + columns: everything below is sized by this bound
+    c->nsc_max = n / NB_SC_ATOMS + c->ncol;
+    c->nclusters_max = c->nsc_max * NB_SUPER_SIZE;
+    c->nslots_max = c->nsc_max * NB_SC_ATOMS;
     NB_CUDA(c, c->col_count.ensure(c->ncol + 1, st));
     NB_CUDA(c, c->col_atom_off.ensure(c->ncol + 1, st));
     NB_CUDA(c, c->col_sc_off.ensure(c->ncol + 1, st));
@@ -332,41 +378,39 @@ int nbi_grid(nb_ctx* c)
     NB_CUDA(c, c->image.ensure(n, st));
     NB_CUDA(c, c->xw_atom.ensure(n, st));
     NB_CUDA(c, c->slot_of_atom.ensure(n, st));
-    NB_CUDA(c, c->grid_totals.ensure(4, st));
+    NB_CUDA(c, c->xq.ensure(c->nslots_max + NB_C * NB_NDUMMY, st));   // + dummy clusters (index >= nclusters_max), see below
+    NB_CUDA(c, c->type_slot.ensure(c->nslots_max + NB_C * NB_NDUMMY, st));
+    NB_CUDA(c, c->atom_of_slot.ensure(c->nslots_max, st));
+    NB_CUDA(c, c->bb_lo.ensure(c->nclusters_max, st));
+    NB_CUDA(c, c->bb_hi.ensure(c->nclusters_max, st));
+    NB_CUDA(c, c->sbb_lo.ensure(c->nsc_max, st));
+    NB_CUDA(c, c->sbb_hi.ensure(c->nsc_max, st));
+    NB_CUDA(c, c->f4.ensure(c->nslots_max + NB_C * NB_NDUMMY, st));
+    NB_CUDA(c, cudaMemsetAsync(c->f4.p, 0, sizeof(float4) * (c->nslots_max + NB_C * NB_NDUMMY), st));
     NB_CUDA(c, cudaMemsetAsync(c->col_count.p, 0, sizeof(int) * (c->ncol + 1), st));
     float3 box = make_float3(L[0], L[1], L[2]);
-    k_bin<<<(n + 255) / 256, 256, 0, st>>>(n, c->x.p, c->q.p, box, c->ncx, c->ncy, c->inv_cx, c->inv_cy,
-                                           c->image.p, c->xw_atom.p, c->atom_col.p, c->atom_rank.p,
-                                           c->col_count.p);
+    k_bin<<<(n + 255) / 256, 256, 0, st>>>(n, c->x.p, c->q.p, c->type.p, c->ntypes, box, c->ncx, c->ncy, c->inv_cx, c->inv_cy,
+                                           c->image.p, c->xw_atom.p, c->atom_col.p, c->atom_rank.p, c->col_count.p, c->tot_dev);
     NB_LAUNCH_CHECK(c);
-    k_col_scan<<<1, 1024, 0, st>>>(c->ncol, c->col_count.p, c->col_atom_off.p, c->col_sc_off.p,
-                                   c->grid_totals.p);
+    k_col_scan<<<1, 1024, 0, st>>>(c->ncol, c->col_count.p, c->col_atom_off.p, c->col_sc_off.p, c->tot_dev);
     NB_LAUNCH_CHECK(c);
     k_col_scatter<<<(n + 255) / 256, 256, 0, st>>>(n, c->atom_col.p, c->atom_rank.p, c->col_atom_off.p,
                                                    c->col_atoms.p);
     NB_LAUNCH_CHECK(c);
-    int tot[2];
-    NB_CUDA(c, cudaMemcpyAsync(tot, c->grid_totals.p, sizeof(tot), cudaMemcpyDeviceToHost, st));
-    NB_CUDA(c, cudaStreamSynchronize(st));
-    c->nsc = tot[0];
-    c->max_col_count = tot[1];
-    c->nclusters = c->nsc * NB_SUPER_SIZE;
-    c->nslots = c->nsc * NB_SC_ATOMS;
-    int np2 = 1;
-    while (np2 < c->max_col_count) np2 <<= 1;
+    if (c->cold) {
+        // no capacity known yet: read the largest column population back and size the in-shared-memory sort from it
+        NB_CUDA(c, cudaMemcpyAsync(c->tot_host, c->tot_dev, sizeof(NbTotals), cudaMemcpyDeviceToHost, st));
+        NB_CUDA(c, cudaStreamSynchronize(st));
+        int want = c->tot_host->max_col + c->tot_host->max_col / 8 + 8, np2 = 64;
+        while (np2 < want) np2 <<= 1;
+        if (np2 / 2 >= c->tot_host->max_col + 8 && np2 > 64) np2 >>= 1;   // (head-room only where the power of two leaves some)
+        c->np2_col = np2;
+    }
+    const int np2 = c->np2_col;
     size_t smem = (size_t)np2 * sizeof(unsigned long long);
     if (smem > 200 * 1024)
         return nb_fail(c, NB_ERR_OVERFLOW, "grid column holds %d atoms; the in-shared-memory z-sort takes at most 25600",
-                       c->max_col_count);
-    NB_CUDA(c, c->xq.ensure(c->nslots + NB_C * NB_NDUMMY, st));   // + dummy clusters (index >= nclusters), see below
-    NB_CUDA(c, c->type_slot.ensure(c->nslots + NB_C * NB_NDUMMY, st));
-    NB_CUDA(c, c->atom_of_slot.ensure(c->nslots, st));
-    NB_CUDA(c, c->bb_lo.ensure(c->nclusters, st));
-    NB_CUDA(c, c->bb_hi.ensure(c->nclusters, st));
-    NB_CUDA(c, c->sbb_lo.ensure(c->nsc, st));
-    NB_CUDA(c, c->sbb_hi.ensure(c->nsc, st));
-    NB_CUDA(c, c->f4.ensure(c->nslots + NB_C * NB_NDUMMY, st));
-    NB_CUDA(c, cudaMemsetAsync(c->f4.p, 0, sizeof(float4) * (c->nslots + NB_C * NB_NDUMMY), st));
+                       c->tot_host->max_col);
     NB_CUDA(c, cudaFuncSetAttribute(k_col_layout, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     float pb[3], pd[3];
     for (int k = 0; k < 3; k++) {
@@ -377,12 +421,17 @@ int nbi_grid(nb_ctx* c)
                                              c->xw_atom.p, c->type.p, c->ntypes, np2, c->xq.p, c->type_slot.p,
                                              c->atom_of_slot.p, c->slot_of_atom.p, c->bb_lo.p, c->bb_hi.p,
                                              c->sbb_lo.p, c->sbb_hi.p, make_float3(pb[0], pb[1], pb[2]),
-                                             make_float3(pd[0], pd[1], pd[2]));
+                                             make_float3(pd[0], pd[1], pd[2]), c->tot_dev);
     NB_LAUNCH_CHECK(c);
-    if (c->dummy_at != (const void*)(c->xq.p + c->nslots) || c->dummy_box[0] != L[0] || c->dummy_box[1] != L[1] ||
+    k_grid_tail<<<(c->ncol * NB_SC_ATOMS + 255) / 256, 256, 0, st>>>(c->nsc_max, c->tot_dev, c->ntypes, c->xq.p, c->type_slot.p,
+                                                                   c->atom_of_slot.p, c->bb_lo.p, c->bb_hi.p, c->sbb_lo.p,
+                                                                   c->sbb_hi.p, make_float3(pb[0], pb[1], pb[2]),
+                                                                   make_float3(pd[0], pd[1], pd[2]));
+    NB_LAUNCH_CHECK(c);
+    if (c->dummy_at != (const void*)(c->xq.p + c->nslots_max) || c->dummy_box[0] != L[0] || c->dummy_box[1] != L[1] ||
         c->dummy_box[2] != L[2]) {
         // (rewritten only when the box or their place in the arrays has changed)
-        // Dummy j-clusters (index nclusters .. nclusters + NB_NDUMMY - 1): padding-like atoms beyond the
+        // Dummy j-clusters (index nclusters_max .. nclusters_max + NB_NDUMMY - 1): padding-like atoms beyond the
         // padding lattice that interact with nothing.  The prune kernel may fill an inner list
         // segment up to a multiple of 8 half-clusters with them; the (zero) forces the force kernel adds to their
         // slots are never read, and spreading them over NB_NDUMMY clusters avoids atomic hot spots.
@@ -390,10 +439,10 @@ int nbi_grid(nb_ctx* c)
         std::vector<int32_t> ht((size_t)NB_C * NB_NDUMMY, c->ntypes);
         for (size_t i = 0; i < hx.size(); i++)
             hx[i] = make_float4(pb[0] - pd[0] * (float)(64 + (i % NB_C)), pb[1], pb[2], 0.f);
-        NB_CUDA(c, cudaMemcpyAsync(c->xq.p + c->nslots, hx.data(), sizeof(float4) * hx.size(), cudaMemcpyHostToDevice, st));
-        NB_CUDA(c, cudaMemcpyAsync(c->type_slot.p + c->nslots, ht.data(), sizeof(int32_t) * ht.size(), cudaMemcpyHostToDevice, st));
+        NB_CUDA(c, cudaMemcpyAsync(c->xq.p + c->nslots_max, hx.data(), sizeof(float4) * hx.size(), cudaMemcpyHostToDevice, st));
+        NB_CUDA(c, cudaMemcpyAsync(c->type_slot.p + c->nslots_max, ht.data(), sizeof(int32_t) * ht.size(), cudaMemcpyHostToDevice, st));
         NB_CUDA(c, cudaStreamSynchronize(st));
-        c->dummy_at = c->xq.p + c->nslots;
+        c->dummy_at = c->xq.p + c->nslots_max;
         for (int k = 0; k < 3; k++) c->dummy_box[k] = L[k];
     }
     c->grid_box[0] = L[0];
@@ -402,9 +451,6 @@ int nbi_grid(nb_ctx* c)
     c->have_grid = true;
     c->st.ncolumns_x = c->ncx;
     c->st.ncolumns_y = c->ncy;
-    c->st.nsuper = c->nsc;
-    c->st.nclusters = c->nclusters;
-    c->st.nslots = c->nslots;
     c->st.cluster_size = NB_C;
     return NB_OK;
 }

@@ -20,6 +20,25 @@
 #define NB_NDUMMY 1024                // dummy j-clusters behind the real ones (spread the never-read force adds)
 #define NB_PAD_TYPE_ROW 1             // LJ table carries one extra all-zero type for padding atoms
 
+// Counts produced on the device during a search.  Lives in device memory (`tot_dev`) where the stage
+// kernels read their bounds from, and is copied to a pinned host mirror once, at the end of nb_search:
+// the host sizes buffers from the previous search with head-room and only reads counts back to check
+// that nothing overflowed ("host only reads back list counts when it must grow buffers").
+struct NbTotals {
+    int nsc, max_col;          // (a2) super-clusters, largest column population
+    int njslots;               // (a3) joint j slots (multiple of NB_BATCH)
+    int nunits;                // (a5) work units
+    int nmask;                 // (a4) joint entries with an exclusion mask
+    int il_total, ilm_total;   // extents of the compact lists (sum of segment capacities)
+    int nseg_launch;           // segments with a non-empty outer list
+    int overflow;              // NB_OVF_* bits: a stage found its buffer too small and did nothing
+    int bad_type;              // an atom type outside [0, ntypes)
+    int pad[6];
+};
+enum { NB_OVF_COL = 1, NB_OVF_JOINT = 2, NB_OVF_UNITS = 4, NB_OVF_MASKS = 8, NB_OVF_IL = 16, NB_OVF_ILM = 32 };
+#define NB_SEG_MAXKEY 2080              // segment length key (half entries + 2 x masked) is below this
+#define NB_MAX_SORT_PARTS 16            // rolling parts whose prune order is sorted longest first (more: canonical order)
+
 // One growable device array.
 template <typename T>
 struct DevBuf {
@@ -56,6 +75,7 @@ struct DevBuf {
 struct NbConst {
     float box[3];
     float rc2;            // rc^2
+    float rcv2;           // rc_vdw^2 (twin cut-offs; = rc^2 otherwise)
     float epsfac;
     float beta, beta2, beta3;
     float ewald_shift;    // erfc(beta rc)/rc if potential-shift else 0
@@ -75,6 +95,7 @@ struct nb_ctx {
     NbConst kc;
     float beta = 0.f;
     double beta_d = 0.0;                       // Ewald beta in fp64 (coefficient folding)
+    bool twin = false;                         // rc_vdw < rc: the TWIN kernel flavours
 
     // --- state machine ---
     bool have_atoms = false, have_grid = false, have_list = false, atoms_since_search = false;
@@ -99,10 +120,10 @@ struct nb_ctx {
     int ncx = 0, ncy = 0, ncol = 0;
     float inv_cx = 0.f, inv_cy = 0.f;          // columns per nm
     DevBuf<int32_t> col_count, col_atom_off, col_sc_off, atom_col, atom_rank, col_atoms;
-    DevBuf<int32_t> grid_totals;               // [4]: nsc, max column count, ...
     DevBuf<char4> image;                       // periodic image fixed at the last search
     DevBuf<float4> xw_atom;                    // wrapped (x,y,z,q) in caller order, search scratch
-    int nsc = 0, nslots = 0, nclusters = 0, max_col_count = 0;
+    int nsc = 0, nslots = 0, nclusters = 0, max_col_count = 0;   // exact, known after the end-of-search synchronisation
+    int nclusters_max = 0, nslots_max = 0;     // nsc_max * 8, * 64: array extents; the dummy clusters start at nclusters_max
     DevBuf<float4> xq;                         // [nslots] x,y,z,q   (cluster order)
     DevBuf<int32_t> type_slot, atom_of_slot, slot_of_atom;
     DevBuf<float4> bb_lo, bb_hi;               // per cluster; lo.w = number of real atoms
@@ -113,7 +134,6 @@ struct nb_ctx {
     int nent = 0;                              // nsc * NB_NHALF (super-cluster, shift) slots, some empty
     DevBuf<int32_t> ent_count;                 // [nent] joint entries per slot
     DevBuf<int32_t> ent_jbegin;                // [nent+1] first j slot (multiple of NB_BATCH)
-    std::vector<int32_t> h_ent_count, h_ent_jbegin;
     int64_t njslots = 0, nbatch = 0;
     DevBuf<int2> jl;                           // [njslots] {cj, exclusion mask ref (0 = none)}
     DevBuf<uint8_t> imask_outer;               // [njslots] 8-bit interaction mask
@@ -125,36 +145,54 @@ struct nb_ctx {
     int64_t nmask = 0;
     DevBuf<long long> counters;                // device counters (list statistics)
 
+    // --- device-side counts (nb_list.cu) ---
+    NbTotals* tot_dev = nullptr;               // device
+    NbTotals* tot_host = nullptr;              // pinned mirror, valid after the end-of-search synchronisation
+    bool cold = true;                          // no capacities known yet (first search, or after an overflow): stage by stage
+    int nsc_max = 0;                           // natoms/64 + columns: host-side bound of nsc, everything is sized and launched by it
+    int np2_col = 0;                           // shared-memory sort size of k_col_layout (power of two >= largest column, with head-room)
+    size_t cap_jslots = 0, cap_units = 0, cap_masks = 0, cap_il = 0, cap_ilm = 0;   // what the list buffers hold
+    bool stats_dirty = true;                   // list statistics are computed lazily in nb_get_stats
+    bool planes_dirty = false;                 // plane_inner (introspection only) is stale with respect to the compact inner list
+
     // --- work units (a5) ---
-    std::vector<int4> h_units;
-    DevBuf<int4> units_canon, units_sorted;    // {entry slot, batch begin, batch end, sci}
-    DevBuf<int32_t> unit_order;                // canonical unit index, longest first (force kernel launch order)
-    // prune launch order: (canonical unit*8 + i-cluster), each rolling part longest list first; one
-    // cached table per recently used nparts, rebuilt lazily after a search
-    struct PruneOrder { int nparts = 0; int64_t search = -1; DevBuf<int32_t> d; std::vector<int32_t> h; };
+    DevBuf<int4> units_canon;                  // {entry slot, batch begin, batch end, sci}, canonical order (rolling parts are ranges of it)
+    DevBuf<int32_t> unit_nsplit, unit_off;     // [nent] scan scratch
+    int nunits = 0;
+    // prune launch order per nparts: segment ids (positions in the force kernel's order), each rolling part
+    // longest list first; one cached table per recently used nparts, rebuilt lazily after a search
+    struct PruneOrder { int nparts = 0; int64_t search = -1; DevBuf<int32_t> d; };
     PruneOrder prune_orders[4];
     int prune_order_next = 0;
-    std::vector<int32_t> h_unit_order, h_seg_sorted, h_seg_pos;   // host copies made at search time (sources of async uploads)
+    DevBuf<int32_t> sort_hist;                 // [parts * NB_SEG_MAXKEY] counting-sort buckets
+    DevBuf<int32_t> seg_len;                   // [nunits*8] by s0: sort key of the launch orders (outer list length)
     float dummy_box[3] = {0, 0, 0};            // box the dummy clusters were last written for
     const void* dummy_at = nullptr;            // ... and where
-    int nunits = 0;
 
-    // --- compact inner list (a6 -> a7): per (work unit, i-cluster) the j-clusters whose inner mask bit is set ---
-    DevBuf<int32_t> il_off, ilm_off;           // [nunits*8] scan scratch: first entry of the segment in il / ilm
-    DevBuf<int4> seg;                          // [nunits*8], one per (work unit, i-cluster), longest outer list first:
-                                               // {il offset, ilm offset, unmasked half-cluster entries (multiple of 8), masked entries}
-    DevBuf<int32_t> unit_pos;                  // canonical unit index -> launch position (inverse of unit_order)
-    DevBuf<int32_t> seg_pos;                   // [nunits*8] (unit launch position*8 + i-cluster) -> index into seg (longest first)
-    DevBuf<int2> seg_ci;                       // [nunits*8] {i-cluster, shift id} of each seg entry
-    size_t il_total = 0, ilm_total = 0;        // allocated extents of il / ilm in use (sum of segment capacities)
-    int nseg_launch = 0;                       // seg entries with a non-empty outer list (= force kernel grid)
-    std::vector<int32_t> h_caps;               // host scratch
-    DevBuf<int32_t> il;                        // cj of cluster pairs without a mask for this i-cluster
-    DevBuf<int2> ilm;                          // {cj, mask ref} of cluster pairs with a mask, plus each segment's tail
-    // compact OUTER list (a3 -> a6): what the prune kernel streams; written once per search
-    DevBuf<int2> ol;                           // {cj, unit-local joint slot}; segment at il offset + ilm offset: the cluster pairs
-                                               // without a mask, then (from a multiple of 4 on) those with a mask
-    DevBuf<int2> ol_cnt;                       // [nunits*8] {unmasked, masked} entries per segment (index: unit launch position*8 + i-cluster)
+    // --- compact lists (a3 -> a6 -> a7), per (work unit, i-cluster) SEGMENT ---
+    // s0 = canonical unit * 8 + i-cluster names a segment at search time; t = its position in the force
+    // kernel's launch order (longest outer list first) names it everywhere afterwards.
+    DevBuf<int32_t> il_off, ilm_off;           // [nunits*8] by s0: first entry of the segment in il / ilm (scan output)
+    DevBuf<int32_t> seg_of_s0;                 // [nunits*8] s0 -> t
+    DevBuf<int4> segd;                         // [nunits*8] by t: {il offset, ilm offset, i-cluster | shift id << 26, canonical unit}
+    DevBuf<int2> ol_cnt;                       // [nunits*8] by t: OUTER {cluster pairs without a mask, with a mask}
+    DevBuf<int2> seg_cnt[2];                   // [nunits*8] by t: INNER {half-cluster entries (multiple of 8), masked cluster pairs}
+    DevBuf<int32_t> olu;                       // OUTER list, cluster pairs without a mask: cj, segment at il offset; written once per search
+    DevBuf<int2> olm;                          // OUTER list, cluster pairs with a mask: {cj, mask ref}, segment at ilm offset
+    DevBuf<int32_t> il[2];                     // INNER list: surviving half j-clusters 2*cj + half (+ dummies up to a multiple of 8)
+    DevBuf<int2> ilm[2];                       // INNER list: surviving masked cluster pairs {cj, mask ref}
+    // Two inner buffers: nb_prune_overlapped writes the part it prunes into the buffer the force kernel is
+    // NOT reading and the part flips at the next nb_put_atoms.  Bit p of bufmask = buffer holding part p
+    // (parts as in buf_nparts); 0 everywhere unless the overlapped mode is in use.
+    unsigned bufmask = 0;
+    int buf_nparts = 1;
+    bool have_buf1 = false;
+    int pending_part = -1;                     // overlapped prune in flight on side_stream (its part), else -1
+    cudaStream_t side_stream = nullptr;
+    cudaEvent_t ev_main = nullptr, ev_side = nullptr;
+    size_t il_total = 0, ilm_total = 0;        // extents of il / ilm in use
+    int nseg_launch = 0;                       // segments with a non-empty outer list (= force kernel grid)
+    DevBuf<float4> ljrow;                      // [nclusters_max * 4 * (ntypes+1)] paired LJ rows per i-cluster (nb_force.cu), written at search
     DevBuf<double> fshift;                     // [27*3] per-shift i-force sums (virial)
 
     // --- per-stage device timing (nb_timing_enable / nb_timing_read) ---
@@ -235,32 +273,20 @@ __device__ __forceinline__ void nb_ilist_finish(int nu, int nm, int salt, int la
     if (lane == 0) *cnt = make_int2(nu, nm);
 }
 
-// Writes the compact inner list segment of (unit, i-cluster warp) from the unit's inner mask
-// words `bits_of(b)` (b = batch index relative to the unit), keeping BOTH halves of every
-// cluster (used after a search: inner := outer).  Entries whose exclusion mask is trivial for
-// this i-cluster go to `il` (two half-cluster indices), the others to `ilm` {cj, mask ref}.
-// One warp, all 32 lanes.
-template <typename BitsOf>
-__device__ __forceinline__ void nb_ilist_write(BitsOf bits_of, int b0, int b1, int warp, int lane, int cj_dummy,
-                                               const uint32_t* __restrict__ plane_excl, const int2* __restrict__ jl,
-                                               int32_t* __restrict__ il, int2* __restrict__ ilm, int2* __restrict__ cnt)
+// Rolling part of a canonical work unit: part p of k is the range [p*nu/k, (p+1)*nu/k) (reading A15).
+__host__ __device__ __forceinline__ int nb_part_of_unit(int u, int nparts, int nunits)
 {
-    const unsigned lt = (1u << lane) - 1u;
-    int nu = 0, nm = 0;
-    for (int b = b0; b < b1; b++) {
-        const unsigned bits = bits_of(b - b0);
-        const unsigned eb = plane_excl[(size_t)b * 8 + warp] & bits, nb = bits & ~eb;
-        if ((bits >> lane) & 1u) {
-            const int2 e = jl[(size_t)b * 32 + lane];
-            if ((nb >> lane) & 1u)
-                *reinterpret_cast<int2*>(&il[nu + 2 * __popc(nb & lt)]) = make_int2(2 * e.x, 2 * e.x + 1);
-            else ilm[nm + __popc(eb & lt)] = e;
-        }
-        nu += 2 * __popc(nb);
-        nm += __popc(eb);
-    }
-    __syncwarp();
-    nb_ilist_finish(nu, nm, b0 * 8 + warp, lane, cj_dummy, il, ilm, cnt);
+    if (nparts <= 1) return 0;
+    int p = (int)(((long long)u * nparts) / nunits);
+    if (p > nparts - 1) p = nparts - 1;
+    while (p + 1 < nparts && ((long long)(p + 1) * nunits) / nparts <= u) p++;
+    while (p > 0 && ((long long)p * nunits) / nparts > u) p--;
+    return p;
+}
+// Which of the two inner-list buffers holds the segment of canonical unit u (nb_ctx::bufmask).
+__device__ __forceinline__ int nb_seg_buf(int u, unsigned bufmask, int nparts, int nunits)
+{
+    return bufmask ? (int)((bufmask >> nb_part_of_unit(u, nparts, nunits)) & 1u) : 0;
 }
 #endif
 
@@ -284,12 +310,19 @@ int nbi_refresh_xq(nb_ctx* c);                             // (a1) nb_grid.cu
 int nbi_put_device(nb_ctx* c, const float* x, const float* q, const int32_t* type, bool refresh);   // (a1) nb_grid.cu
 int nbi_search(nb_ctx* c, float rlist);                    // (a3)-(a5) nb_list.cu
 int nbi_prune(nb_ctx* c, float rlist_inner, int part, int nparts);   // (a6) nb_prune.cu
-int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial);   // (a7)-(a8) nb_force.cu
+int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial, float rlist_inner_fused = 0.f);   // (a7)-(a8) nb_force.cu
 int nbi_list_count(nb_ctx* c, int which, int64_t* n);      // nb_list.cu
 int nbi_list_dump(nb_ctx* c, int which, int32_t* ci, int32_t* cj, int32_t* shift, uint64_t* pairmask,
                   int32_t* part);
 int nbi_measure_fp32_peak(nb_ctx* c, double* fma_per_s);   // nb_force.cu
 int nbi_count_pairs(nb_ctx* c, int64_t* n_interacting, int64_t* n_excluded);   // nb_force.cu
 int nbi_count_slots(nb_ctx* c, int64_t* slots);            // nb_force.cu
-int nbi_inner_dump(nb_ctx* c, int64_t* n, int32_t* ci, int32_t* entry, int32_t* shift, int32_t* kind);   // nb_force.cu
+int nbi_inner_dump(nb_ctx* c, int64_t* n, int32_t* ci, int32_t* entry, int32_t* shift, int32_t* kind, int32_t* part);   // nb_force.cu
+int nbi_prune_overlapped(nb_ctx* c, float rlist_inner, int part, int nparts);   // nb_prune.cu
+int nbi_commit_pending(nb_ctx* c);                          // nb_prune.cu: join an overlapped prune and flip its part
+int nbi_consolidate(nb_ctx* c);                             // nb_prune.cu: move every segment back to inner buffer 0
+int nbi_rebuild_inner_planes(nb_ctx* c);                    // nb_list.cu: plane_inner from the compact inner list (introspection)
+int nbi_list_stats(nb_ctx* c);                              // nb_list.cu: lazily computed list statistics
+int nbi_prune_order(nb_ctx* c, int nparts, const int32_t** table);   // nb_list.cu: prune launch order for nparts rolling parts
+int nbi_ljrows(nb_ctx* c);                                  // nb_force.cu: paired LJ rows per i-cluster, at search time
 int nbi_exclusive_scan(nb_ctx* c, const int32_t* in, int32_t* out, int64_t n, int32_t* total_dev);  // nb_list.cu

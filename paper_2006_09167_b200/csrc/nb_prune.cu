@@ -3,17 +3,21 @@
 // "A particle-pair distance based list pruning is carried out on the GPU which
 // eliminates non-interacting cluster pairs"; L193: dual pair list, "frequent pruning steps
 // produce a pair list based on the inner cut-off ... pruning is done in a rolling fashion
-// scheduled in chunks between force computations".
+// scheduled in chunks between force computations ... which allows it to overlap other work".
 //
-// The outer masks are never modified; every prune of a part restarts from them (atoms move
-// both ways) and rewrites the inner mask words of that part only (reading A15).  Part p of k
-// is the contiguous range [p*nu/k, (p+1)*nu/k) of the canonically ordered work units.
-// Block = 8 warps = the 8 i-clusters of one super-cluster (one work unit); warp w owns the
-// bit-plane w of the unit's mask words, so no cross-warp combination is needed.  Lanes own
-// j atoms: 4 j-clusters x 8 atoms per step, the 8 i-atoms live in registers.  The set bits of
-// the outer plane words are compacted into a per-warp queue (as in the force kernel), so every
-// step but the unit's last is full, and the j coordinates of the next step are loaded before
-// the current step's arithmetic.
+// The outer list is never modified; every prune of a part restarts from it (atoms move both ways)
+// and rewrites the inner list segments of that part only (reading A15).  Part p of k is the
+// contiguous range [p*nu/k, (p+1)*nu/k) of the canonically ordered work units.
+// One thread block = one warp = one SEGMENT (one i-cluster of one work unit): it streams the
+// segment's compact outer list (nb_list.cu k_ilist_build: plain cj for the cluster pairs without a
+// mask, {cj, mask ref} for those with one), 4 j-clusters per step, lanes own j atoms, the 8 i atoms
+// live in registers as packed pairs; ONE ballot per step gives the surviving halves (or clusters),
+// which the leader lanes append to the inner list segment the force kernel streams.
+//
+// Two ways to schedule it: nb_prune enqueues the kernel on the context's stream (the next nb_forces
+// sees its result); nb_prune_overlapped runs it on a second stream next to the force kernel of the
+// same step, writing into the inner-list buffer the force kernel is not reading; the part flips to the
+// new buffer at the next nb_put_atoms.
 #include "nb_internal.h"
 
 #include <algorithm>
@@ -21,25 +25,21 @@
 namespace {
 
 struct PruneArgs {
-    const int4* units;        // canonical order
-    const int* order;         // launch order of this part: canonical unit indices, longest first
-    const int2* jl;
-    const uint32_t* plane_outer;
-    const int2* ol;           // compact outer list (nb_list.cu k_ilist_build)
+    const int* order;         // launch order of this part: segment ids, longest outer list first
+    const int4* segd;
     const int2* ol_cnt;
-    uint32_t* plane_inner;
+    const int32_t* olu;       // compact outer list (nb_list.cu k_ilist_build)
+    const int2* olm;
     const float4* xq;
     float box[3];
-    float rl2;   // fl32(rlist_inner^2), reading A12
-    // compact inner list written for the force kernel (nb_internal.h)
-    int u0;      // canonical index of units[0]
+    float rl2;                // fl32(rlist_inner^2), reading A12
     int cj_dummy;
-    const uint32_t* plane_excl;
-    const int* unit_pos;
-    const int* seg_pos;
-    int4* seg;
-    int32_t* il;
-    int2* ilm;
+    // inner list written for the force kernel (nb_internal.h): buffer `wbuf` when the segment's part bit says so
+    int32_t* il[2];
+    int2* ilm[2];
+    int2* seg_cnt[2];
+    unsigned wmask;           // bit p: part p is written into buffer 1
+    int nparts, nunits;
 };
 
 // 8 exact (A12) distance checks of this lane's j atom against the i atoms (packed pairs 2p, 2p+1:
@@ -65,74 +65,61 @@ __device__ __forceinline__ bool prune_checks(const float2 (&xi)[4], const float2
     return found;
 }
 
-// One survivor-append step: 4 j-clusters (lane groups), entry e = {cj, unit-local joint slot | masked << 30}.
-struct PruneState {
-    int nu, nm;
-};
-
 // One step over 4 cluster pairs WITHOUT a mask: a half j-cluster (4 atoms) survives iff one of its
 // atoms is within rlist_inner of an i atom; the survivors' half-cluster indices are appended to il.
-__device__ __forceinline__ void prune_step_unmasked(const PruneArgs& A, const float2 (&xi)[4], const float2 (&yi)[4],
-                                                    const float2 (&zi)[4], const int2 e, const float4 x, const bool valid,
-                                                    const int lane, unsigned* res, int32_t* il, PruneState& st)
+__device__ __forceinline__ void prune_step_unmasked(const float2 (&xi)[4], const float2 (&yi)[4], const float2 (&zi)[4],
+                                                    const float rl2, const int cj, const float4 x, const bool valid,
+                                                    const int lane, int32_t* __restrict__ il, int& nu)
 {
-    const bool found = prune_checks<false>(xi, yi, zi, x, A.rl2, false, 0);
+    const bool found = prune_checks<false>(xi, yi, zi, x, rl2, false, 0);
     const unsigned gm = __ballot_sync(0xffffffffu, found && valid);
     unsigned hm = gm | (gm >> 1);
     hm = (hm | (hm >> 2)) & 0x11111111u;          // bit 4h: half h of the step (lanes 4h..4h+3) has a survivor
-    if ((hm >> lane) & 1u) {                      // its leader lane (lane % 4 == 0)
-        il[st.nu + __popc(hm & ((1u << lane) - 1u))] = 2 * e.x + ((lane >> 2) & 1);
-        if ((lane & 4) == 0 || !((hm >> (lane - 4)) & 1u)) atomicOr(&res[e.y >> 5], 1u << (e.y & 31));   // once per cluster
-    }
-    st.nu += __popc(hm);
+    if ((hm >> lane) & 1u)                        // its leader lane (lane % 4 == 0)
+        il[nu + __popc(hm & ((1u << lane) - 1u))] = 2 * cj + ((lane >> 2) & 1);
+    nu += __popc(hm);
 }
 
 // One step over 4 cluster pairs WITH a mask (exclusions, or the zero-shift diagonal pair, which keeps
 // only atom pairs b > a): whole clusters, appended to ilm with their mask reference.
-__device__ __forceinline__ void prune_step_masked(const PruneArgs& A, const float2 (&xi)[4], const float2 (&yi)[4],
-                                                  const float2 (&zi)[4], const int2 e, const float4 x, const bool valid,
-                                                  const bool diag, const int b0, const int lane, unsigned* res, int2* ilm,
-                                                  PruneState& st)
+__device__ __forceinline__ void prune_step_masked(const float2 (&xi)[4], const float2 (&yi)[4], const float2 (&zi)[4],
+                                                  const float rl2, const int2 e, const float4 x, const bool valid,
+                                                  const bool diag, const int lane, int2* __restrict__ ilm, int& nm)
 {
-    const int g = lane >> 3, k = lane & 7;
-    const bool found = prune_checks<true>(xi, yi, zi, x, A.rl2, diag, k);
+    const int k = lane & 7;
+    const bool found = prune_checks<true>(xi, yi, zi, x, rl2, diag, k);
     const unsigned gm = __ballot_sync(0xffffffffu, found && valid);
     unsigned cm = gm | (gm >> 1);
     cm |= cm >> 2;
     cm = (cm | (cm >> 4)) & 0x01010101u;          // bit 8g: cluster pair g of the step survives
-    if ((cm >> lane) & 1u) {
-        atomicOr(&res[e.y >> 5], 1u << (e.y & 31));
-        ilm[st.nm + __popc(cm & ((1u << lane) - 1u))] = make_int2(e.x, A.jl[(size_t)b0 * 32 + e.y].y);
-    }
-    st.nm += __popc(cm);
+    if ((cm >> lane) & 1u) ilm[nm + __popc(cm & ((1u << lane) - 1u))] = e;
+    nm += __popc(cm);
 }
 
-// One warp per block = one i-cluster of one work unit: streams its compact outer list segment.
+// One warp per block = one segment: streams its compact outer list.
 __global__ void __launch_bounds__(32) k_prune(PruneArgs A)
 {
-    __shared__ unsigned s_res[NB_MAX_UNIT_BATCHES];   // inner mask words of this i-cluster's plane
-    const int sidx = A.order[blockIdx.x];   // canonical unit * 8 + i-cluster, longest list first within the part
-    const int ucan = sidx >> 3, warp = sidx & 7;
-    const int4 u = A.units[ucan];
+    const int t = A.order[blockIdx.x];
+    const int2 n = A.ol_cnt[t];             // {cluster pairs without a mask, with a mask}
+    if (n.x + n.y == 0) return;             // (an empty outer segment has an empty inner one, set at search time)
+    const int4 sd = A.segd[t];
     const int lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7;
-    const int sci = u.w, h = u.x - sci * NB_NHALF, ci = sci * 8 + warp;
-    const int s0 = A.unit_pos[ucan] * 8 + warp;
-    int4* sg = &A.seg[A.seg_pos[s0]];
-    const int2 off = *reinterpret_cast<const int2*>(sg);
-    const int2 n = A.ol_cnt[s0];            // {cluster pairs without a mask, with a mask}
-    const int2* __restrict__ ol = A.ol + off.x + off.y;
-    int32_t* il = A.il + off.x;
-    int2* ilm = A.ilm + off.y;
+    const int ci = sd.z & 0x3ffffff, sid = sd.z >> 26;
+    const int wb = A.wmask ? (int)((A.wmask >> nb_part_of_unit(sd.w, A.nparts, A.nunits)) & 1u) : 0;
+    const int32_t* __restrict__ olu = A.olu + sd.x;
+    const int2* __restrict__ olm = A.olm + sd.y;
+    int32_t* il = A.il[wb] + sd.x;
+    int2* ilm = A.ilm[wb] + sd.y;
     const int ns = (n.x + 3) >> 2;
-    int2 ea = make_int2(ci, 0), eb = ea, ea2 = ea, eb2 = ea;
+    int ea = ci, eb = ci, ea2 = ci, eb2 = ci;
     if (ns > 0) {
-        ea = ol[min(g, n.x - 1)];
-        eb = ol[min(4 + g, n.x - 1)];
-        ea2 = ol[min(8 + g, n.x - 1)];
-        eb2 = ol[min(12 + g, n.x - 1)];
+        ea = olu[min(g, n.x - 1)];
+        eb = olu[min(4 + g, n.x - 1)];
+        ea2 = olu[min(8 + g, n.x - 1)];
+        eb2 = olu[min(12 + g, n.x - 1)];
     }
     int sx, sy, sz;
-    nb_shift_vec(nb_half_shift_id(h), sx, sy, sz);
+    nb_shift_vec(sid, sx, sy, sz);
     float2 xi[4], yi[4], zi[4];
 #pragma unroll
     for (int p = 0; p < 4; p++) {
@@ -142,92 +129,171 @@ __global__ void __launch_bounds__(32) k_prune(PruneArgs A)
         yi[p] = make_float2(__fmaf_rn((float)sy, A.box[1], v0.y), __fmaf_rn((float)sy, A.box[1], v1.y));
         zi[p] = make_float2(__fmaf_rn((float)sz, A.box[2], v0.z), __fmaf_rn((float)sz, A.box[2], v1.z));
     }
-    unsigned* res = s_res;
-    if (lane < NB_MAX_UNIT_BATCHES) res[lane] = 0u;
-    __syncwarp();
-    PruneState st = {0, 0};
+    int nu = 0, nm = 0;
     // cluster pairs with a mask: few (about one step per zero-shift segment), no pipeline
-    const int mbase = (n.x + 3) & ~3;
     for (int s = 0; s < n.y; s += 4) {
         const bool valid = s + g < n.y;
-        const int2 e = ol[mbase + min(s + g, n.y - 1)];
+        const int2 e = olm[min(s + g, n.y - 1)];
         const float4 x = A.xq[e.x * 8 + k];
-        prune_step_masked(A, xi, yi, zi, e, x, valid, e.x == ci && h == 0, u.y, lane, res, ilm, st);
+        prune_step_masked(xi, yi, zi, A.rl2, e, x, valid, e.x == ci && sid == NB_SHIFT_CENTER, lane, ilm, nm);
     }
     if (ns > 0) {
         // two alternating register sets (a: even steps, b: odd steps); j coordinates two steps ahead,
         // list entries four steps ahead, indices clamped to the segment (as in the force kernel)
-        float4 xa = A.xq[ea.x * 8 + k], xb = A.xq[eb.x * 8 + k];
+        float4 xa = A.xq[ea * 8 + k], xb = A.xq[eb * 8 + k];
         int s = 0;
         for (; s + 1 < ns; s += 2) {
-            prune_step_unmasked(A, xi, yi, zi, ea, xa, 4 * s + g < n.x, lane, res, il, st);
+            prune_step_unmasked(xi, yi, zi, A.rl2, ea, xa, 4 * s + g < n.x, lane, il, nu);
             ea = ea2;
-            xa = A.xq[ea.x * 8 + k];
-            ea2 = ol[min(4 * (s + 4) + g, n.x - 1)];
-            prune_step_unmasked(A, xi, yi, zi, eb, xb, 4 * (s + 1) + g < n.x, lane, res, il, st);
+            xa = A.xq[ea * 8 + k];
+            ea2 = olu[min(4 * (s + 4) + g, n.x - 1)];
+            prune_step_unmasked(xi, yi, zi, A.rl2, eb, xb, 4 * (s + 1) + g < n.x, lane, il, nu);
             eb = eb2;
-            xb = A.xq[eb.x * 8 + k];
-            eb2 = ol[min(4 * (s + 5) + g, n.x - 1)];
+            xb = A.xq[eb * 8 + k];
+            eb2 = olu[min(4 * (s + 5) + g, n.x - 1)];
         }
-        if (s < ns) prune_step_unmasked(A, xi, yi, zi, ea, xa, 4 * s + g < n.x, lane, res, il, st);
+        if (s < ns) prune_step_unmasked(xi, yi, zi, A.rl2, ea, xa, 4 * s + g < n.x, lane, il, nu);
     }
     __syncwarp();
-    nb_ilist_finish(st.nu, st.nm, u.y * 8 + warp, lane, A.cj_dummy, il, ilm, reinterpret_cast<int2*>(sg) + 1);
-    if (lane < u.z - u.y) A.plane_inner[(size_t)(u.y + lane) * 8 + warp] = res[lane];
+    nb_ilist_finish(nu, nm, sd.x + ci, lane, A.cj_dummy, il, ilm, &A.seg_cnt[wb][t]);
+}
+
+// Copies the segments that live in inner buffer 1 back to buffer 0 (one warp per segment).
+__global__ void k_consolidate(int nseg, const int4* __restrict__ segd, unsigned bufmask, int nparts, int nunits,
+                              const int2* __restrict__ cnt1, int2* __restrict__ cnt0, const int32_t* __restrict__ il1,
+                              int32_t* __restrict__ il0, const int2* __restrict__ ilm1, int2* __restrict__ ilm0)
+{
+    const int t = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (t >= nseg) return;
+    const int4 sd = segd[t];
+    if (!nb_seg_buf(sd.w, bufmask, nparts, nunits)) return;
+    const int2 cnt = cnt1[t];
+    for (int e = lane; e < cnt.x; e += 32) il0[sd.x + e] = il1[sd.x + e];
+    for (int e = lane; e < cnt.y; e += 32) ilm0[sd.y + e] = ilm1[sd.y + e];
+    if (lane == 0) cnt0[t] = cnt;
+}
+
+int launch_prune(nb_ctx* c, float rlist_inner, int part, int nparts, unsigned wmask, cudaStream_t st)
+{
+    const long long nu = c->nunits;
+    const int u0 = (int)((long long)part * nu / nparts), u1 = (int)((long long)(part + 1) * nu / nparts);
+    if (u1 <= u0) return NB_OK;
+    const int32_t* order = nullptr;
+    int rc = nbi_prune_order(c, nparts, &order);   // (built on the context's stream, before anything below is enqueued)
+    if (rc != NB_OK) return rc;
+    PruneArgs A;
+    A.order = order + (size_t)u0 * 8;
+    A.segd = c->segd.p;
+    A.ol_cnt = c->ol_cnt.p;
+    A.olu = c->olu.p;
+    A.olm = c->olm.p;
+    A.xq = c->xq.p;
+    for (int k = 0; k < 3; k++) A.box[k] = c->box[k];
+    A.rl2 = rlist_inner * rlist_inner;
+    A.cj_dummy = c->nclusters_max;
+    for (int b = 0; b < 2; b++) {
+        A.il[b] = c->il[b].p;
+        A.ilm[b] = c->ilm[b].p;
+        A.seg_cnt[b] = c->seg_cnt[b].p;
+    }
+    A.wmask = wmask;
+    A.nparts = nparts;
+    A.nunits = c->nunits;
+    k_prune<<<(u1 - u0) * 8, 32, 0, st>>>(A);
+    NB_LAUNCH_CHECK(c);
+    return NB_OK;
+}
+
+// The parts of the two-buffer scheme are those of buf_nparts; a call with another nparts first moves
+// every segment back to buffer 0.
+int set_buf_nparts(nb_ctx* c, int nparts)
+{
+    if (c->buf_nparts == nparts) return NB_OK;
+    int rc = nbi_consolidate(c);
+    if (rc != NB_OK) return rc;
+    c->buf_nparts = nparts;
+    return NB_OK;
 }
 
 }  // namespace
 
+int nbi_consolidate(nb_ctx* c)
+{
+    int rc = nbi_commit_pending(c);
+    if (rc != NB_OK) return rc;
+    if (c->bufmask && c->nseg_launch > 0) {
+        k_consolidate<<<(c->nseg_launch * 32 + 255) / 256, 256, 0, c->stream>>>(
+            c->nseg_launch, c->segd.p, c->bufmask, c->buf_nparts, c->nunits, c->seg_cnt[1].p, c->seg_cnt[0].p, c->il[1].p,
+            c->il[0].p, c->ilm[1].p, c->ilm[0].p);
+        NB_LAUNCH_CHECK(c);
+    }
+    c->bufmask = 0;
+    return NB_OK;
+}
+
+// Joins an overlapped prune: the context's stream waits for it, and its part flips to the buffer it wrote.
+int nbi_commit_pending(nb_ctx* c)
+{
+    if (c->pending_part < 0) return NB_OK;
+    NB_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_side, 0));
+    c->bufmask ^= 1u << c->pending_part;
+    c->pending_part = -1;
+    c->planes_dirty = true;
+    return NB_OK;
+}
+
 int nbi_prune(nb_ctx* c, float rlist_inner, int part, int nparts)
 {
-    const long long nu = c->nunits;
-    const int u0 = (int)((long long)part * nu / nparts), u1 = (int)((long long)(part + 1) * nu / nparts);
+    int rc = nbi_commit_pending(c);
+    if (rc != NB_OK) return rc;
+    if (nparts > 32 && c->bufmask) {
+        if ((rc = nbi_consolidate(c)) != NB_OK) return rc;
+    }
+    if (c->bufmask || nparts <= 32) {
+        if ((rc = set_buf_nparts(c, nparts <= 32 ? nparts : 1)) != NB_OK) return rc;
+    }
     c->last_nparts = nparts;
     c->st.prune_count++;
-    if (u1 <= u0) return NB_OK;
-    // Launch order inside each rolling part: longest i-cluster list first, so that the last
-    // wave of blocks is made of short lists.  Derived in one pass from the force kernel's global
-    // longest-first order (made at search time); cached per nparts until the next search.
-    nb_ctx::PruneOrder* po = nullptr;
-    for (auto& e : c->prune_orders)
-        if (e.nparts == nparts && e.search == c->st.search_count) po = &e;
-    if (!po) {
-        po = &c->prune_orders[c->prune_order_next];
-        c->prune_order_next = (c->prune_order_next + 1) % 4;
-        std::vector<int32_t> fill(nparts), part_of(nu);
-        for (int p = 0; p < nparts; p++) {
-            const long long a = (long long)p * nu / nparts, b = (long long)(p + 1) * nu / nparts;
-            fill[p] = (int)(a * 8);
-            for (long long i = a; i < b; i++) part_of[i] = p;
-        }
-        po->h.resize(nu * 8);
-        for (long long t = 0; t < nu * 8; t++) {
-            const int s0 = c->h_seg_sorted[t], ucan = c->h_unit_order[s0 >> 3];
-            po->h[fill[part_of[ucan]]++] = ucan * 8 + (s0 & 7);
-        }
-        NB_CUDA(c, po->d.ensure(nu * 8, c->stream));
-        NB_CUDA(c, cudaMemcpyAsync(po->d.p, po->h.data(), sizeof(int) * nu * 8, cudaMemcpyHostToDevice, c->stream));
-        po->nparts = nparts;
-        po->search = c->st.search_count;
-    }
-    PruneArgs A;
-    A.units = c->units_canon.p;
-    A.order = po->d.p + (size_t)u0 * 8;
-    A.jl = c->jl.p;
-    A.plane_outer = c->plane_outer.p;
-    A.ol = c->ol.p;
-    A.ol_cnt = c->ol_cnt.p;
-    A.plane_inner = c->plane_inner.p;
-    A.xq = c->xq.p;
-    for (int k = 0; k < 3; k++) A.box[k] = c->box[k];
-    A.rl2 = rlist_inner * rlist_inner;
-    A.u0 = u0;
-    A.cj_dummy = c->nclusters;
-    A.plane_excl = c->plane_excl.p;
-    A.unit_pos = c->unit_pos.p; A.seg_pos = c->seg_pos.p; A.seg = c->seg.p;
-    A.il = c->il.p; A.ilm = c->ilm.p;
+    c->planes_dirty = true;
     NbStageTimer tm(c, NB_T_PRUNE);
-    k_prune<<<(u1 - u0) * 8, 32, 0, c->stream>>>(A);
-    NB_LAUNCH_CHECK(c);
+    // in place: each part is rewritten in the buffer it lives in
+    return launch_prune(c, rlist_inner, part, nparts, c->bufmask, c->stream);
+}
+
+int nbi_prune_overlapped(nb_ctx* c, float rlist_inner, int part, int nparts)
+{
+    int rc = nbi_commit_pending(c);
+    if (rc != NB_OK) return rc;
+    if (nparts > 32) return nb_fail(c, NB_ERR_ARG, "nb_prune_overlapped: at most 32 rolling parts (got %d)", nparts);
+    cudaStream_t st = c->stream;
+    if (!c->side_stream) {
+        // lower priority than the caller's stream: the prune fills what the force kernel leaves free
+        int lo = 0, hi = 0;
+        NB_CUDA(c, cudaDeviceGetStreamPriorityRange(&lo, &hi));
+        NB_CUDA(c, cudaStreamCreateWithPriority(&c->side_stream, cudaStreamNonBlocking, lo));
+        NB_CUDA(c, cudaEventCreateWithFlags(&c->ev_main, cudaEventDisableTiming));
+        NB_CUDA(c, cudaEventCreateWithFlags(&c->ev_side, cudaEventDisableTiming));
+    }
+    if (!c->have_buf1) {
+        NB_CUDA(c, c->il[1].ensure(c->il[0].cap, st));
+        NB_CUDA(c, c->ilm[1].ensure(c->ilm[0].cap, st));
+        NB_CUDA(c, c->seg_cnt[1].ensure(c->seg_cnt[0].cap, st));
+        c->have_buf1 = true;
+    }
+    if ((rc = set_buf_nparts(c, nparts)) != NB_OK) return rc;
+    c->last_nparts = nparts;
+    c->st.prune_count++;
+    const int32_t* order = nullptr;
+    if ((rc = nbi_prune_order(c, nparts, &order)) != NB_OK) return rc;   // on the main stream, before the fork
+    // fork: the side stream sees everything enqueued so far (the coordinates of the last nb_put_atoms)
+    NB_CUDA(c, cudaEventRecord(c->ev_main, st));
+    NB_CUDA(c, cudaStreamWaitEvent(c->side_stream, c->ev_main, 0));
+    // the part is written into the buffer it does NOT live in
+    const unsigned wmask = c->bufmask ^ (1u << part);
+    rc = launch_prune(c, rlist_inner, part, nparts, wmask, c->side_stream);
+    if (rc != NB_OK) return rc;
+    NB_CUDA(c, cudaEventRecord(c->ev_side, c->side_stream));
+    const long long nu = c->nunits;
+    if ((int)((long long)(part + 1) * nu / nparts) > (int)((long long)part * nu / nparts)) c->pending_part = part;
     return NB_OK;
 }

@@ -24,8 +24,8 @@ NB_SHIFT_CENTER = 13
 EXPORTS = ["nb_init", "nb_put_atoms", "nb_put_atoms_host", "nb_search", "nb_prune", "nb_forces",
            "nb_forces_host", "nb_free", "nb_last_error", "nb_get_layout", "nb_get_slots", "nb_list_count",
            "nb_list_dump", "nb_get_stats", "nb_measure_fp32_peak", "nb_count_pairs", "nb_timing_enable",
-           "nb_timing_read", "nb_timing_stages", "nb_count_slots", "nb_inner_dump"]
-NB_T_NAMES = ["put", "grid", "search", "masks", "prune", "force", "reduce"]
+           "nb_timing_read", "nb_timing_stages", "nb_count_slots", "nb_inner_dump", "nb_prune_overlapped", "nb_forces_prune"]
+NB_T_NAMES = ["put", "grid", "search", "masks", "prune", "force", "reduce", "force_energy"]
 
 
 class nb_params(C.Structure):
@@ -33,7 +33,7 @@ class nb_params(C.Structure):
                 ("excl_off", C.c_void_p), ("excl_idx", C.c_void_p), ("rc", C.c_float),
                 ("coulomb", C.c_int32), ("ewald_beta", C.c_float), ("ewald_rtol", C.c_float),
                 ("eps_rf", C.c_float), ("epsfac", C.c_float), ("lj_modifier", C.c_int32),
-                ("coul_modifier", C.c_int32), ("device", C.c_int32), ("stream", C.c_void_p)]
+                ("coul_modifier", C.c_int32), ("device", C.c_int32), ("stream", C.c_void_p), ("rc_vdw", C.c_float)]
 
 
 class nb_stats(C.Structure):
@@ -84,7 +84,7 @@ class Context:
 
     def __init__(self, natoms, lj_c6c12, excl_off, excl_idx, rc, coulomb="ewald", ewald_beta=0.0,
                  ewald_rtol=1e-5, eps_rf=0.0, epsfac=0.0, lj_modifier=NB_MOD_POTSHIFT,
-                 coul_modifier=NB_MOD_POTSHIFT, device=0, stream=None):
+                 coul_modifier=NB_MOD_POTSHIFT, device=0, stream=None, rc_vdw=0.0):
         import torch
         self._torch = torch
         self.natoms = int(natoms)
@@ -99,7 +99,7 @@ class Context:
         p = nb_params(self.natoms, self.ntypes, _hptr(lj), _hptr(eo), _hptr(ei), float(rc),
                       {"ewald": NB_COUL_EWALD, "rf": NB_COUL_RF, "none": NB_COUL_NONE}[coulomb], float(ewald_beta), float(ewald_rtol),
                       float(eps_rf), float(epsfac), int(lj_modifier), int(coul_modifier), int(device),
-                      C.c_void_p(self.stream.cuda_stream))
+                      C.c_void_p(self.stream.cuda_stream), float(rc_vdw))
         self._h = C.c_void_p(0)
         rcode = lib().nb_init(C.byref(p), C.byref(self._h))
         if rcode != NB_OK:
@@ -137,9 +137,16 @@ class Context:
     def prune(self, rlist_inner, part=0, nparts=1):
         self._check(lib().nb_prune(self._h, C.c_float(rlist_inner), C.c_int(part), C.c_int(nparts)))
 
+    def prune_overlapped(self, rlist_inner, part=0, nparts=1):
+        self._check(lib().nb_prune_overlapped(self._h, C.c_float(rlist_inner), C.c_int(part), C.c_int(nparts)))
+
     def forces(self, f, energies=None, virial=None):
         """f [N,3] f32 CUDA tensor (overwritten); energies [2] f64, virial [9] f64 CUDA tensors or None."""
         self._check(lib().nb_forces(self._h, _dptr(f), _dptr(energies), _dptr(virial)))
+
+    def forces_prune(self, rlist_inner, f, energies=None, virial=None):
+        """The fused first prune: forces over the outer list + the whole inner list for rlist_inner in one kernel."""
+        self._check(lib().nb_forces_prune(self._h, C.c_float(rlist_inner), _dptr(f), _dptr(energies), _dptr(virial)))
 
     def forces_host(self, f, energies=None, virial=None):
         self._check(lib().nb_forces_host(self._h, _hptr(f), _hptr(energies), _hptr(virial)))
@@ -199,11 +206,11 @@ class Context:
 
     def inner_dump(self):
         """The compact inner list the force kernel streams: numpy arrays ci, entry, shift id, kind
-        (0: entry = half j-cluster index 2*cj + half; 1: entry = whole j-cluster with a mask)."""
+        (0: entry = half j-cluster index 2*cj + half; 1: entry = whole j-cluster with a mask), part."""
         n = C.c_int64()
         null = C.c_void_p(0)
-        self._check(lib().nb_inner_dump(self._h, C.byref(n), null, null, null, null))
-        arr = [np.zeros(max(n.value, 1), dtype=np.int32) for _ in range(4)]
+        self._check(lib().nb_inner_dump(self._h, C.byref(n), null, null, null, null, null))
+        arr = [np.zeros(max(n.value, 1), dtype=np.int32) for _ in range(5)]
         self._check(lib().nb_inner_dump(self._h, C.byref(n), *[_hptr(a) for a in arr]))
         return tuple(a[: n.value] for a in arr)
 

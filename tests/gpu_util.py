@@ -55,6 +55,11 @@ class Driver:
         ci, cj, sid, pm, part = self.ctx.list_dump(which)
         return ci, cj, self.nb.shift_vectors(sid), pm, part
 
+    def inner_dump(self):
+        """The compact half-cluster inner list: ci, entry, shift vectors, kind, part."""
+        ci, ent, sid, kind, part = self.ctx.inner_dump()
+        return ci, ent, self.nb.shift_vectors(sid), kind, part
+
 
 def rel_rms(f, ref):
     return float(np.sqrt(((f - ref) ** 2).sum() / (ref**2).sum()))

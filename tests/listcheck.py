@@ -33,11 +33,15 @@ def canonicalise(ci, cj, s, mask=None, C=8):
     return ci2, cj2, s2, np.where(flip, mt, m)
 
 
-def close_atom_pairs(atom_of_slot, xq, box, radius):
+def close_atom_pairs(atom_of_slot, xq, box, radius, subset=None):
     """All slot pairs (si<sj, valid atoms) with fp64 minimum-image distance < radius, with the
-    image vector s such that d = x_si + s L - x_sj is that minimum image."""
+    image vector s such that d = x_si + s L - x_sj is that minimum image.  `subset` (bool per slot)
+    restricts the search to pairs with BOTH atoms in it (a spatial sample of a large box)."""
     aos = np.asarray(atom_of_slot)
-    valid = np.nonzero(aos >= 0)[0]
+    ok = aos >= 0
+    if subset is not None:
+        ok = ok & np.asarray(subset)
+    valid = np.nonzero(ok)[0]
     box = np.asarray(box, dtype=np.float64)
     x = np.asarray(xq, dtype=np.float64).reshape(-1, 4)[valid, :3]
     xw = np.mod(x, box)
@@ -51,11 +55,24 @@ def close_atom_pairs(atom_of_slot, xq, box, radius):
     return si[keep], sj[keep], s[keep], dist[keep]
 
 
-def coverage_missing(atom_of_slot, xq, box, radius, ci, cj, s, C=8):
+def coverage_missing(atom_of_slot, xq, box, radius, ci, cj, s, C=8, subset=None):
     """Number of atom pairs closer than `radius` whose canonical cluster triple is NOT in the
     given triple set (must be 0 for a complete list), and the number of pairs checked."""
-    si, sj, sp, _ = close_atom_pairs(atom_of_slot, xq, box, radius)
+    si, sj, sp, _ = close_atom_pairs(atom_of_slot, xq, box, radius, subset)
     pci, pcj, ps = canonicalise(si // C, sj // C, sp)
     have = np.unique(triple_keys(*canonicalise(ci, cj, s)))
     need = triple_keys(pci, pcj, ps)
     return int((~np.isin(need, have)).sum()), int(need.size)
+
+
+def z_slab_subset(xq, box, z0, thickness):
+    """Slots whose wrapped z lies in [z0, z0 + thickness) modulo Lz (a slab; z0 + thickness > Lz makes it
+    straddle the periodic face, which exercises the shifted list entries)."""
+    z = np.mod(np.asarray(xq, dtype=np.float64).reshape(-1, 4)[:, 2] - z0, float(box[2]))
+    return z < thickness
+
+
+def half_entry_keys(ci, entry, s, kind):
+    """Unique int64 key per entry of the compact half-cluster inner list (same packing as oracle.HalfListResult.keys)."""
+    return ((np.asarray(ci).astype(np.int64) << 38) | (np.asarray(entry).astype(np.int64) << 9)
+            | (shift_id(s) << 1) | np.asarray(kind).astype(np.int64))

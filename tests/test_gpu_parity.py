@@ -84,6 +84,54 @@ def check_lists(d, w, rl_outer, rl_inner, c_range=None):
     return ref
 
 
+def spread_ranges(ncl, nranges, width):
+    """nranges cluster ranges of `width` clusters spread evenly over [0, ncl), the first and last touching the ends."""
+    starts = np.unique(np.linspace(0, max(ncl - width, 0), nranges).astype(int))
+    return [(int(a), int(min(a + width, ncl))) for a in starts]
+
+
+def check_half_list(d, w, c_ranges=None, part=None, before=None):
+    """The compact inner list the force kernel streams (nb_inner_dump) against oracle_half_lists on the
+    library's slot table at the CURRENT coordinates, bit-exact as sets (no guard band: both sides decide
+    in fp32 with the A12 operation order); no duplicates, no dummy entries.
+    c_ranges: compare only entries whose first or second cluster lies in one of the ranges (sampled check);
+    part: compare only the entries of this rolling part (the one just pruned) -- the other parts must be
+    what they were in `before` (a previous return value of this function: the keys of all entries)."""
+    aos, xq = d.slots()
+    ncl = aos.size // 8
+    ci, ent, s, kind, prt = d.inner_dump()
+    keys = LC.half_entry_keys(ci, ent, s, kind)
+    assert np.unique(keys).size == keys.size, "duplicate entry in the compact inner list"
+    cj = np.where(kind == 0, ent // 2, ent)
+    assert ent.size == 0 or (cj.max() < ncl and cj.min() >= 0 and ci.max() < ncl), "dummy or out-of-range entry leaked"
+    if part is not None:
+        # the oracle's entries of that part: the part of an entry is the part of its outer triple in the library's list
+        oci, ocj, os_, _, opart = d.dump(0)
+        okeys = LC.triple_keys(oci, ocj, os_)
+        order = np.argsort(okeys)
+        okeys, opart = okeys[order], opart[order]
+    for (c0, c1) in (c_ranges if c_ranges is not None else [(0, ncl)]):
+        ref = O.half_lists(aos, xq, w.box, w.rlist_outer, w.rlist_inner, w.excl_off, w.excl_idx, c_begin=c0, c_end=c1)
+        rkeys = ref.keys()
+        sel = ((ci >= c0) & (ci < c1)) | ((cj >= c0) & (cj < c1))
+        if part is not None:
+            rcj = np.where(ref.kind == 0, ref.entry // 2, ref.entry)
+            tk = LC.triple_keys(ref.ci, rcj, ref.s)
+            pos = np.searchsorted(okeys, tk)
+            assert (pos < okeys.size).all() and np.array_equal(okeys[pos], tk), "oracle inner entry outside the library's outer list"
+            rkeys = rkeys[opart[pos] == part]
+            sel &= prt == part
+        got, want = np.sort(keys[sel]), np.sort(rkeys)
+        assert got.size == want.size and np.array_equal(got, want), (c0, c1, part, got.size, want.size)
+    if part is not None and before is not None:
+        # label the earlier entries with TODAY's parts (through their outer triple) and compare the other parts
+        bci, bent, bsid, bkind = before >> 38, (before >> 9) & ((1 << 29) - 1), (before >> 1) & 0xFF, before & 1
+        btk = (bci << 36) | (np.where(bkind == 0, bent // 2, bent) << 8) | bsid
+        bpart = opart[np.searchsorted(okeys, btk)]
+        assert np.array_equal(np.sort(before[bpart != part]), np.sort(keys[prt != part])), "a prune changed another part"
+    return keys
+
+
 def test_config0_layout_lists_forces(cfg0):
     w = cfg0
     d = Driver(w)
@@ -118,7 +166,10 @@ def test_config0_layout_lists_forces(cfg0):
     assert rel_rms(f, img.f) <= TOL_F
     st = d.ctx.get_stats()
     assert st["n_pairs_inner"] == ref_l.inner.sum() and st["n_pairs_outer"] == ref_l.inner.size
-    assert st["slots_last_forces"] == 64 * st["n_pairs_inner"]
+    assert st["slots_last_forces"] == d.ctx.count_slots() < 64 * st["n_pairs_inner"]
+    hci, hent, _, hkind, _ = d.inner_dump()
+    assert st["slots_last_forces"] == 32 * int((hkind == 0).sum()) + 64 * int((hkind == 1).sum())
+    check_half_list(d, w)
     # mean number of set interaction-mask bits per joint entry: the paper's "approximately four of eight" (L135)
     assert 2.5 < st["n_pairs_outer"] / st["n_joint_outer"] < 6.5
 
@@ -241,11 +292,14 @@ def test_config1_parity_and_rolling_prune(cfg1):
     d.ctx.search(w.rlist_outer)
     check_layout(d, w)
     ref = oracle_forces(w, method="cells")
-    # full-size list parity on a sample of clusters (the oracle's all-pairs bb loop is O(n^2))
-    ncl = d.ctx.get_layout()["nclusters"]
+    # full-size list parity over ALL clusters (outer, inner, pair masks; then the half-cluster list the force kernel streams)
     d.ctx.prune(w.rlist_inner)
-    for c0 in (0, ncl // 2 + 3, ncl - 24):
-        check_lists(d, w, w.rlist_outer, w.rlist_inner, c_range=(c0, c0 + 24))
+    check_lists(d, w, w.rlist_outer, w.rlist_inner)
+    check_half_list(d, w)
+    aos, xq = d.slots()
+    ci, cj, s, _, _ = d.dump(1)
+    miss, n = LC.coverage_missing(aos, xq, w.box, w.rlist_inner - 1e-6, ci, cj, s)
+    assert miss == 0 and n > 5_000_000
     f, e, vir = d.forces(energy=True, virial=True)
     assert rel_rms(f, ref.f) <= TOL_F
     assert abs(e.sum() - ref.energy) / abs(ref.energy) <= TOL_E
@@ -263,7 +317,9 @@ def test_config1_parity_and_rolling_prune(cfg1):
     for a, b in zip(full[:4], rolled[:4]):
         assert np.array_equal(a, b)
     assert set(np.unique(rolled[4]).tolist()) == set(range(w.nparts))
-    # rolling over moving atoms (motion recipe): forces stay equal to the all-pairs oracle
+    # rolling over moving atoms (motion recipe): forces, energies and virial stay equal to the all-pairs oracle,
+    # the pruned part of the compact inner list is bit-exact against the oracle at the coordinates of the prune
+    hl = check_half_list(d, w)
     for t in (1, 2, 50, 99):
         x = w.positions_at(t)
         d.put(x)
@@ -275,7 +331,12 @@ def test_config1_parity_and_rolling_prune(cfg1):
         kb = LC.triple_keys(before[0], before[1], before[2])[before[4] != part]
         ka = LC.triple_keys(after[0], after[1], after[2])[after[4] != part]
         assert np.array_equal(kb, ka)
+        hl = check_half_list(d, w, part=part, before=hl)
         r = oracle_forces(w, x=x, method="cells")
+        f, e, vir = d.forces(energy=True, virial=True)
+        assert rel_rms(f, r.f) <= TOL_F
+        assert abs(e.sum() - r.energy) / abs(r.energy) <= TOL_E
+        assert np.linalg.norm(vir - r.virial) / np.linalg.norm(r.virial) <= TOL_E
         assert rel_rms(d.forces(), r.f) <= TOL_F
     # determinism (T16): same inputs, same dump
     d.put()
@@ -289,19 +350,46 @@ def test_config1_parity_and_rolling_prune(cfg1):
 @pytest.mark.parametrize("which", ["cfg2_ewald", "cfg2_rf", "cfg4", "cfg3"])
 def test_full_size_configs_in_bench_schedule(which):
     """BASELINE.json configs[2] (both Coulomb flavours), [4] and [3] at full size, driven the way bench.py
-    drives them (search, full prune, then rolling parts on the motion recipe): list parity on sampled
-    cluster ranges (the list oracle is O(n^2)), forces / energy / virial against the fp64 linked-cell
-    oracle (pinned equal to all-pairs), effective pair count against the oracle's."""
+    drives them (search, full prune, then rolling parts on the motion recipe).  Lists: config 2 Ewald over ALL
+    clusters (outer, inner, pair masks, and the half-cluster list the force kernel streams); the others on
+    >= 1 % of the clusters in >= 8 ranges (the list oracle is O(n^2)), config 4's ranges including the
+    slab/vapour boundaries; k-d-tree completeness of the inner list (whole box, or slabs of config 3 that
+    include the periodic face).  Forces / energy / virial against the fp64 linked-cell oracle (pinned equal to
+    all-pairs) at t = 0 and on moved frames after rolling prunes; effective pair count against the oracle's."""
     w = {"cfg2_ewald": lambda: W.config2("ewald"), "cfg2_rf": lambda: W.config2("rf"), "cfg4": W.config4,
          "cfg3": W.config3}[which]()
     d = Driver(w)
     d.put()
     d.ctx.search(w.rlist_outer)
-    check_layout(d, w)
+    aos, xq = check_layout(d, w)
     d.ctx.prune(w.rlist_inner)
     ncl = d.ctx.get_layout()["nclusters"]
-    for c0 in (0, ncl // 3 + 5, ncl - 16):
-        check_lists(d, w, w.rlist_outer, w.rlist_inner, c_range=(c0, c0 + 16))
+    if which == "cfg2_ewald":
+        ranges = None
+        check_lists(d, w, w.rlist_outer, w.rlist_inner)
+    else:
+        width = {"cfg2_rf": 16, "cfg4": 24, "cfg3": 176}[which]
+        ranges = spread_ranges(ncl, 8, width)
+        if which == "cfg4":
+            # clusters at the two slab/vapour interfaces (x ~ 0 = 36.2 and x ~ 18.1): where cluster occupancy and list lengths jump
+            xc = np.nanmean(np.where((aos >= 0)[:, None], xq[:, :3], np.nan).reshape(-1, 8, 3)[:, :, 0], axis=1)
+            for x0 in (18.1, 0.3):
+                c = int(np.nanargmin(np.abs(xc - x0)))
+                ranges.append((max(c - 12, 0), min(c + 12, ncl)))
+        assert sum(b - a for a, b in ranges) >= 0.01 * ncl and len(ranges) >= 8
+        for r in ranges:
+            check_lists(d, w, w.rlist_outer, w.rlist_inner, c_range=r)
+    hl = check_half_list(d, w, c_ranges=ranges)
+    # layout-independent completeness of the inner list (k-d tree, fp64)
+    ci, cj, s, _, _ = d.dump(1)
+    if which == "cfg2_ewald":
+        miss, n = LC.coverage_missing(aos, xq, w.box, w.rlist_inner - 1e-6, ci, cj, s)
+        assert miss == 0 and n > 20_000_000
+    else:
+        for z0 in (3.0, float(w.box[2]) - 1.2):   # one slab inside the box, one across the periodic face
+            sub = LC.z_slab_subset(xq, w.box, z0, 2.4)
+            miss, n = LC.coverage_missing(aos, xq, w.box, w.rlist_inner - 1e-6, ci, cj, s, subset=sub)
+            assert miss == 0 and n > 3_000_000
     ref = oracle_forces(w, method="cells")
     f, e, vir = d.forces(energy=True, virial=True)
     assert rel_rms(f, ref.f) <= TOL_F
@@ -311,42 +399,51 @@ def test_full_size_configs_in_bench_schedule(which):
     assert abs(npairs - ref.npairs) <= 2 + 1e-6 * ref.npairs     # fp32 vs fp64 at r = rc
     fsum = np.abs(f.sum(axis=0)).max() / (np.sqrt((f**2).mean()) * w.natoms)
     assert fsum < 1e-6                                           # T6 on the GPU
-    for t in (1, 2, w.nparts + 1):
+    sample = ranges if ranges is not None else spread_ranges(ncl, 8, 32)
+    for t in (1, 2, w.nparts + 1, 50, 99) if which != "cfg3" else (1, w.nparts + 1, 99):
         x = w.positions_at(t)
         d.put(x)
-        d.ctx.prune(w.rlist_inner, t % w.nparts, w.nparts)
+        part = t % w.nparts
+        d.ctx.prune(w.rlist_inner, part, w.nparts)
+        # the pruned part of the compact list against the oracle at THESE coordinates (config 2 Ewald: all clusters at t = 1)
+        hl = check_half_list(d, w, c_ranges=None if (which == "cfg2_ewald" and t == 1) else sample, part=part,
+                             before=hl if which != "cfg3" else None)
         r = oracle_forces(w, x=x, method="cells")
+        if t in (1, 99):
+            f, e, vir = d.forces(energy=True, virial=True)     # energies and virial on a moved frame after a rolling prune
+            assert abs(e.sum() - r.energy) / abs(r.energy) <= TOL_E
+            assert np.linalg.norm(vir - r.virial) / np.linalg.norm(r.virial) <= TOL_E
+            assert rel_rms(f, r.f) <= TOL_F
         assert rel_rms(d.forces(), r.f) <= TOL_F
 
 
 @pytest.mark.parametrize("which", ["cfg0", "rect_rf", "lj"])
 def test_half_cluster_inner_list(which):
     """The compact inner list the force kernel streams is kept at half-j-cluster granularity (DESIGN.md
-    section 5).  Layout-independent check in fp64 on the library's own slot table, with a 1e-6 nm guard band
-    around rlist_inner (the kernel decides in fp32): COMPLETE -- every atom pair closer than rlist_inner
-    is covered by a listed half-cluster of the other atom's cluster or by a masked cluster pair -- and
-    MINIMAL -- every listed half has an atom within rlist_inner of the i-cluster; the cluster pairs it
-    spans are exactly the inner list of nb_list_dump."""
+    section 5).  Bit-exact against oracle_half_lists after a full prune and after rolling parts on moved
+    coordinates; layout-independent fp64 check (k-d tree) that it is COMPLETE; the cluster pairs it spans
+    are exactly the inner list of nb_list_dump (which is derived from it)."""
     w = {"cfg0": W.config0, "lj": lambda: W.lj_fluid(12, rc=0.9),
          "rect_rf": lambda: W.small_water(150, 2.0, seed=21, rc=0.8, rlist_outer=0.9, rlist_inner=0.84,
                                           box_scale=(1.0, 1.1, 1.25), coulomb="rf")}[which]()
     d = Driver(w)
     d.put()
     d.ctx.search(w.rlist_outer)
-    for x, part, nparts in ((None, 0, 1), (w.positions_at(40), 0, 2), (w.positions_at(40), 1, 2)):
+    d.ctx.prune(w.rlist_inner, 0, 1)
+    hl = check_half_list(d, w)
+    for x, part, nparts in ((w.positions_at(40), 0, 2), (w.positions_at(41), 1, 2), (w.positions_at(42), 0, 2)):
         d.put(x)
         d.ctx.prune(w.rlist_inner, part, nparts)
+        hl = check_half_list(d, w, part=part, before=hl)
     aos, xq = d.slots()
     box = np.asarray(w.box, dtype=np.float64)
-    ci, ent, sid, kind = d.ctx.inner_dump()
-    svec = d.nb.shift_vectors(sid).astype(np.int64)
+    ci, ent, svec, kind, _ = d.inner_dump()
     half = kind == 0
     skey = LC.shift_id(svec)
     hkeys = set(zip(ci[half].tolist(), ent[half].tolist(), skey[half].tolist()))
     mkeys = set(zip(ci[~half].tolist(), ent[~half].tolist(), skey[~half].tolist()))
-    assert len(hkeys) == int(half.sum()) and len(mkeys) == int((~half).sum())      # no duplicates
-    # complete
-    si, sj, sp, _ = LC.close_atom_pairs(aos, xq, box, w.rlist_inner - 1e-6)
+    # complete for the CURRENT coordinates at rc (parts pruned at earlier frames keep what was within rlist_inner then)
+    si, sj, sp, _ = LC.close_atom_pairs(aos, xq, box, w.rc)
     ka, kb = LC.shift_id(sp), LC.shift_id(-sp)
     missing = 0
     for a, b, k1, k2 in zip(si.tolist(), sj.tolist(), ka.tolist(), kb.tolist()):
@@ -355,21 +452,119 @@ def test_half_cluster_inner_list(which):
             continue
         missing += 1
     assert missing == 0 and si.size > 1000
-    # minimal: every listed half has a real atom within rlist_inner (+ guard) of a real atom of ci
-    x = np.asarray(xq, dtype=np.float64).reshape(-1, 4)[:, :3]
-    real = np.asarray(aos) >= 0
-    hci, hent, hs = ci[half], ent[half], svec[half]
-    xi = x[hci[:, None] * 8 + np.arange(8)[None, :]] + (hs * box)[:, None, :]           # [n,8,3], shift on the i side
-    xj = x[hent[:, None] * 4 + np.arange(4)[None, :]]                                   # [n,4,3]
-    d2 = ((xi[:, :, None, :] - xj[:, None, :, :]) ** 2).sum(-1)
-    ok = real[hci[:, None] * 8 + np.arange(8)[None, :]][:, :, None] & real[hent[:, None] * 4 + np.arange(4)[None, :]][:, None, :]
-    dmin = np.sqrt(np.where(ok, d2, np.inf).min(axis=(1, 2)))
-    assert (dmin < w.rlist_inner + 1e-6).all()
     # same cluster pairs as the bit-plane inner list
     dci, dcj, dsv, _, _ = d.dump(1)
     planes = set(zip(dci.tolist(), dcj.tolist(), LC.shift_id(dsv).tolist()))
     spanned = {(a, e // 2, k) for a, e, k in hkeys} | mkeys
     assert spanned == planes
+
+
+def test_overlapped_prune(cfg1):
+    """nb_prune_overlapped: the prune of a rolling part runs on the library's second stream next to the force
+    kernel and the part switches to the new list at the next nb_put_atoms.  Forces of the step that issued
+    it still come from the previous list; after the switch the part is bit-exact against the oracle ON THE
+    COORDINATES THE PRUNE SAW, the other parts are untouched; forces / energies stay equal to the oracle over
+    a run that alternates parts; plain nb_prune and a change of nparts in between keep everything consistent."""
+    w = cfg1
+    d = Driver(w)
+    d.put()
+    d.ctx.search(w.rlist_outer)
+    d.ctx.prune(w.rlist_inner)
+    hl = check_half_list(d, w)
+    k = w.nparts
+    for t in range(1, 8):
+        x = w.positions_at(t)
+        d.put(x)                                     # joins the prune of step t-1: its part flips here
+        if t > 1:
+            # the part pruned at t-1 must equal the oracle at x_{t-1}; check by putting x_{t-1} back for the comparison only
+            d.put(w.positions_at(t - 1))
+            hl = check_half_list(d, w, c_ranges=spread_ranges(d.ctx.get_layout()["nclusters"], 6, 24), part=(t - 1) % k, before=hl)
+            d.put(x)
+        d.ctx.prune_overlapped(w.rlist_inner, t % k, k)
+        f, e, vir = d.forces(energy=True, virial=True)
+        r = oracle_forces(w, x=x, method="cells")
+        assert rel_rms(f, r.f) <= TOL_F
+        assert abs(e.sum() - r.energy) / abs(r.energy) <= TOL_E
+        assert np.linalg.norm(vir - r.virial) / np.linalg.norm(r.virial) <= TOL_E
+    # a plain prune of the other part while one part lives in the second buffer, then a different nparts
+    x = w.positions_at(8)
+    d.put(x)
+    cur = check_half_list(d, w, c_ranges=[(0, 0)])   # (nothing compared: just the current entries)
+    d.ctx.prune(w.rlist_inner, 0, k)
+    hl = check_half_list(d, w, part=0, before=cur)
+    assert rel_rms(d.forces(), oracle_forces(w, x=x, method="cells").f) <= TOL_F
+    d.ctx.prune_overlapped(w.rlist_inner, 2, 3)
+    assert rel_rms(d.forces(), oracle_forces(w, x=x, method="cells").f) <= TOL_F
+    d.put(x)
+    hl = check_half_list(d, w, part=2)
+    d.ctx.prune(w.rlist_inner)                       # full prune: everything back in one buffer
+    check_half_list(d, w)
+    assert rel_rms(d.forces(), oracle_forces(w, x=x, method="cells").f) <= TOL_F
+
+
+@pytest.mark.parametrize("which", ["cfg0", "cfg1", "rect_rf", "lj"])
+def test_fused_first_prune(which):
+    """nb_forces_prune -- one kernel walks the OUTER list of a fresh search,
+    computes forces (+ energies, virial) and writes the inner list.  The list it writes is bit-equal to
+    nb_prune's and to the oracle's half-cluster list; forces / energies / virial within 1e-5 of the oracle,
+    in every flavour {Ewald, RF, LJ-only} x {F, F+E+virial}; the steps after it run on its list."""
+    w = {"cfg0": W.config0, "cfg1": W.config1, "lj": lambda: W.lj_fluid(12, rc=0.9),
+         "rect_rf": lambda: W.small_water(150, 2.0, seed=21, rc=0.8, rlist_outer=0.9, rlist_inner=0.84,
+                                          box_scale=(1.0, 1.1, 1.25), coulomb="rf")}[which]()
+    method = "cells" if which == "cfg1" else "allpairs"
+    ref = oracle_forces(w, method=method)
+    d = Driver(w)
+    d.put()
+    d.ctx.search(w.rlist_outer)
+    d.ctx.prune(w.rlist_inner)
+    by_prune = np.sort(LC.half_entry_keys(*d.inner_dump()[:4]))
+    for energy in (False, True):
+        d.ctx.search(w.rlist_outer)
+        d.f.fill_(float("nan"))
+        d.ctx.forces_prune(w.rlist_inner, d.f, d.e if energy else None, d.v if energy else None)
+        d.torch.cuda.synchronize()
+        f = d.f.cpu().numpy().astype(np.float64)
+        assert rel_rms(f, ref.f) <= TOL_F
+        if energy:
+            e, vir = d.e.cpu().numpy(), d.v.cpu().numpy().reshape(3, 3)
+            assert abs(e.sum() - ref.energy) / abs(ref.energy) <= TOL_E
+            assert np.linalg.norm(vir - ref.virial) / np.linalg.norm(ref.virial) <= TOL_E
+        fused = check_half_list(d, w)                                   # bit-exact against the oracle ...
+        assert np.array_equal(np.sort(fused), by_prune)                 # ... and against the separate prune kernel
+        assert rel_rms(d.forces(), ref.f) <= TOL_F                      # the next step runs on the list it wrote
+    x = w.positions_at(3)
+    d.put(x)
+    d.ctx.prune(w.rlist_inner, 1 % w.nparts, w.nparts)
+    assert rel_rms(d.forces(), oracle_forces(w, x=x, method=method).f) <= TOL_F
+    st = d.ctx.get_stats()
+    assert st["prune_count"] == 4 and st["search_count"] == 3
+
+
+@pytest.mark.parametrize("coulomb", ["ewald", "rf"])
+def test_twin_cutoffs(coulomb):
+    """SURVEY 8.1 (f4), PAPER.md L205 / L215: rc_vdw < rc (electrostatics cut-off scaled up by PME load balancing).
+    Forces, both energies and the virial against the oracle's twin cut-off reading, plain and fused-prune flavours."""
+    w = W.small_water(150, 2.0, seed=21, rc=0.9, rlist_outer=0.98, rlist_inner=0.93, box_scale=(1.0, 1.1, 1.25), coulomb=coulomb)
+    rcv = 0.7
+    p = O.Params(rc=w.rc, ntypes=w.ntypes, coulomb=coulomb, beta=O.beta_from_rtol(w.rc, w.ewald_rtol) if coulomb == "ewald" else 0.0,
+                 rc_vdw=rcv)
+    ref = O.forces(w.x, w.q, w.type, w.box, w.lj_c6c12, w.excl_off, w.excl_idx, p)
+    single = oracle_forces(w)
+    assert abs(ref.e_lj - single.e_lj) > 1e-3 * abs(single.e_lj)       # the second cut-off matters on this box
+    d = Driver(w, rc_vdw=rcv)
+    d.put()
+    d.ctx.search(w.rlist_outer)
+    d.ctx.forces_prune(w.rlist_inner, d.f, d.e, d.v)
+    d.torch.cuda.synchronize()
+    for f, e, vir in ((d.f.cpu().numpy().astype(np.float64), d.e.cpu().numpy(), d.v.cpu().numpy().reshape(3, 3)),
+                      d.forces(energy=True, virial=True)):
+        assert rel_rms(f, ref.f) <= TOL_F
+        assert abs(e[0] - ref.e_lj) <= TOL_E * abs(ref.energy) and abs(e[1] - ref.e_coul) <= TOL_E * abs(ref.energy)
+        assert np.linalg.norm(vir - ref.virial) / np.linalg.norm(ref.virial) <= TOL_E
+    assert rel_rms(d.forces(), ref.f) <= TOL_F
+    from paper_2006_09167_b200 import nb
+    with pytest.raises(nb.NbError):
+        nb.context_for(w, rc_vdw=1.0)                                  # rc_vdw > rc
 
 
 def test_work_efficiency_table_against_oracle():
@@ -519,7 +714,7 @@ def test_pair_count_and_stage_timing(cfg0):
     d.forces(energy=True, virial=True)
     t = d.ctx.timing_read()
     assert t["put"][1] == 2 and t["grid"][1] == 1 and t["search"][1] == 1 and t["masks"][1] == 1
-    assert t["prune"][1] == 1 and t["force"][1] == 2 and t["reduce"][1] == 2
+    assert t["prune"][1] == 1 and t["force"][1] == 1 and t["force_energy"][1] == 1 and t["reduce"][1] == 2
     assert all(v[0] > 0 for v in t.values())
     t2 = d.ctx.timing_read()
     assert all(v == (0.0, 0) for v in t2.values())
