@@ -245,6 +245,8 @@ __global__ void __launch_bounds__(32, PRUNE ? 8 : 16) k_force(ForceArgs A)
         cj = entry(0) * APE + k4;              // unmasked path: cj* hold this lane's j SLOT
         cj_n = entry(min(1, ns - 1)) * APE + k4;
     }
+    // ... and so is the first step of the masked loop (its loads chain entry -> atoms -> mask)
+    int2 ce_next = g < cnt.y ? ilm[g] : make_int2(ci, 0);
     int sx, sy, sz;
     nb_shift_vec(sid, sx, sy, sz);
     IAtoms I;
@@ -273,7 +275,8 @@ __global__ void __launch_bounds__(32, PRUNE ? 8 : 16) k_force(ForceArgs A)
     // unmasked one was measured slower.)
     for (int s = 0; s < cnt.y; s += 4) {
         const bool valid = s + g < cnt.y;
-        const int2 ce = valid ? ilm[s + g] : make_int2(ci, 0);
+        const int2 ce = ce_next;
+        if (s + 4 < cnt.y) ce_next = s + 4 + g < cnt.y ? ilm[s + 4 + g] : make_int2(ci, 0);
         const float4 xm = A.xq[ce.x * 8 + k];
         const int tm = A.type_slot[ce.x * 8 + k];
         const ulonglong2 mm = *reinterpret_cast<const ulonglong2*>(&A.masks[((size_t)ce.y * 8 + warp) * 2]);

@@ -10,8 +10,7 @@ the C ABI; efficiency = atom pairs with r < rc (any exclusion status, counted by
 list) / (64 x listed cluster pairs).  Two cluster numbers are printed: the searched list (bounding-box
 predicate, what the paper's CPU search produces) and the list after a prune at the same rlist (atom
 distances, the dual-list inner list).  The 1x1 reference is the ideal-gas ratio (rc / rlist)^3.
-The tolerance-based Verlet-buffer estimate of L159-L161 needs masses, temperature and constraints,
-which this path does not have: not built.
+The tolerance-based Verlet-buffer estimate of L159-L161 is paper_2006_09167_b200/verlet_buffer.py.
 """
 from __future__ import annotations
 
