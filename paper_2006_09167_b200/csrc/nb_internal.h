@@ -148,6 +148,7 @@ struct nb_ctx {
     // --- device-side counts (nb_list.cu) ---
     NbTotals* tot_dev = nullptr;               // device
     NbTotals* tot_host = nullptr;              // pinned mirror, valid after the end-of-search synchronisation
+    int nsm = 148;                             // multiprocessors of the device (persistent kernels are sized by it)
     bool cold = true;                          // no capacities known yet (first search, or after an overflow): stage by stage
     int nsc_max = 0;                           // natoms/64 + columns: host-side bound of nsc, everything is sized and launched by it
     int np2_col = 0;                           // shared-memory sort size of k_col_layout (power of two >= largest column, with head-room)
@@ -186,12 +187,16 @@ struct nb_ctx {
     // (parts as in buf_nparts); 0 everywhere unless the overlapped mode is in use.
     unsigned bufmask = 0;
     int buf_nparts = 1;
+    int seg_part_nparts = 0;
+    int64_t seg_part_search = -1;              // what seg_part was last computed for
+    DevBuf<int32_t> seg_part;                  // [nunits*8] by t: rolling part of the segment under buf_nparts (read only while bufmask != 0)
     bool have_buf1 = false;
     int pending_part = -1;                     // overlapped prune in flight on side_stream (its part), else -1
     cudaStream_t side_stream = nullptr;
     cudaEvent_t ev_main = nullptr, ev_side = nullptr;
     size_t il_total = 0, ilm_total = 0;        // extents of il / ilm in use
     int nseg_launch = 0;                       // segments with a non-empty outer list (= force kernel grid)
+    DevBuf<int32_t> ticket;                    // [1] work counter of the persistent force kernel, zero between launches
     DevBuf<float4> ljrow;                      // [nclusters_max * 4 * (ntypes+1)] paired LJ rows per i-cluster (nb_force.cu), written at search
     DevBuf<double> fshift;                     // [27*3] per-shift i-force sums (virial)
 

@@ -38,8 +38,7 @@ struct PruneArgs {
     int32_t* il[2];
     int2* ilm[2];
     int2* seg_cnt[2];
-    unsigned wmask;           // bit p: part p is written into buffer 1
-    int nparts, nunits;
+    int wb;                   // inner buffer this part is written into (all segments of a launch belong to one part)
 };
 
 // 8 exact (A12) distance checks of this lane's j atom against the i atoms (packed pairs 2p, 2p+1:
@@ -105,7 +104,7 @@ __global__ void __launch_bounds__(32) k_prune(PruneArgs A)
     const int4 sd = A.segd[t];
     const int lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7;
     const int ci = sd.z & 0x3ffffff, sid = sd.z >> 26;
-    const int wb = A.wmask ? (int)((A.wmask >> nb_part_of_unit(sd.w, A.nparts, A.nunits)) & 1u) : 0;
+    const int wb = A.wb;
     const int32_t* __restrict__ olu = A.olu + sd.x;
     const int2* __restrict__ olm = A.olm + sd.y;
     int32_t* il = A.il[wb] + sd.x;
@@ -158,6 +157,13 @@ __global__ void __launch_bounds__(32) k_prune(PruneArgs A)
     nb_ilist_finish(nu, nm, sd.x + ci, lane, A.cj_dummy, il, ilm, &A.seg_cnt[wb][t]);
 }
 
+// Rolling part of every segment under `nparts`, looked up by the force kernel while some part lives in inner buffer 1.
+__global__ void k_seg_parts(int nseg, const int4* __restrict__ segd, int nparts, int nunits, int32_t* __restrict__ seg_part)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < nseg) seg_part[t] = nb_part_of_unit(segd[t].w, nparts, nunits);
+}
+
 // Copies the segments that live in inner buffer 1 back to buffer 0 (one warp per segment).
 __global__ void k_consolidate(int nseg, const int4* __restrict__ segd, unsigned bufmask, int nparts, int nunits,
                               const int2* __restrict__ cnt1, int2* __restrict__ cnt0, const int32_t* __restrict__ il1,
@@ -196,9 +202,7 @@ int launch_prune(nb_ctx* c, float rlist_inner, int part, int nparts, unsigned wm
         A.ilm[b] = c->ilm[b].p;
         A.seg_cnt[b] = c->seg_cnt[b].p;
     }
-    A.wmask = wmask;
-    A.nparts = nparts;
-    A.nunits = c->nunits;
+    A.wb = part < 32 ? (int)((wmask >> part) & 1u) : 0;   // (more than 32 parts only without the two-buffer scheme: wmask = 0)
     k_prune<<<(u1 - u0) * 8, 32, 0, st>>>(A);
     NB_LAUNCH_CHECK(c);
     return NB_OK;
@@ -208,10 +212,21 @@ int launch_prune(nb_ctx* c, float rlist_inner, int part, int nparts, unsigned wm
 // every segment back to buffer 0.
 int set_buf_nparts(nb_ctx* c, int nparts)
 {
-    if (c->buf_nparts == nparts) return NB_OK;
-    int rc = nbi_consolidate(c);
-    if (rc != NB_OK) return rc;
-    c->buf_nparts = nparts;
+    if (c->buf_nparts != nparts) {
+        int rc = nbi_consolidate(c);
+        if (rc != NB_OK) return rc;
+        c->buf_nparts = nparts;
+    }
+    if (c->seg_part_nparts != nparts || c->seg_part_search != c->st.search_count) {
+        const int nseg = c->nunits * 8;
+        NB_CUDA(c, c->seg_part.ensure(std::max(nseg, 1), c->stream));
+        if (nseg > 0) {
+            k_seg_parts<<<(nseg + 255) / 256, 256, 0, c->stream>>>(nseg, c->segd.p, nparts, c->nunits, c->seg_part.p);
+            NB_LAUNCH_CHECK(c);
+        }
+        c->seg_part_nparts = nparts;
+        c->seg_part_search = c->st.search_count;
+    }
     return NB_OK;
 }
 
