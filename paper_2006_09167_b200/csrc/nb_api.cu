@@ -141,8 +141,6 @@ extern "C" int nb_init(const nb_params* p, nb_ctx** out)
     NB_CUDA(c, cudaMallocHost((void**)&c->tot_host, sizeof(NbTotals)));
     memset(c->tot_host, 0, sizeof(NbTotals));
     NB_CUDA(c, cudaMemsetAsync(c->tot_dev, 0, sizeof(NbTotals), st));
-    NB_CUDA(c, c->ticket.ensure(1, st));
-    NB_CUDA(c, cudaMemsetAsync(c->ticket.p, 0, sizeof(int32_t), st));
     NB_CUDA(c, cudaStreamSynchronize(st));   // host staging vectors go out of scope
     return NB_OK;
 }
@@ -296,7 +294,7 @@ extern "C" void nb_free(nb_ctx* c)
     c->fshift.release(); c->unit_nsplit.release(); c->unit_off.release(); c->sort_hist.release(); c->seg_len.release();
     for (auto& po : c->prune_orders) po.d.release();
     c->il_off.release(); c->ilm_off.release(); c->seg_of_s0.release(); c->segd.release(); c->ol_cnt.release();
-    c->olu.release(); c->olm.release(); c->ljrow.release(); c->seg_part.release(); c->ticket.release();
+    c->olu.release(); c->olm.release(); c->ljrow.release(); c->seg_part.release();
     for (int b = 0; b < 2; b++) { c->seg_cnt[b].release(); c->il[b].release(); c->ilm[b].release(); }
     delete c;
 }

@@ -37,8 +37,7 @@ struct ForceArgs {
     const int* il[2];
     const int2* ilm[2];
     unsigned bufmask;           // which inner buffer each rolling part lives in (nb_prune_overlapped), 0 = all in buffer 0
-    const int32_t* seg_part;    // rolling part of every segment (read only while bufmask != 0)
-    int* ticket;                // work counter of the persistent kernel; zero between launches (the gather resets it)
+    const int32_t* seg_part;    // rolling part of every segment under buf_nparts (read only while bufmask != 0)
     int nparts, nunits;
     // the fused first prune (k_force<..., PRUNE = true>): outer list in, inner list (buffer 0) out
     const int2* ol_cnt;
@@ -217,7 +216,8 @@ __global__ void __launch_bounds__(32, PRUNE ? 8 : 16) k_force(ForceArgs A)
     const NbConst& K = A.kc;
     const int lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7;
     const int4 sd = A.segd[blockIdx.x];
-    const int buf = PRUNE ? 0 : nb_seg_buf(sd.w, A.bufmask, A.nparts, A.nunits);
+    // (the part comes from a table written when nparts changes: deriving it from the unit index costs a 64-bit division)
+    const int buf = PRUNE || !A.bufmask ? 0 : (int)((A.bufmask >> A.seg_part[blockIdx.x]) & 1u);
     // PRUNE: outer counts {cluster pairs without a mask, with a mask}; else inner {half entries, masked pairs}
     const int2 cnt = PRUNE ? A.ol_cnt[blockIdx.x] : A.seg_cnt[buf][blockIdx.x];
     const int ci = sd.z & 0x3ffffff, sid = sd.z >> 26, warp = ci & 7;
@@ -387,279 +387,6 @@ __global__ void __launch_bounds__(32, PRUNE ? 8 : 16) k_force(ForceArgs A)
     if ((lane & 3) == 0) red_add_v4(&A.f4[ci * 8 + (lane >> 2)], fi[0], fi[1], fi[2]);
 }
 
-// ---------------------------------------------------------------- the persistent force kernel
-// Asynchronous copies global -> shared (LDGSTS): the data lands in shared memory without passing through
-// registers and without stalling the issuing warp; cp_async_wait_all() + __syncwarp() make it visible.
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
-{
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async8(void* smem, const void* gmem)
-{
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async4(void* smem, const void* gmem)
-{
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all()
-{
-    asm volatile("cp.async.wait_all;" ::: "memory");
-    __syncwarp();
-}
-
-// What a warp needs to START a segment, staged in shared memory while it still works on the previous one
-// (followed by the paired LJ rows of the i-cluster, double-buffered: the rows of the segment being worked
-// on are read from shared memory in every step).
-struct SegStage {
-    int4 segd;                 // stage 1: the segment descriptor, the inner counts in both buffers, the rolling part
-    int2 cnt[2];
-    int part, pad[3];
-    float4 iat[8];             // stage 2 (needs the descriptor): the i atoms,
-    int ilh[32];               //   the first 32 half-cluster entries (4 steps),
-    int2 ilmh[4];              //   the first 4 masked cluster pairs
-    float4 xs[2][32];          // stage 3 (needs the entries): j atoms of the first two unmasked steps,
-    int ts[2][32];
-    float4 xm[32];             //   j atoms and masks of the first masked step
-    int tm[32];
-    ulonglong2 mk[32];
-};
-
-__device__ __forceinline__ void seg_stage1(const ForceArgs& A, SegStage& S, int seg, int lane)
-{
-    if (lane == 0) cp_async16(&S.segd, &A.segd[seg]);
-    if (lane == 1) cp_async8(&S.cnt[0], &A.seg_cnt[0][seg]);
-    if (A.bufmask) {
-        if (lane == 2) cp_async8(&S.cnt[1], &A.seg_cnt[1][seg]);
-        if (lane == 3) cp_async4(&S.part, &A.seg_part[seg]);
-    }
-}
-__device__ __forceinline__ void seg_stage2(const ForceArgs& A, SegStage& S, float4* lj, int ljn, int lane)
-{
-    const int4 sd = S.segd;
-    const int buf = A.bufmask ? (int)((A.bufmask >> S.part) & 1u) : 0;
-    const int2 cnt = S.cnt[buf];
-    const int ci = sd.z & 0x3ffffff;
-    if (lane < 8) cp_async16(&S.iat[lane], &A.xq[ci * 8 + lane]);
-    for (int i = lane; i < ljn; i += 32) cp_async16(&lj[i], &A.ljrow[(size_t)ci * ljn + i]);
-    if (4 * lane < min(cnt.x, 32)) cp_async16(&S.ilh[4 * lane], A.il[buf] + sd.x + 4 * lane);   // (counts are multiples of 8)
-    if (lane < min(cnt.y, 4)) cp_async8(&S.ilmh[lane], A.ilm[buf] + sd.y + lane);
-}
-__device__ __forceinline__ void seg_stage3(const ForceArgs& A, SegStage& S, int lane)
-{
-    const int buf = A.bufmask ? (int)((A.bufmask >> S.part) & 1u) : 0;
-    const int2 cnt = S.cnt[buf];
-    const int ci = S.segd.z & 0x3ffffff, ns = cnt.x >> 3;
-    if (ns > 0) {
-#pragma unroll
-        for (int st = 0; st < 2; st++) {
-            const int slot = S.ilh[8 * min(st, ns - 1) + (lane >> 2)] * 4 + (lane & 3);
-            cp_async16(&S.xs[st][lane], &A.xq[slot]);
-            cp_async4(&S.ts[st][lane], &A.type_slot[slot]);
-        }
-    }
-    if (cnt.y > 0) {
-        const int g = lane >> 3;
-        const int2 ce = g < cnt.y ? S.ilmh[g] : make_int2(ci, 0);
-        const int slot = ce.x * 8 + (lane & 7);
-        cp_async16(&S.xm[lane], &A.xq[slot]);
-        cp_async4(&S.tm[lane], &A.type_slot[slot]);
-        cp_async16(&S.mk[lane], &A.masks[((size_t)ce.y * 8 + (ci & 7)) * 2]);
-    }
-}
-
-// The force kernel over the inner list.  PERSISTENT warps: the grid is one warp per register-file slot
-// (16 per SM), warp b works through the segments b, b + G, b + 2G, ... of the longest-first order -- with
-// sorted lengths this round-robin deal balances the warps to within one segment.  While a warp is in the
-// step loop of one segment it stages what the NEXT one needs to start (SegStage: three dependent rounds of
-// asynchronous copies, issued at the start, five steps and two steps before the end of the loop), so that the
-// chain descriptor -> list entries -> j atoms, which cost a block-per-segment kernel about half of its
-// warp-time (ncu source view, profiles/r2a), is paid while the FP32 pipe is busy.
-template <int COUL, bool ENERGY, bool TWIN>
-__global__ void __launch_bounds__(32, 16) k_force_ps(ForceArgs A, int nseg)
-{
-    extern __shared__ __align__(16) unsigned char s_raw[];
-    const NbConst& K = A.kc;
-    const int lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7, g8 = lane >> 2, k4 = lane & 3;
-    const int nt1 = K.ntypes1, ljn = 4 * nt1, G = gridDim.x;
-    SegStage& S = *reinterpret_cast<SegStage*>(s_raw);
-    float4* const ljbuf = reinterpret_cast<float4*>(s_raw + sizeof(SegStage));
-    const float2 p3 = K.ewp2[3];
-    int seg = blockIdx.x, b = 0;
-    // Segments beyond the first G are handed out by a ticket counter, in the longest-first order, to whichever
-    // warp gets there first (a static deal left 17 % of the warp slots idle at the end, ncu).  The ticket for the
-    // segment after the next is drawn at the start of a segment and read one segment later: never waited for.
-    int ticket = lane == 0 ? atomicAdd(A.ticket, 1) : 0;
-    // the first segment of the warp: the three rounds one after the other
-    seg_stage1(A, S, seg, lane);
-    cp_async_wait_all();
-    seg_stage2(A, S, ljbuf, ljn, lane);
-    cp_async_wait_all();
-    seg_stage3(A, S, lane);
-    for (;;) {
-        cp_async_wait_all();
-        const int4 sd = S.segd;
-        const int buf = A.bufmask ? (int)((A.bufmask >> S.part) & 1u) : 0;
-        const int2 cnt = S.cnt[buf];   // {half entries, masked pairs}
-        const int ci = sd.z & 0x3ffffff, sid = sd.z >> 26, warp = ci & 7;
-        const float4* ljw = ljbuf + b * ljn;
-        const int* __restrict__ il = A.il[buf] + sd.x;
-        const int2* __restrict__ ilm = A.ilm[buf] + sd.y;
-        const int ns = cnt.x >> 3;
-        int sx, sy, sz;
-        nb_shift_vec(sid, sx, sy, sz);
-        IAtoms I;
-#pragma unroll
-        for (int p = 0; p < 4; p++) {
-            const float4 v0 = S.iat[2 * p], v1 = S.iat[2 * p + 1];
-            I.x[p] = f2(fmaf((float)sx, K.box[0], v0.x), fmaf((float)sx, K.box[0], v1.x));
-            I.y[p] = f2(fmaf((float)sy, K.box[1], v0.y), fmaf((float)sy, K.box[1], v1.y));
-            I.z[p] = f2(fmaf((float)sz, K.box[2], v0.z), fmaf((float)sz, K.box[2], v1.z));
-            I.q[p] = f2(K.epsfac * v0.w, K.epsfac * v1.w);
-        }
-        // operands of the first masked step and of the first two unmasked steps, staged by seg_stage3
-        int2 ce_next = g < cnt.y ? S.ilmh[g] : make_int2(ci, 0);
-        float4 xm = S.xm[lane];
-        int tm = S.tm[lane];
-        ulonglong2 mm = S.mk[lane];
-        int cj = 0, cj_n = 0, e2 = 0, e3 = 0;
-        float4 xj = make_float4(0.f, 0.f, 0.f, 0.f), xj1 = xj;
-        int tj = 0, tj1 = 0;
-        if (ns > 0) {
-            cj = S.ilh[g8] * 4 + k4;                       // cj, cj_n: this lane's j SLOT of this and the next step
-            cj_n = S.ilh[8 * min(1, ns - 1) + g8] * 4 + k4;
-            e2 = S.ilh[8 * min(2, ns - 1) + g8];           // e2, e3: list entries of the steps after, as loaded
-            e3 = S.ilh[8 * min(3, ns - 1) + g8];
-            xj = S.xs[0][lane]; tj = S.ts[0][lane];
-            xj1 = S.xs[1][lane]; tj1 = S.ts[1][lane];
-        }
-        __syncwarp();
-        // round 1 for the next segment of this warp, and the ticket for the one after
-        const int nxt = G + __shfl_sync(0xffffffffu, ticket, 0);
-        int phase = nxt < nseg ? 0 : 2;   // 0: round 2 to be issued, 1: round 3 to be issued, 2: nothing left
-        if (phase == 0) {
-            seg_stage1(A, S, nxt, lane);
-            if (lane == 0) ticket = atomicAdd(A.ticket, 1);
-        }
-        const int p2_at = max(ns - 5, 0), p3_at = max(ns - 2, p2_at + 1);
-
-        float2 fix[4], fiy[4], fiz[4];
-#pragma unroll
-        for (int p = 0; p < 4; p++) { fix[p] = f2(0.f); fiy[p] = f2(0.f); fiz[p] = f2(0.f); }
-        float elj = 0.f, ecoul = 0.f;
-
-        // cluster pairs with exclusion / self / diagonal masks, 4 per step (first step: staged operands)
-        for (int s = 0; s < cnt.y; s += 4) {
-            const bool valid = s + g < cnt.y;
-            const int2 ce = ce_next;
-            if (s + 4 < cnt.y) ce_next = s + 4 + g < cnt.y ? ilm[s + 4 + g] : make_int2(ci, 0);
-            if (s > 0) {
-                xm = A.xq[ce.x * 8 + k];
-                tm = A.type_slot[ce.x * 8 + k];
-                mm = *reinterpret_cast<const ulonglong2*>(&A.masks[((size_t)ce.y * 8 + warp) * 2]);
-            }
-            const unsigned cbyte = valid ? (unsigned)(mm.y >> (8 * k)) & 0xffu : 0u;
-            const unsigned mbyte = (unsigned)(mm.x >> (8 * k)) & cbyte;
-            float2 fjx, fjy, fjz;
-            pair_step<COUL, ENERGY, true, TWIN, false>(K, ljw + tm, nt1, I, fix, fiy, fiz, elj, ecoul, xm, cbyte, mbyte, fjx, fjy,
-                                                       fjz, p3, 0.f);
-            if (valid) red_add_v4(&A.f4[ce.x * 8 + k], -(fjx.x + fjx.y), -(fjy.x + fjy.y), -(fjz.x + fjz.y));
-        }
-
-        // cluster pairs without a mask: full steps of 8 half-clusters; j data two steps and list entries
-        // four steps ahead in registers (ptxas sinks loads whose consumer is an iteration away to the END of
-        // a step, so a distance of one step exposed the latency)
-#pragma unroll 2
-        for (int s = 0; s < ns; s++) {
-            if (phase == 0 && s == p2_at) {
-                cp_async_wait_all();
-                seg_stage2(A, S, ljbuf + (b ^ 1) * ljn, ljn, lane);
-                phase = 1;
-            } else if (phase == 1 && s >= p3_at) {
-                cp_async_wait_all();
-                seg_stage3(A, S, lane);
-                phase = 2;
-            }
-            // (the entry loaded here is first touched two steps later, when its slot is formed: forming it
-            // at once made ptxas wait for the load at the end of the same unrolled pair of steps)
-            const int e4 = il[8 * min(s + 4, ns - 1) + g8];
-            const int cj2 = e2 * 4 + k4;
-            const float4 x2 = A.xq[cj2];
-            const int t2 = A.type_slot[cj2];
-            float2 fjx, fjy, fjz;
-            pair_step<COUL, ENERGY, false, TWIN, false>(K, ljw + tj, nt1, I, fix, fiy, fiz, elj, ecoul, xj, 0xffu, 0xffu, fjx, fjy,
-                                                        fjz, p3, 0.f);
-            red_add_v4(&A.f4[cj], -(fjx.x + fjx.y), -(fjy.x + fjy.y), -(fjz.x + fjz.y));
-            cj = cj_n; xj = xj1; tj = tj1;
-            cj_n = cj2; xj1 = x2; tj1 = t2;
-            e2 = e3; e3 = e4;
-        }
-        // a short segment: whatever the loop did not get to
-        if (phase == 0) {
-            cp_async_wait_all();
-            seg_stage2(A, S, ljbuf + (b ^ 1) * ljn, ljn, lane);
-            phase = 1;
-        }
-        if (phase == 1) {
-            cp_async_wait_all();
-            seg_stage3(A, S, lane);
-        }
-
-        float fi[24];
-#pragma unroll
-        for (int p = 0; p < 4; p++) {
-            fi[6 * p + 0] = fix[p].x; fi[6 * p + 1] = fiy[p].x; fi[6 * p + 2] = fiz[p].x;
-            fi[6 * p + 3] = fix[p].y; fi[6 * p + 4] = fiy[p].y; fi[6 * p + 5] = fiz[p].y;
-        }
-        if (ENERGY) {
-            // per-shift sum of i forces for the virial (reading A8) and the energies, fp64 atomics per segment
-            float sxs = 0.f, sys = 0.f, szs = 0.f;
-#pragma unroll
-            for (int a = 0; a < 8; a++) { sxs += fi[3 * a]; sys += fi[3 * a + 1]; szs += fi[3 * a + 2]; }
-#pragma unroll
-            for (int d = 16; d > 0; d >>= 1) {
-                sxs += __shfl_xor_sync(0xffffffffu, sxs, d);
-                sys += __shfl_xor_sync(0xffffffffu, sys, d);
-                szs += __shfl_xor_sync(0xffffffffu, szs, d);
-                elj += __shfl_xor_sync(0xffffffffu, elj, d);
-                ecoul += __shfl_xor_sync(0xffffffffu, ecoul, d);
-            }
-            if (lane == 0) {
-                if (sid != NB_SHIFT_CENTER) {
-                    atomicAdd(&A.fshift[sid * 3 + 0], (double)sxs);
-                    atomicAdd(&A.fshift[sid * 3 + 1], (double)sys);
-                    atomicAdd(&A.fshift[sid * 3 + 2], (double)szs);
-                }
-                atomicAdd(&A.energies[0], (double)elj);
-                atomicAdd(&A.energies[1], (double)ecoul);
-            }
-        }
-        // (a8) i-force reduction: butterfly reduce-scatter of the 24 partial sums over the 32 lanes;
-        // afterwards the quad lane>>2 == a holds (fx,fy,fz) of i atom a.
-#pragma unroll
-        for (int half = 12, d = 16; half >= 3; half >>= 1, d >>= 1) {
-            const bool upper = (lane & d) != 0;
-#pragma unroll
-            for (int i = 0; i < half; i++) {
-                const float keep = upper ? fi[i + half] : fi[i];
-                const float send = upper ? fi[i] : fi[i + half];
-                fi[i] = keep + __shfl_xor_sync(0xffffffffu, send, d);
-            }
-        }
-#pragma unroll
-        for (int d = 2; d > 0; d >>= 1) {
-            fi[0] += __shfl_xor_sync(0xffffffffu, fi[0], d);
-            fi[1] += __shfl_xor_sync(0xffffffffu, fi[1], d);
-            fi[2] += __shfl_xor_sync(0xffffffffu, fi[2], d);
-        }
-        if ((lane & 3) == 0) red_add_v4(&A.f4[ci * 8 + (lane >> 2)], fi[0], fi[1], fi[2]);
-
-        if (nxt >= nseg) break;
-        seg = nxt;
-        b ^= 1;
-    }
-}
-
 // Paired LJ rows per i-cluster, written once per search (types are fixed between searches):
 // ljrow[(ci*4 + p)*nt1 + tj] = (-6c6, -6c6', 12c12, 12c12') of the i atoms 2p, 2p+1 of cluster ci against
 // j type tj -- what the force kernel's prologue copies to shared memory with one coalesced load.
@@ -678,10 +405,9 @@ __global__ void k_ljrows(int nrows, int nt1, const int* __restrict__ type_slot, 
 template <bool VIRIAL>
 __global__ void __launch_bounds__(256) k_gather(int nslots, float4* __restrict__ f4, const int* __restrict__ atom_of_slot,
                                                 const float4* __restrict__ xq, float* __restrict__ f,
-                                                double* __restrict__ xf /* [9] sum x (x) f */, int* __restrict__ ticket)
+                                                double* __restrict__ xf /* [9] sum x (x) f */)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s == 0) *ticket = 0;   // the force kernel's work counter, for its next launch
     double v[9];
 #pragma unroll
     for (int i = 0; i < 9; i++) v[i] = 0.0;
@@ -722,10 +448,9 @@ __global__ void __launch_bounds__(256) k_gather(int nslots, float4* __restrict__
 // Force-only gather, 4 consecutive slots per thread (nslots is a multiple of 64): the loads of a
 // thread are independent and issued together, which matters more than bytes at these sizes.
 __global__ void __launch_bounds__(256) k_gather4(int nquads, float4* __restrict__ f4, const int4* __restrict__ atom_of_slot4,
-                                                 float* __restrict__ f, int* __restrict__ ticket)
+                                                 float* __restrict__ f)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t == 0) *ticket = 0;   // the force kernel's work counter, for its next launch
     if (t >= nquads) return;
     const int4 a = atom_of_slot4[t];
     float4* p = f4 + 4 * (size_t)t;
@@ -840,28 +565,24 @@ __global__ void k_count_slots(ForceArgs A, int nseg, int nhalf_real, unsigned lo
     if ((threadIdx.x & 31) == 0 && n) atomicAdd(out, n);
 }
 
-// The fused first prune keeps one block per segment (k_force<..., PRUNE = true>: once per list lifetime);
-// everything else is the persistent kernel.
-template <int COUL, bool ENERGY, bool TWIN>
-int launch_force_p(nb_ctx* c, const ForceArgs& A, bool prune)
+template <int COUL, bool ENERGY, bool TWIN, bool PRUNE>
+int launch_force(nb_ctx* c, const ForceArgs& A)
 {
-    if (prune) {
-        const size_t smem = sizeof(float4) * 4 * (size_t)c->kc.ntypes1;   // paired LJ table of one i-cluster, 64 B per type
-        if (smem > 48 * 1024)
-            NB_CUDA(c, cudaFuncSetAttribute(k_force<COUL, ENERGY, TWIN, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        k_force<COUL, ENERGY, TWIN, true><<<c->nseg_launch, 32, smem, c->stream>>>(A);
-    } else {
-        const size_t smem = sizeof(SegStage) + 2 * sizeof(float4) * 4 * (size_t)c->kc.ntypes1;
-        if (smem > 48 * 1024)
-            NB_CUDA(c, cudaFuncSetAttribute(k_force_ps<COUL, ENERGY, TWIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        const int grid = std::min(c->nseg_launch, c->nsm * 16);   // one warp per register-file slot
-        k_force_ps<COUL, ENERGY, TWIN><<<grid, 32, smem, c->stream>>>(A, c->nseg_launch);
-    }
+    const size_t smem = sizeof(float4) * 4 * (size_t)c->kc.ntypes1;   // paired LJ table of one i-cluster, 64 B per type
+    if (smem > 48 * 1024)
+        NB_CUDA(c, cudaFuncSetAttribute(k_force<COUL, ENERGY, TWIN, PRUNE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_force<COUL, ENERGY, TWIN, PRUNE><<<c->nseg_launch, 32, smem, c->stream>>>(A);
     NB_LAUNCH_CHECK(c);
     return NB_OK;
 }
+
 // One instantiation per combination of electrostatics, energy / no energy, single / twin cut-off and
 // plain / fused-prune ("separate kernels are used for different combinations ... to avoid conditionals").
+template <int COUL, bool ENERGY, bool TWIN>
+int launch_force_p(nb_ctx* c, const ForceArgs& A, bool prune)
+{
+    return prune ? launch_force<COUL, ENERGY, TWIN, true>(c, A) : launch_force<COUL, ENERGY, TWIN, false>(c, A);
+}
 template <int COUL, bool ENERGY>
 int launch_force_t(nb_ctx* c, const ForceArgs& A, bool twin, bool prune)
 {
@@ -889,7 +610,6 @@ static void fill_force_args(nb_ctx* c, ForceArgs& A)
     }
     A.bufmask = c->bufmask;
     A.seg_part = c->seg_part.p;
-    A.ticket = c->ticket.p;
     A.nparts = c->buf_nparts;
     A.nunits = c->nunits;
     A.xq = c->xq.p;
@@ -966,10 +686,10 @@ int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial, float rlis
     const int nb = (nslots + 255) / 256;
     NbStageTimer tm(c, NB_T_REDUCE);
     if (virial)
-        k_gather<true><<<nb, 256, 0, st>>>(nslots, c->f4.p, c->atom_of_slot.p, c->xq.p, f, xf, c->ticket.p);
+        k_gather<true><<<nb, 256, 0, st>>>(nslots, c->f4.p, c->atom_of_slot.p, c->xq.p, f, xf);
     else
         k_gather4<<<(nslots / 4 + 255) / 256, 256, 0, st>>>(nslots / 4, c->f4.p,
-                                                           reinterpret_cast<const int4*>(c->atom_of_slot.p), f, c->ticket.p);
+                                                           reinterpret_cast<const int4*>(c->atom_of_slot.p), f);
     NB_LAUNCH_CHECK(c);
     if (virial) {
         k_virial_final<<<1, 32, 0, st>>>(xf, c->fshift.p, make_float3(c->box[0], c->box[1], c->box[2]), virial);

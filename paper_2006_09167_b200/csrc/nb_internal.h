@@ -196,7 +196,6 @@ struct nb_ctx {
     cudaEvent_t ev_main = nullptr, ev_side = nullptr;
     size_t il_total = 0, ilm_total = 0;        // extents of il / ilm in use
     int nseg_launch = 0;                       // segments with a non-empty outer list (= force kernel grid)
-    DevBuf<int32_t> ticket;                    // [1] work counter of the persistent force kernel, zero between launches
     DevBuf<float4> ljrow;                      // [nclusters_max * 4 * (ntypes+1)] paired LJ rows per i-cluster (nb_force.cu), written at search
     DevBuf<double> fshift;                     // [27*3] per-shift i-force sums (virial)
 
