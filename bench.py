@@ -92,9 +92,15 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-flush", action="store_true", help="do not flush L2 between timed steps")
-    ap.add_argument("--prune", default="overlapped", choices=["plain", "overlapped"],
+    ap.add_argument("--prune", default="plain", choices=["plain", "overlapped"],
                     help="rolling prune on the caller's stream before the force kernel (plain) or on the library's second "
                          "stream next to it (overlapped, PAPER.md L193)")
+    ap.add_argument("--inner-step", default="nb_step", choices=["nb_step", "calls"],
+                    help="inner steps of the device leg through nb_step (one call, one CUDA graph launch) or through the three "
+                         "calls nb_put_atoms / nb_prune / nb_forces; the e2e leg and the stage-timing passes always use the calls")
+    ap.add_argument("--first-prune", default="separate", choices=["separate", "fused"],
+                    help="first use of a fresh list: nb_prune(.., 0, 1) then nb_forces (separate), or the one-kernel nb_forces_prune "
+                         "(fused, PAPER.md L189)")
     return ap.parse_args()
 
 
@@ -170,7 +176,7 @@ class ClockSampler(threading.Thread):
 class Replica:
     """One box on one GPU, driven through the Python binding of the C ABI."""
 
-    def __init__(self, w, device_index, flush, overlapped=False):
+    def __init__(self, w, device_index, flush, overlapped=False, fused_first=False):
         import numpy as np
         import torch
         from paper_2006_09167_b200 import nb
@@ -198,6 +204,7 @@ class Replica:
         self.pairs_at_frame = None
         self.slots_at_frame = None
         self.overlapped = overlapped
+        self.fused_first = fused_first
 
     def _rolling_prune(self, fr):
         w, c = self.w, self.ctx
@@ -214,11 +221,23 @@ class Replica:
         c.put_atoms(self.x_dev[fr], self.q_dev if fr == 0 else None, self.t_dev if fr == 0 else None, w.box)
         if fr == 0:
             c.search(w.rlist_outer)
-            c.prune(w.rlist_inner, 0, 1)           # first use of a fresh list: full prune
-            c.forces(self.f_dev, self.e_dev, self.v_dev)   # energies + virial once per list lifetime
+            if self.fused_first:                   # first use of a fresh list: prune inside the force kernel
+                c.forces_prune(w.rlist_inner, self.f_dev, self.e_dev, self.v_dev)
+            else:
+                c.prune(w.rlist_inner, 0, 1)       # ... or a full prune (L187) followed by the force kernel
+                c.forces(self.f_dev, self.e_dev, self.v_dev)   # energies + virial once per list lifetime
         else:
             self._rolling_prune(fr)
             c.forces(self.f_dev, None, None)
+
+    def step_device_graph(self, t):
+        """Same schedule, inner steps through nb_step (put + rolling prune + forces as one call / one CUDA graph launch)."""
+        w, c = self.w, self.ctx
+        fr = t % w.nstlist
+        if fr == 0:
+            self.step_device(t)
+        else:
+            c.step(self.x_dev[fr], w.rlist_inner, fr % w.nparts, w.nparts, self.f_dev)
 
     def step_host(self, t):
         """Host buffers in, host buffers out (the `e2e` leg): copies inside the timed region."""
@@ -441,7 +460,8 @@ def run_b200(args):
     barrier, max_over_ranks, sum_over_ranks = ranks.barrier, ranks.max, ranks.sum
 
     w = load_workload(args)
-    rep = Replica(w, local_rank, flush=not args.no_flush, overlapped=args.prune == "overlapped" and w.nparts <= 32)
+    rep = Replica(w, local_rank, flush=not args.no_flush, overlapped=args.prune == "overlapped" and w.nparts <= 32,
+                  fused_first=args.first_prune == "fused")
     ctx = rep.ctx
     fma_peak = ctx.measure_fp32_peak()          # lane-FMA/s of a register-resident FFMA chain, this GPU, now
     rep.count_pass()                            # untimed: per-frame pair and slot counts (also warms everything up)
@@ -453,25 +473,32 @@ def run_b200(args):
     # ---------------- device-resident leg: `value` ----------------
     for i in range(W):
         rep.step_device(i)
-    # Inside the timed region only the force kernel (the roofline's kernel) carries an event pair:
-    # every timed stage costs two event records per call (~3 us of stream time per stage and step;
-    # with all seven stages timed the step was 13-26 % longer).  The other stages are timed in a
-    # second pass over the same steps that does not count towards `value`.
-    force_bit = (1 << nb.NB_T_NAMES.index("force")) | (1 << nb.NB_T_NAMES.index("force_energy"))
-    ctx.timing_stages(force_bit)
-    ctx.timing_enable(True)
-    ctx.timing_read(reset=True)
+    # The `value` pass carries no stage timing at all: an event pair around one kernel costs two event records per
+    # launch, each a serialisation point of the stream (measured: +5 us on the 116 us inner step of config 2 with only
+    # the force kernel timed, 13-26 % with every stage timed).  The force kernel (the roofline's kernel) is timed with
+    # CUDA events in a second pass over the same schedule positions, the remaining stages in a third.
+    ctx.timing_enable(False)
+    use_step = args.inner_step == "nb_step" and not rep.overlapped
+    step_value = rep.step_device_graph if use_step else rep.step_device
+    for i in range(W):
+        step_value(i)
     launches0 = ctx.get_stats()["kernel_launches"]
     barrier()
     sampler = ClockSampler(local_rank)
     sampler.start()
-    pop = rep.timed(rep.step_device, positions)
+    pop = rep.timed(step_value, positions)
     barrier()
     clocks = sampler.result()
-    stages = ctx.timing_read(reset=True)
     st1 = ctx.get_stats()
     launches = st1["kernel_launches"] - launches0 - 3   # get_stats itself launches three counting kernels
-    # second pass, plain prune (the stage timer brackets launches on the caller's stream): the other stages
+    # second pass: the same steps with an event pair around the force kernel only
+    force_bit = (1 << nb.NB_T_NAMES.index("force")) | (1 << nb.NB_T_NAMES.index("force_energy"))
+    ctx.timing_stages(force_bit)
+    ctx.timing_enable(True)
+    ctx.timing_read(reset=True)
+    pop_f = rep.timed(rep.step_device, positions)
+    stages = ctx.timing_read(reset=True)
+    # third pass, plain prune (the stage timer brackets launches on the caller's stream): the other stages
     ctx.timing_stages(0xFFFFFFFF & ~force_bit)
     was_overlapped, rep.overlapped = rep.overlapped, False
     rep.timed(rep.step_device, positions)
@@ -481,6 +508,7 @@ def run_b200(args):
     ctx.timing_stages(0xFFFFFFFF)
     ctx.timing_enable(False)
     ms_step, pairs_step, slots_step = schedule_mean(pop, w.nstlist)
+    ms_step_f, _, _ = schedule_mean(pop_f, w.nstlist)
     ms_step_max = max_over_ranks(ms_step)
     value = sum_over_ranks(float(pairs_step)) / (ms_step_max * 1e-3)
     ms_search = max_over_ranks(pop["search"][0] / max(pop["search"][1], 1))
@@ -524,8 +552,10 @@ def run_b200(args):
                 "measured_ffma_chain_tflops": 2 * fma_peak / 1e12,
                 "frac_of_measured_ffma_chain": achieved / (2 * fma_peak / 1e12),
                 "flop_per_slot": flop_slot, "slots_per_launch": slots_per_launch, "kernel_us": force_us,
-                "kernel_us_is": "mean of the F-only launches (the inner steps) inside the timed region; the F+E+virial launches of "
-                                "the search steps are stage_us.force_energy"}
+                "kernel_us_is": "mean of the F-only launches (the inner steps), CUDA events on the launching stream, in a second timed "
+                                "pass over the same schedule positions (ms_per_step of that pass: ms_per_step_with_force_events); "
+                                "the F+E+virial launches of the search steps are stage_us.force_energy",
+                "ms_per_step_with_force_events": ms_step_f}
 
     line = None
     if rank == 0:
@@ -564,7 +594,9 @@ def run_b200(args):
                 "ms_per_step": ms_step_max, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic",
                 "config": workload_config(w, args, {"l2": "flushed between timed steps (256 MiB fill)" if not args.no_flush
-                                                    else "not flushed", "prune": "overlapped" if rep.overlapped else "plain"}),
+                                                    else "not flushed", "prune": "overlapped" if rep.overlapped else "plain",
+                                                    "first_prune": args.first_prune,
+                                                    "inner_step": "nb_step (CUDA graph)" if use_step else "three calls"}),
                 "schedule": {"timed_inner_steps": pop["inner"][1], "timed_search_steps": S, "ms_inner_step": ms_inner,
                              "ms_search_step": ms_search,
                              "ms_per_step_is": "(ms_search_step + (nstlist-1) * ms_inner_step) / nstlist"},
@@ -575,7 +607,8 @@ def run_b200(args):
                 "stage_us": per_stage_us,
                 "stage_share_of_step": {k: ((v / w.nstlist if k in ("grid", "search", "masks") else v) / (1e3 * ms_step) if v else None)
                                         for k, v in per_stage_us.items()},
-                "stage_timing": "force: event pair inside the timed region; other stages: second pass over the same steps with the plain prune",
+                "stage_timing": "the timed region of `value` carries no stage events; force: second pass over the same steps with an event "
+                                "pair around the force kernel; other stages: third pass with the plain prune",
                 "list": {k: st[k] for k in ("nsuper", "n_sci_entries", "n_joint_outer", "n_pairs_outer", "n_pairs_inner",
                                             "n_excl_masks", "n_work_units", "list_grow_retries")}}
         if world == 1 and not args.no_cpu_baseline:

@@ -144,6 +144,17 @@ int nb_forces_host(nb_ctx*, float* f, double* energies, double* virial);
  * same inner list bit for bit, forces equal up to summation order.  Same argument rules as nb_prune / nb_forces. */
 int nb_forces_prune(nb_ctx*, float rlist_inner, float* f, double* energies, double* virial);
 
+/* One inner step of the schedule as ONE call: nb_put_atoms(x, NULL, NULL, the box of the last search) +
+ * nb_prune(rlist_inner, part, nparts) + nb_forces(f, NULL, NULL): the same kernels in the same order, so the same inner
+ * list bit for bit and the same forces up to the order of the atomic adds.
+ * From the second use of a (part, nparts, rlist_inner) on a given list the three stages are enqueued as one CUDA graph
+ * launch (captured once, updated in place after every search; x and f are patched into it at each call), which is what
+ * makes small systems, whose step is a handful of 3-30 us kernels, launch-bound no longer (the
+ * strong-scaling regime of a few hundred atoms per SM).  x [dev] natoms*3 continuous coordinates, f [dev] natoms*3.
+ * Needs a valid list and an unchanged box (NB_ERR_STATE otherwise); other errors as nb_prune / nb_forces.
+ * With stage timing on, an overlapped prune in flight or more than 32 parts it simply runs the three calls. */
+int nb_step(nb_ctx*, const float* x, float rlist_inner, int part, int nparts, float* f);
+
 void nb_free(nb_ctx*);
 const char* nb_last_error(const nb_ctx*);
 

@@ -192,6 +192,8 @@ extern "C" int nb_put_atoms_host(nb_ctx* c, const float* x, const float* q, cons
     return put_atoms_common(c, x, q, type, box, cudaMemcpyHostToDevice);
 }
 
+static void step_graphs_refresh(nb_ctx* c);
+
 extern "C" int nb_search(nb_ctx* c, float rlist_outer)
 {
     if (!c) return NB_ERR_ARG;
@@ -201,7 +203,9 @@ extern "C" int nb_search(nb_ctx* c, float rlist_outer)
     if (!(rlist_outer >= c->prm.rc) || !(rlist_outer <= 0.5f * minL))
         return nb_fail(c, NB_ERR_CUTOFF, "rlist_outer = %g must satisfy rc = %g <= rlist_outer <= min(L)/2 = %g", rlist_outer, c->prm.rc, 0.5f * minL);
     c->have_list = false;
-    return nbi_search(c, rlist_outer);
+    int rc = nbi_search(c, rlist_outer);
+    if (rc == NB_OK) step_graphs_refresh(c);   // the step graphs of the previous list, re-captured for this one
+    return rc;
 }
 
 static int prune_checks(nb_ctx* c, float rlist_inner, int part, int nparts)
@@ -251,6 +255,156 @@ extern "C" int nb_forces_prune(nb_ctx* c, float rlist_inner, float* f, double* e
     return nbi_forces(c, f, energies, virial, rlist_inner);
 }
 
+// ---- nb_step -------------------------------------------------------------------------------------------
+static int step_plain(nb_ctx* c, const float* x, float rlist_inner, int part, int nparts, float* f)
+{
+    int rc = nbi_commit_pending(c);
+    if (rc != NB_OK) return rc;
+    c->atoms_since_search = true;
+    if ((rc = nbi_put_device(c, x, nullptr, nullptr, true)) != NB_OK) return rc;
+    if ((rc = nbi_prune(c, rlist_inner, part, nparts)) != NB_OK) return rc;
+    return nbi_forces(c, f, nullptr, nullptr);
+}
+
+static void step_graph_release(nb_ctx::StepGraph& g)
+{
+    if (g.exec) cudaGraphExecDestroy(g.exec);
+    if (g.graph) cudaGraphDestroy(g.graph);
+    g.exec = nullptr;
+    g.graph = nullptr;
+    g.put = g.gather = nullptr;
+}
+
+// Captures put + prune + forces for this key on the private stream and instantiates (or updates) the executable graph.
+static int step_capture(nb_ctx* c, nb_ctx::StepGraph& g, const float* x, float* f)
+{
+    if (!c->capture_stream && cudaStreamCreateWithFlags(&c->capture_stream, cudaStreamNonBlocking) != cudaSuccess) return NB_ERR_CUDA;
+    const nb_stats saved = c->st;
+    cudaStream_t user = c->stream;
+    cudaGraph_t graph = nullptr;
+    if (cudaStreamBeginCapture(c->capture_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) return NB_ERR_CUDA;
+    c->stream = c->capture_stream;
+    int rc = step_plain(c, x, g.rl, g.part, g.nparts, f);
+    c->stream = user;
+    const cudaError_t ee = cudaStreamEndCapture(c->capture_stream, &graph);
+    c->st = saved;   // nothing ran: the counters move when the graph is launched
+    if (rc != NB_OK || ee != cudaSuccess || !graph) {
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        return NB_ERR_CUDA;
+    }
+    cudaGraphNode_t nodes[16];
+    size_t nn = 16;
+    cudaGraphNode_t put = nullptr, gather = nullptr;
+    if (cudaGraphGetNodes(graph, nodes, &nn) != cudaSuccess) { cudaGraphDestroy(graph); return NB_ERR_CUDA; }
+    for (size_t i = 0; i < nn && i < 16; i++) {
+        cudaGraphNodeType ty;
+        cudaKernelNodeParams kp;
+        if (cudaGraphNodeGetType(nodes[i], &ty) != cudaSuccess || ty != cudaGraphNodeTypeKernel) continue;
+        if (cudaGraphKernelNodeGetParams(nodes[i], &kp) != cudaSuccess) continue;
+        if (kp.func == nbi_put_kernel()) put = nodes[i];
+        if (kp.func == nbi_gather4_kernel()) gather = nodes[i];
+    }
+    if (!put || !gather) { cudaGraphDestroy(graph); return NB_ERR_CUDA; }
+    if (g.exec) {
+        // Same topology as before the search: update the executable graph in place.  Node handles used with an executable
+        // graph must be those of the graph it was instantiated from, so that graph stays, and its put / gather nodes take
+        // over the new parameter blocks (they are what nb_step patches x and f into).
+        cudaGraphExecUpdateResultInfo info;
+        cudaKernelNodeParams kput, kgat;
+        if (cudaGraphExecUpdate(g.exec, graph, &info) == cudaSuccess && cudaGraphKernelNodeGetParams(put, &kput) == cudaSuccess &&
+            cudaGraphKernelNodeGetParams(gather, &kgat) == cudaSuccess && cudaGraphKernelNodeSetParams(g.put, &kput) == cudaSuccess &&
+            cudaGraphKernelNodeSetParams(g.gather, &kgat) == cudaSuccess) {
+            cudaGraphDestroy(graph);
+            return NB_OK;
+        }
+        cudaGetLastError();
+        step_graph_release(g);
+    }
+    if (cudaGraphInstantiate(&g.exec, graph, 0) != cudaSuccess) {
+        cudaGetLastError();
+        cudaGraphDestroy(graph);
+        g.exec = nullptr;
+        return NB_ERR_CUDA;
+    }
+    g.graph = graph;   // kept: node handles and the parameter blocks patched at every launch live in it
+    g.put = put;
+    g.gather = gather;
+    return NB_OK;
+}
+
+// After a search: the graphs that were in use on the previous list are brought up to date here, once per list
+// lifetime, instead of on their next use (a capture is ~50 us of host time that a step should not wait for).
+static void step_graphs_refresh(nb_ctx* c)
+{
+    if (c->timing) return;
+    const int64_t gen = c->st.search_count;
+    for (auto& g : c->step_graphs) {
+        if (!g.exec || g.broken || g.rl > c->rlist_outer || g.rl < c->prm.rc) continue;
+        if (nbi_prepare_parts(c, g.nparts) != NB_OK) { g.broken = true; continue; }   // part tables and launch orders of this list
+        if (step_capture(c, g, c->x.p, c->x.p) != NB_OK) { g.broken = true; continue; }   // (x and f are patched at every launch)
+        g.warm_search = g.graph_search = gen;
+    }
+}
+
+extern "C" int nb_step(nb_ctx* c, const float* x, float rlist_inner, int part, int nparts, float* f)
+{
+    if (!c) return NB_ERR_ARG;
+    DeviceGuard guard(c);
+    if (!x || !f) return nb_fail(c, NB_ERR_ARG, "nb_step: null argument");
+    if (!c->have_list || !c->have_grid) return nb_fail(c, NB_ERR_STATE, "nb_step without a valid list (call nb_search)");
+    if (c->box[0] != c->grid_box[0] || c->box[1] != c->grid_box[1] || c->box[2] != c->grid_box[2])
+        return nb_fail(c, NB_ERR_STATE, "nb_step: the box changed since the search (nb_put_atoms + nb_search first)");
+    int rc = prune_checks(c, rlist_inner, part, nparts);
+    if (rc != NB_OK) return rc;
+    // the graph covers the steady state only: no stage timing, no overlapped prune in flight, at most 32 parts
+    if (c->timing || nparts > 32 || c->pending_part >= 0 || c->bufmask) return step_plain(c, x, rlist_inner, part, nparts, f);
+    nb_ctx::StepGraph* g = nullptr;
+    for (auto& e : c->step_graphs)
+        if (e.part == part && e.nparts == nparts && e.rl == rlist_inner) g = &e;
+    if (!g) {
+        g = &c->step_graphs[c->step_graph_next];
+        c->step_graph_next = (c->step_graph_next + 1) % 8;
+        step_graph_release(*g);
+        *g = nb_ctx::StepGraph();
+        g->part = part; g->nparts = nparts; g->rl = rlist_inner;
+    }
+    const int64_t gen = c->st.search_count;
+    if (g->broken || g->warm_search != gen) {   // first use of this key on this list: the plain path sets everything up
+        g->warm_search = gen;
+        return step_plain(c, x, rlist_inner, part, nparts, f);
+    }
+    if (g->graph_search != gen) {
+        if (step_capture(c, *g, x, f) != NB_OK) {
+            g->broken = true;
+            return step_plain(c, x, rlist_inner, part, nparts, f);
+        }
+        g->graph_search = gen;
+    }
+    // patch the caller's pointers into the put (argument 1: x) and gather (argument 3: f) nodes
+    cudaKernelNodeParams kp;
+    void* args[16];
+    NB_CUDA(c, cudaGraphKernelNodeGetParams(g->put, &kp));
+    for (int i = 0; i < 11; i++) args[i] = kp.kernelParams[i];
+    args[1] = (void*)&x;
+    kp.kernelParams = args;
+    NB_CUDA(c, cudaGraphExecKernelNodeSetParams(g->exec, g->put, &kp));
+    NB_CUDA(c, cudaGraphKernelNodeGetParams(g->gather, &kp));
+    for (int i = 0; i < 4; i++) args[i] = kp.kernelParams[i];
+    args[3] = (void*)&f;
+    kp.kernelParams = args;
+    NB_CUDA(c, cudaGraphExecKernelNodeSetParams(g->exec, g->gather, &kp));
+    NB_CUDA(c, cudaGraphLaunch(g->exec, c->stream));
+    // what the three calls would have recorded on the host
+    c->atoms_since_search = true;
+    c->last_nparts = nparts;
+    c->planes_dirty = true;
+    c->st.prune_count++;
+    c->st.force_count++;
+    c->st.kernel_launches += 4;
+    return NB_OK;
+}
+
 extern "C" int nb_forces_host(nb_ctx* c, float* f, double* energies, double* virial)
 {
     if (!c) return NB_ERR_ARG;
@@ -275,6 +429,8 @@ extern "C" void nb_free(nb_ctx* c)
     if (c->side_stream) cudaStreamSynchronize(c->side_stream);
     cudaStreamSynchronize(c->stream);
     if (c->side_stream) cudaStreamDestroy(c->side_stream);
+    for (auto& g : c->step_graphs) step_graph_release(g);
+    if (c->capture_stream) cudaStreamDestroy(c->capture_stream);
     if (c->ev_main) cudaEventDestroy(c->ev_main);
     if (c->ev_side) cudaEventDestroy(c->ev_side);
     if (c->tot_dev) cudaFree(c->tot_dev);

@@ -213,6 +213,8 @@ __global__ void __launch_bounds__(32, PRUNE ? 8 : 16) k_force(ForceArgs A)
     // Paired LJ table of this block's i-cluster: s_ljp[p*nt1 + tj] = (-6c6, -6c6', 12c12, 12c12') of the
     // i atoms 2p, 2p+1 against j type tj: one LDS.128 feeds both packed operands.
     extern __shared__ float4 s_ljp[];
+    nb_pdl_wait();
+    nb_pdl_trigger();
     const NbConst& K = A.kc;
     const int lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7;
     const int4 sd = A.segd[blockIdx.x];
@@ -407,6 +409,8 @@ __global__ void __launch_bounds__(256) k_gather(int nslots, float4* __restrict__
                                                 const float4* __restrict__ xq, float* __restrict__ f,
                                                 double* __restrict__ xf /* [9] sum x (x) f */)
 {
+    nb_pdl_wait();
+    nb_pdl_trigger();
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     double v[9];
 #pragma unroll
@@ -450,6 +454,8 @@ __global__ void __launch_bounds__(256) k_gather(int nslots, float4* __restrict__
 __global__ void __launch_bounds__(256) k_gather4(int nquads, float4* __restrict__ f4, const int4* __restrict__ atom_of_slot4,
                                                  float* __restrict__ f)
 {
+    nb_pdl_wait();
+    nb_pdl_trigger();
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= nquads) return;
     const int4 a = atom_of_slot4[t];
@@ -571,7 +577,7 @@ int launch_force(nb_ctx* c, const ForceArgs& A)
     const size_t smem = sizeof(float4) * 4 * (size_t)c->kc.ntypes1;   // paired LJ table of one i-cluster, 64 B per type
     if (smem > 48 * 1024)
         NB_CUDA(c, cudaFuncSetAttribute(k_force<COUL, ENERGY, TWIN, PRUNE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_force<COUL, ENERGY, TWIN, PRUNE><<<c->nseg_launch, 32, smem, c->stream>>>(A);
+    NB_CUDA(c, nb_launch_pdl(k_force<COUL, ENERGY, TWIN, PRUNE>, dim3(c->nseg_launch), dim3(32), smem, c->stream, A));
     NB_LAUNCH_CHECK(c);
     return NB_OK;
 }
@@ -620,6 +626,8 @@ static void fill_force_args(nb_ctx* c, ForceArgs& A)
     A.kc = c->kc;
     for (int k = 0; k < 3; k++) A.kc.box[k] = c->box[k];
 }
+
+const void* nbi_gather4_kernel() { return (const void*)k_gather4; }
 
 int nbi_ljrows(nb_ctx* c)
 {
@@ -686,10 +694,10 @@ int nbi_forces(nb_ctx* c, float* f, double* energies, double* virial, float rlis
     const int nb = (nslots + 255) / 256;
     NbStageTimer tm(c, NB_T_REDUCE);
     if (virial)
-        k_gather<true><<<nb, 256, 0, st>>>(nslots, c->f4.p, c->atom_of_slot.p, c->xq.p, f, xf);
+        NB_CUDA(c, nb_launch_pdl(k_gather<true>, dim3(nb), dim3(256), 0, st, nslots, c->f4.p, c->atom_of_slot.p, c->xq.p, f, xf));
     else
-        k_gather4<<<(nslots / 4 + 255) / 256, 256, 0, st>>>(nslots / 4, c->f4.p,
-                                                           reinterpret_cast<const int4*>(c->atom_of_slot.p), f);
+        NB_CUDA(c, nb_launch_pdl(k_gather4, dim3((nslots / 4 + 255) / 256), dim3(256), 0, st, nslots / 4, c->f4.p,
+                                 reinterpret_cast<const int4*>(c->atom_of_slot.p), f));
     NB_LAUNCH_CHECK(c);
     if (virial) {
         k_virial_final<<<1, 32, 0, st>>>(xf, c->fshift.p, make_float3(c->box[0], c->box[1], c->box[2]), virial);

@@ -317,6 +317,8 @@ __global__ void __launch_bounds__(256) k_put(int n, const float* __restrict__ x,
                                              int* __restrict__ ctype, const char4* __restrict__ image,
                                              const int* __restrict__ slot_of_atom, float3 box, float4* __restrict__ xq)
 {
+    nb_pdl_wait();
+    nb_pdl_trigger();
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const float px = x[3 * i], py = x[3 * i + 1], pz = x[3 * i + 2];
@@ -333,11 +335,13 @@ __global__ void __launch_bounds__(256) k_put(int n, const float* __restrict__ x,
 
 }  // namespace
 
+const void* nbi_put_kernel() { return (const void*)k_put; }
+
 int nbi_put_device(nb_ctx* c, const float* x, const float* q, const int32_t* type, bool refresh)
 {
     int n = c->natoms;
-    k_put<<<(n + 255) / 256, 256, 0, c->stream>>>(n, x, q, type, c->x.p, c->q.p, c->type.p, c->image.p, c->slot_of_atom.p,
-                                                  make_float3(c->box[0], c->box[1], c->box[2]), refresh ? c->xq.p : nullptr);
+    NB_CUDA(c, nb_launch_pdl(k_put, dim3((n + 255) / 256), dim3(256), 0, c->stream, n, x, q, type, c->x.p, c->q.p, c->type.p, c->image.p, c->slot_of_atom.p,
+                                                  make_float3(c->box[0], c->box[1], c->box[2]), refresh ? c->xq.p : nullptr));
     NB_LAUNCH_CHECK(c);
     return NB_OK;
 }

@@ -199,6 +199,24 @@ struct nb_ctx {
     DevBuf<float4> ljrow;                      // [nclusters_max * 4 * (ntypes+1)] paired LJ rows per i-cluster (nb_force.cu), written at search
     DevBuf<double> fshift;                     // [27*3] per-shift i-force sums (virial)
 
+    // --- nb_step: the inner step (put + rolling prune + forces) as one CUDA graph launch ---
+    // One cached graph per (part, nparts, rlist_inner); captured on a private stream (the caller's may be the legacy
+    // default stream, which cannot be captured) the second time a key is used after a search, updated in place after
+    // the next search; the caller's x and f pointers are patched into the put / gather nodes at every launch.
+    struct StepGraph {
+        int part = -1, nparts = 0;
+        float rl = 0.f;
+        int64_t warm_search = -1;              // the plain path ran for this key on this list (buffers, orders, tables exist)
+        int64_t graph_search = -1;             // the graph was captured for this list
+        cudaGraph_t graph = nullptr;
+        cudaGraphExec_t exec = nullptr;
+        cudaGraphNode_t put = nullptr, gather = nullptr;
+        bool broken = false;                   // capture or instantiation failed: always the plain path
+    };
+    StepGraph step_graphs[8];
+    int step_graph_next = 0;
+    cudaStream_t capture_stream = nullptr;
+
     // --- per-stage device timing (nb_timing_enable / nb_timing_read) ---
     bool timing = false;
     unsigned timing_mask = ~0u;                // stages to time (nb_timing_stages)
@@ -294,6 +312,30 @@ __device__ __forceinline__ int nb_seg_buf(int u, unsigned bufmask, int nparts, i
 }
 #endif
 
+// Programmatic dependent launch: a kernel launched with nb_launch_pdl may be scheduled while its predecessor in the
+// stream is still draining (its launch latency and the predecessor's tail overlap); it must call nb_pdl_wait() before it
+// touches anything -- the wait returns when the predecessor grid has completed and its writes are visible.  A kernel calls
+// nb_pdl_trigger() to let its successor start being scheduled (all blocks must have called it or exited).
+#ifdef __CUDACC__
+__device__ __forceinline__ void nb_pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void nb_pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+template <typename... KArgs, typename... Args>
+inline cudaError_t nb_launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+#endif
+
 #define NB_CUDA(c, expr)                                                                              \
     do {                                                                                              \
         cudaError_t e__ = (expr);                                                                     \
@@ -324,9 +366,12 @@ int nbi_count_slots(nb_ctx* c, int64_t* slots);            // nb_force.cu
 int nbi_inner_dump(nb_ctx* c, int64_t* n, int32_t* ci, int32_t* entry, int32_t* shift, int32_t* kind, int32_t* part);   // nb_force.cu
 int nbi_prune_overlapped(nb_ctx* c, float rlist_inner, int part, int nparts);   // nb_prune.cu
 int nbi_commit_pending(nb_ctx* c);                          // nb_prune.cu: join an overlapped prune and flip its part
+int nbi_prepare_parts(nb_ctx* c, int nparts);               // nb_prune.cu: part table and prune launch order for nparts, now
 int nbi_consolidate(nb_ctx* c);                             // nb_prune.cu: move every segment back to inner buffer 0
 int nbi_rebuild_inner_planes(nb_ctx* c);                    // nb_list.cu: plane_inner from the compact inner list (introspection)
 int nbi_list_stats(nb_ctx* c);                              // nb_list.cu: lazily computed list statistics
 int nbi_prune_order(nb_ctx* c, int nparts, const int32_t** table);   // nb_list.cu: prune launch order for nparts rolling parts
 int nbi_ljrows(nb_ctx* c);                                  // nb_force.cu: paired LJ rows per i-cluster, at search time
 int nbi_exclusive_scan(nb_ctx* c, const int32_t* in, int32_t* out, int64_t n, int32_t* total_dev);  // nb_list.cu
+const void* nbi_put_kernel();                               // nb_grid.cu: the k_put entry (node lookup in captured graphs)
+const void* nbi_gather4_kernel();                           // nb_force.cu: the k_gather4 entry

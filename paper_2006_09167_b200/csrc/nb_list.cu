@@ -121,6 +121,30 @@ __global__ void k_scan_add(int* __restrict__ out, const int* __restrict__ blk, l
     long long i = (long long)blockIdx.x * 1024 + threadIdx.x;
     if (i < n) out[i] += blk[blockIdx.x];
 }
+// Second half of the two-launch scan: every block sums the totals of the blocks before it (a few dozen values)
+// and adds that base to its 1024 outputs; the last block also writes the grand total.
+__global__ void __launch_bounds__(1024) k_scan_fix(int* __restrict__ out, const int* __restrict__ blk, long long n, int nblk,
+                                                   int* __restrict__ total)
+{
+    __shared__ int s_part[32];
+    __shared__ int s_base;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int v = 0;
+    for (int b = threadIdx.x; b < (int)blockIdx.x; b += 1024) v += blk[b];
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    if (lane == 0) s_part[warp] = v;
+    __syncthreads();
+    if (warp == 0) {
+        int w = s_part[lane];
+        for (int d = 16; d > 0; d >>= 1) w += __shfl_xor_sync(0xffffffffu, w, d);
+        if (lane == 0) s_base = w;
+    }
+    __syncthreads();
+    const int base = s_base;
+    const long long i = (long long)blockIdx.x * 1024 + threadIdx.x;
+    if (i < n) out[i] += base;
+    if (total && (int)blockIdx.x == nblk - 1 && threadIdx.x == 0) *total = base + blk[nblk - 1];
+}
 
 template <typename F>
 int exclusive_scan(nb_ctx* c, F f, int32_t* out, int64_t n, int32_t* total_dev)
@@ -129,7 +153,7 @@ int exclusive_scan(nb_ctx* c, F f, int32_t* out, int64_t n, int32_t* total_dev)
         if (total_dev) NB_CUDA(c, cudaMemsetAsync(total_dev, 0, sizeof(int), c->stream));
         return NB_OK;
     }
-    if (n <= 96 * 1024) {
+    if (n <= 4096) {   // one block, up to four rounds
         k_scan_1blk<<<1, 1024, 0, c->stream>>>(f, out, n, total_dev);
         NB_LAUNCH_CHECK(c);
         return NB_OK;
@@ -138,6 +162,11 @@ int exclusive_scan(nb_ctx* c, F f, int32_t* out, int64_t n, int32_t* total_dev)
     NB_CUDA(c, c->scan_blk.ensure(nblk + 1, c->stream));
     k_scan_blocks<<<nblk, 1024, 0, c->stream>>>(f, out, c->scan_blk.p, n);
     NB_LAUNCH_CHECK(c);
+    if (nblk <= 8192) {   // two launches: each block adds up the totals before it (a one-block scan of 21k list elements took 23 us)
+        k_scan_fix<<<nblk, 1024, 0, c->stream>>>(out, c->scan_blk.p, n, nblk, total_dev);
+        NB_LAUNCH_CHECK(c);
+        return NB_OK;
+    }
     k_scan_1blk<<<1, 1024, 0, c->stream>>>(FnArr{c->scan_blk.p}, c->scan_blk.p, nblk, total_dev);
     NB_LAUNCH_CHECK(c);
     k_scan_add<<<nblk, 1024, 0, c->stream>>>(out, c->scan_blk.p, n);
@@ -339,6 +368,8 @@ __global__ void k_unit_fill(int nent, const int* __restrict__ ent_count, const i
 // ---------------------------------------------------------------- exclusion masks (a4)
 struct ExclArgs {
     int natoms;
+    float box[3], rl2;
+    const float4 *bb_lo, *bb_hi;
     const int *excl_off, *excl_idx, *slot_of_atom, *ent_count, *ent_jbegin;
     int2* jl;
     const uint8_t* imask;
@@ -362,23 +393,34 @@ __global__ void k_excl(ExclArgs A)
         int j = A.excl_idx[e];
         if (j <= i) continue;
         int sl[2] = {A.slot_of_atom[i], A.slot_of_atom[j]};
+        const float4 lo[2] = {A.bb_lo[sl[0] >> 3], A.bb_lo[sl[1] >> 3]}, hi[2] = {A.bb_hi[sl[0] >> 3], A.bb_hi[sl[1] >> 3]};
 #pragma unroll
         for (int o = 0; o < 2; o++) {
             int p = sl[o], q = sl[1 - o];
             int cp = p >> 3, cq = q >> 3, a = p & 7, b = q & 7;
             int scp = cp >> 3, w = cp & 7;
             for (int h = 0; h < NB_NHALF; h++) {
+                // the cluster pair is listed under this shift only if its boxes pass the search's own predicate
+                // (reading A13: the outer list is the pure bounding-box test): most of the 14 shifts end here,
+                // without touching the list
+                int sx, sy, sz;
+                nb_shift_vec(nb_half_shift_id(h), sx, sy, sz);
+                const float ib[6] = {__fmaf_rn((float)sx, A.box[0], lo[o].x), __fmaf_rn((float)sy, A.box[1], lo[o].y),
+                                     __fmaf_rn((float)sz, A.box[2], lo[o].z), __fmaf_rn((float)sx, A.box[0], hi[o].x),
+                                     __fmaf_rn((float)sy, A.box[1], hi[o].y), __fmaf_rn((float)sz, A.box[2], hi[o].z)};
+                if (!(bb_dist2_exact(ib, lo[1 - o], hi[1 - o]) < A.rl2)) continue;
                 int ent = scp * NB_NHALF + h;
                 int cnt = A.ent_count[ent];
                 if (cnt == 0) continue;
-                int lo = A.ent_jbegin[ent], hi = lo + cnt;
-                while (lo < hi) {
-                    int mid = (lo + hi) >> 1;
-                    if (A.jl[mid].x < cq) lo = mid + 1; else hi = mid;
+                int lo_ = A.ent_jbegin[ent], hi_ = lo_ + cnt;
+                const int end = hi_;
+                while (lo_ < hi_) {
+                    int mid = (lo_ + hi_) >> 1;
+                    if (A.jl[mid].x < cq) lo_ = mid + 1; else hi_ = mid;
                 }
-                if (lo < A.ent_jbegin[ent] + cnt && A.jl[lo].x == cq && ((A.imask[lo] >> w) & 1)) {
-                    if (MODE == 0) A.jl[lo].y = 1;
-                    else atomicAnd(&A.masks[((size_t)A.jl[lo].y * 8 + w) * 2], ~(1ull << (b * 8 + a)));
+                if (lo_ < end && A.jl[lo_].x == cq && ((A.imask[lo_] >> w) & 1)) {
+                    if (MODE == 0) A.jl[lo_].y = 1;
+                    else atomicAnd(&A.masks[((size_t)A.jl[lo_].y * 8 + w) * 2], ~(1ull << (b * 8 + a)));
                 }
             }
         }
@@ -845,7 +887,11 @@ int search_attempt(nb_ctx* c, float rlist)
     delete tm;
     tm = new NbStageTimer(c, NB_T_MASKS);
     ExclArgs E;
-    E.natoms = c->natoms; E.excl_off = c->excl_off.p; E.excl_idx = c->excl_idx.p; E.slot_of_atom = c->slot_of_atom.p;
+    E.natoms = c->natoms;
+    for (int k = 0; k < 3; k++) E.box[k] = c->box[k];
+    E.rl2 = rlist * rlist;
+    E.bb_lo = c->bb_lo.p; E.bb_hi = c->bb_hi.p;
+    E.excl_off = c->excl_off.p; E.excl_idx = c->excl_idx.p; E.slot_of_atom = c->slot_of_atom.p;
     E.ent_count = c->ent_count.p; E.ent_jbegin = c->ent_jbegin.p; E.jl = c->jl.p; E.imask = c->imask_outer.p;
     E.masks = nullptr; E.tot = c->tot_dev; E.caps = caps;
     if (c->nexcl) {

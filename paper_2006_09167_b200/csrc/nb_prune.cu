@@ -98,6 +98,8 @@ __device__ __forceinline__ void prune_step_masked(const float2 (&xi)[4], const f
 // One warp per block = one segment: streams its compact outer list.
 __global__ void __launch_bounds__(32) k_prune(PruneArgs A)
 {
+    nb_pdl_wait();
+    nb_pdl_trigger();
     const int t = A.order[blockIdx.x];
     const int2 n = A.ol_cnt[t];             // {cluster pairs without a mask, with a mask}
     if (n.x + n.y == 0) return;             // (an empty outer segment has an empty inner one, set at search time)
@@ -203,7 +205,7 @@ int launch_prune(nb_ctx* c, float rlist_inner, int part, int nparts, unsigned wm
         A.seg_cnt[b] = c->seg_cnt[b].p;
     }
     A.wb = part < 32 ? (int)((wmask >> part) & 1u) : 0;   // (more than 32 parts only without the two-buffer scheme: wmask = 0)
-    k_prune<<<(u1 - u0) * 8, 32, 0, st>>>(A);
+    NB_CUDA(c, nb_launch_pdl(k_prune, dim3((u1 - u0) * 8), dim3(32), 0, st, A));
     NB_LAUNCH_CHECK(c);
     return NB_OK;
 }
@@ -217,20 +219,37 @@ int set_buf_nparts(nb_ctx* c, int nparts)
         if (rc != NB_OK) return rc;
         c->buf_nparts = nparts;
     }
-    if (c->seg_part_nparts != nparts || c->seg_part_search != c->st.search_count) {
-        const int nseg = c->nunits * 8;
-        NB_CUDA(c, c->seg_part.ensure(std::max(nseg, 1), c->stream));
-        if (nseg > 0) {
-            k_seg_parts<<<(nseg + 255) / 256, 256, 0, c->stream>>>(nseg, c->segd.p, nparts, c->nunits, c->seg_part.p);
-            NB_LAUNCH_CHECK(c);
-        }
-        c->seg_part_nparts = nparts;
-        c->seg_part_search = c->st.search_count;
+    return NB_OK;
+}
+
+// The part table the force kernel reads while some part lives in inner buffer 1: needed by the overlapped mode only.
+int ensure_seg_part(nb_ctx* c)
+{
+    const int nparts = c->buf_nparts;
+    if (c->seg_part_nparts == nparts && c->seg_part_search == c->st.search_count) return NB_OK;
+    const int nseg = c->nunits * 8;
+    NB_CUDA(c, c->seg_part.ensure(std::max(nseg, 1), c->stream));
+    if (nseg > 0) {
+        k_seg_parts<<<(nseg + 255) / 256, 256, 0, c->stream>>>(nseg, c->segd.p, nparts, c->nunits, c->seg_part.p);
+        NB_LAUNCH_CHECK(c);
     }
+    c->seg_part_nparts = nparts;
+    c->seg_part_search = c->st.search_count;
     return NB_OK;
 }
 
 }  // namespace
+
+// Everything a prune of `nparts` rolling parts needs besides the kernel itself (part table, launch order), built now.
+int nbi_prepare_parts(nb_ctx* c, int nparts)
+{
+    if (nparts < 1 || nparts > 32) return NB_ERR_ARG;
+    int rc = nbi_commit_pending(c);
+    if (rc != NB_OK) return rc;
+    if ((rc = set_buf_nparts(c, nparts)) != NB_OK) return rc;
+    const int32_t* order = nullptr;
+    return nbi_prune_order(c, nparts, &order);
+}
 
 int nbi_consolidate(nb_ctx* c)
 {
@@ -296,6 +315,7 @@ int nbi_prune_overlapped(nb_ctx* c, float rlist_inner, int part, int nparts)
         c->have_buf1 = true;
     }
     if ((rc = set_buf_nparts(c, nparts)) != NB_OK) return rc;
+    if ((rc = ensure_seg_part(c)) != NB_OK) return rc;
     c->last_nparts = nparts;
     c->st.prune_count++;
     const int32_t* order = nullptr;

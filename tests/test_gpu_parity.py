@@ -502,6 +502,59 @@ def test_overlapped_prune(cfg1):
     assert rel_rms(d.forces(), oracle_forces(w, x=x, method="cells").f) <= TOL_F
 
 
+def inner_keys(d):
+    ci, ent, sv, kind, part = d.inner_dump()
+    return set(zip(ci.tolist(), ent.tolist(), LC.shift_id(sv).tolist(), kind.tolist()))
+
+
+@pytest.mark.parametrize("which", ["cfg1", "tiny"])
+def test_step_graph(which):
+    """nb_step = nb_put_atoms + nb_prune + nb_forces in one call; from the second use of a rolling part on a list
+    it is one CUDA graph launch.  Two contexts on the same box, one driven by the three calls and one by nb_step,
+    over two list lifetimes (the graphs are updated in place after the second search): identical inner lists at every
+    step, forces equal up to the order of the atomic adds and within 1e-5 of the oracle; with stage timing on
+    (plain path inside nb_step) still the same; errors before a search / after a box change."""
+    import torch
+    from paper_2006_09167_b200 import nb
+    w = W.config1() if which == "cfg1" else W.small_water(150, 2.0, seed=23, rc=0.8, rlist_outer=0.9, rlist_inner=0.84)
+    k = 2
+    a, b = Driver(w), Driver(w)
+    with pytest.raises(nb.NbError):
+        b.put()
+        b.ctx.step(b.x, w.rlist_inner, 0, k, b.f)          # no list yet
+    for life in range(2):
+        x0 = w.positions_at(10 * life)
+        for d in (a, b):
+            d.put(x0)
+            d.ctx.search(w.rlist_outer)
+            d.ctx.prune(w.rlist_inner)
+            d.forces()
+        for t in range(1, 9):
+            x = w.positions_at(10 * life + t)
+            a.put(x)
+            a.ctx.prune(w.rlist_inner, t % k, k)
+            fa = a.forces()
+            xb = torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32)).to(b.dev)
+            fb_t = torch.full((w.natoms, 3), float("nan"), dtype=torch.float32, device=b.dev)   # new buffers every step: patched in
+            if t == 6:
+                b.ctx.timing_enable(True)                  # plain path inside nb_step
+            b.ctx.step(xb, w.rlist_inner, t % k, k, fb_t)
+            if t == 6:
+                b.ctx.timing_enable(False)
+            torch.cuda.synchronize()
+            fb = fb_t.cpu().numpy().astype(np.float64)
+            assert rel_rms(fb, fa) <= 2e-6
+            if t in (1, 4, 8):
+                assert rel_rms(fb, oracle_forces(w, x=x, method="cells" if which == "cfg1" else "allpairs").f) <= TOL_F
+                assert inner_keys(a) == inner_keys(b)
+    st = b.ctx.get_stats()
+    assert st["force_count"] == a.ctx.get_stats()["force_count"] and st["prune_count"] == a.ctx.get_stats()["prune_count"]
+    bad_box = np.asarray(w.box, dtype=np.float32) * np.float32(1.01)
+    b.ctx.put_atoms(b.x, b.q, b.t, bad_box)
+    with pytest.raises(nb.NbError):
+        b.ctx.step(b.x, w.rlist_inner, 0, k, b.f)
+
+
 @pytest.mark.parametrize("which", ["cfg0", "cfg1", "rect_rf", "lj"])
 def test_fused_first_prune(which):
     """nb_forces_prune -- one kernel walks the OUTER list of a fresh search,
