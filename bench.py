@@ -464,6 +464,7 @@ def run_b200(args):
                   fused_first=args.first_prune == "fused")
     ctx = rep.ctx
     fma_peak = ctx.measure_fp32_peak()          # lane-FMA/s of a register-resident FFMA chain, this GPU, now
+    fp32_forms = ctx.measure_fp32_pipe()        # pipe occupancy of the FP32 / FP32x2 instruction forms, this GPU, now
     rep.count_pass()                            # untimed: per-frame pair and slot counts (also warms everything up)
     W = max(args.warmup, 3)
     K = args.steps
@@ -551,6 +552,10 @@ def run_b200(args):
                                "MEASURED_PEAKS.json has no FP32 entry",
                 "measured_ffma_chain_tflops": 2 * fma_peak / 1e12,
                 "frac_of_measured_ffma_chain": achieved / (2 * fma_peak / 1e12),
+                "fp32_pipe_cycles_per_warp_instruction": fp32_forms,
+                "fp32_pipe_note": "measured (nb_measure_fp32_pipe, 4 warps per sub-partition): an FFMA2 with three different register "
+                                  "pairs holds the FP32 pipe ~4 cycles (register-file bandwidth), with a repeated or constant operand "
+                                  "~2.3-2.5, a scalar FFMA ~1; the kernel's step is 124 packed instructions, see DESIGN.md section 6",
                 "flop_per_slot": flop_slot, "slots_per_launch": slots_per_launch, "kernel_us": force_us,
                 "kernel_us_is": "mean of the F-only launches (the inner steps), CUDA events on the launching stream, in a second timed "
                                 "pass over the same schedule positions (ms_per_step of that pass: ms_per_step_with_force_events); "

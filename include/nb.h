@@ -184,6 +184,12 @@ int nb_get_stats(nb_ctx*, nb_stats* out);
 /* Measures the device's FP32 FMA issue peak with a register-resident FFMA chain kernel
  * (MEASURED_PEAKS.json has no FP32 entry).  Returns lane-FMA/s in *fma_per_s. */
 int nb_measure_fp32_peak(nb_ctx*, double* fma_per_s);
+/* What the FP32 pipe really sustains for the instruction forms of the force kernel (the FP32x2 forms are bound by
+ * register-file bandwidth, not by the 128 lanes): cycles per warp instruction per SM sub-partition, 4 warps per
+ * sub-partition, everything in registers, at the device's nominal SM clock.  cycles[4] (host) = { scalar FFMA with three
+ * different register operands, FFMA2 with three different register pairs, FFMA2 pair * pair + constant-bank operand,
+ * FMUL2 with two different register pairs }.  bench.py reports them next to the roofline.  Synchronises. */
+int nb_measure_fp32_pipe(nb_ctx*, double* cycles);
 /* Counts, over the current inner list and coordinates, the atom pairs with r^2 < rc^2 that
  * interact (*n_interacting: the paper's "effective" pair count) and those
  * that are force-field exclusions (*n_excluded; they contribute only the Ewald/RF correction).

@@ -160,7 +160,19 @@ static int put_atoms_common(nb_ctx* c, const float* x, const float* q, const int
     int rcp = nbi_commit_pending(c);
     if (rcp != NB_OK) return rcp;
     NbStageTimer tm(c, NB_T_PUT);
-    const bool device = kind == cudaMemcpyDeviceToDevice;
+    bool device = kind == cudaMemcpyDeviceToDevice;
+    if (!device && !q && !type) {
+        // Positions only, from PINNED host memory (cudaHostAlloc / cudaHostRegister, as torch's pin_memory gives): the put
+        // kernel reads them in place over PCIe, coalesced, and writes both the caller-order copy and the cluster-ordered
+        // array -- one kernel instead of a staging copy followed by a refresh kernel.
+        cudaPointerAttributes pa;
+        if (cudaPointerGetAttributes(&pa, x) == cudaSuccess && pa.type == cudaMemoryTypeHost && pa.devicePointer) {
+            x = (const float*)pa.devicePointer;
+            device = true;
+        } else {
+            cudaGetLastError();
+        }
+    }
     if (!device) {
         NB_CUDA(c, cudaMemcpyAsync(c->x.p, x, sizeof(float) * 3 * n, kind, st));
         if (q) NB_CUDA(c, cudaMemcpyAsync(c->q.p, q, sizeof(float) * n, kind, st));
@@ -522,6 +534,13 @@ extern "C" int nb_measure_fp32_peak(nb_ctx* c, double* fma_per_s)
     DeviceGuard guard(c);
     if (!c || !fma_per_s) return NB_ERR_ARG;
     return nbi_measure_fp32_peak(c, fma_per_s);
+}
+
+extern "C" int nb_measure_fp32_pipe(nb_ctx* c, double* cycles)
+{
+    DeviceGuard guard(c);
+    if (!c || !cycles) return NB_ERR_ARG;
+    return nbi_measure_fp32_pipe(c, cycles);
 }
 
 extern "C" int nb_count_pairs(nb_ctx* c, int64_t* n_interacting, int64_t* n_excluded)

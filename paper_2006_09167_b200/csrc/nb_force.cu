@@ -499,6 +499,38 @@ __global__ void __launch_bounds__(256) k_fp32_peak(float* out, int iters, float 
     out[blockIdx.x * blockDim.x + threadIdx.x] = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
 }
 
+// FP32-pipe occupancy of the instruction forms the force kernel is made of, measured in place (nb_measure_fp32_pipe):
+// 8 independent accumulator pairs per thread, 4 warps per SM sub-partition, everything in registers.
+//   0: scalar FFMA, three different register operands      1: FFMA2, three different register PAIRS
+//   2: FFMA2 pair * pair + constant-bank operand            3: FMUL2, two different register pairs
+template <int MODE>
+__global__ void __launch_bounds__(128) k_fp32_forms(float* out, int iters, float2 c0)
+{
+    float2 acc[8], a[8], b[8];
+#pragma unroll
+    for (int i = 0; i < 8; i++) {
+        acc[i] = make_float2(threadIdx.x + i, i);
+        a[i] = make_float2(1.0f + 1e-6f * (threadIdx.x + i), 1.0f - 1e-6f * i);
+        b[i] = make_float2(1e-3f * i, 1e-3f * threadIdx.x);
+    }
+    for (int it = 0; it < iters; it++) {
+#pragma unroll
+        for (int r = 0; r < 4; r++) {
+#pragma unroll
+            for (int i = 0; i < 8; i++) {
+                if (MODE == 0) { acc[i].x = fmaf(a[i].x, b[(i + r) % 8].x, acc[i].x); acc[i].y = fmaf(a[i].y, b[(i + r) % 8].y, acc[i].y); }
+                if (MODE == 1) acc[i] = __ffma2_rn(a[i], b[(i + r) % 8], acc[i]);
+                if (MODE == 2) acc[i] = __ffma2_rn(acc[i], a[i], c0);
+                if (MODE == 3) acc[i] = __fmul2_rn(acc[i], a[(i + r) % 8]);
+            }
+        }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; i++) s += acc[i].x + acc[i].y;
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 // Counts atom pairs with r^2 < rc^2 over the inner list: interacting ("effective" pairs,
 // PAPER.md L167-L173) and excluded-but-counted.  Same block/warp/lane mapping as the prune kernel.
 __global__ void __launch_bounds__(256) k_count_pairs(ForceArgs A, unsigned long long* __restrict__ out)
@@ -731,6 +763,40 @@ int nbi_measure_fp32_peak(nb_ctx* c, double* fma_per_s)
     cudaEventDestroy(e1);
     out.release();
     *fma_per_s = (double)grid * 256 * iters * 64.0 / (best * 1e-3);
+    return NB_OK;
+}
+
+int nbi_measure_fp32_pipe(nb_ctx* c, double* cycles /*[4]*/)
+{
+    int khz = 0;
+    cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, c->prm.device);
+    const int grid = c->nsm * 4, iters = 2000;   // 4 blocks x 4 warps per SM = 4 warps per sub-partition
+    DevBuf<float> out;
+    NB_CUDA(c, out.ensure((size_t)grid * 128, c->stream));
+    cudaEvent_t e0, e1;
+    NB_CUDA(c, cudaEventCreate(&e0));
+    NB_CUDA(c, cudaEventCreate(&e1));
+    for (int mode = 0; mode < 4; mode++) {
+        float best = 1e30f;
+        for (int rep = 0; rep < 4; rep++) {
+            cudaEventRecord(e0, c->stream);
+            const float2 c0 = make_float2(0.5f, 0.25f);
+            if (mode == 0) k_fp32_forms<0><<<grid, 128, 0, c->stream>>>(out.p, iters, c0);
+            if (mode == 1) k_fp32_forms<1><<<grid, 128, 0, c->stream>>>(out.p, iters, c0);
+            if (mode == 2) k_fp32_forms<2><<<grid, 128, 0, c->stream>>>(out.p, iters, c0);
+            if (mode == 3) k_fp32_forms<3><<<grid, 128, 0, c->stream>>>(out.p, iters, c0);
+            cudaEventRecord(e1, c->stream);
+            NB_CUDA(c, cudaEventSynchronize(e1));
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, e0, e1);
+            if (rep > 0 && ms < best) best = ms;
+        }
+        const double warp_instr = (double)iters * 32 * (mode == 0 ? 2 : 1);   // per warp
+        cycles[mode] = best * 1e-3 * (double)khz * 1e3 / (warp_instr * 4);    // 4 warps share a sub-partition
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    out.release();
     return NB_OK;
 }
 

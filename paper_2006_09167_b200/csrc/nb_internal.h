@@ -361,6 +361,7 @@ int nbi_list_count(nb_ctx* c, int which, int64_t* n);      // nb_list.cu
 int nbi_list_dump(nb_ctx* c, int which, int32_t* ci, int32_t* cj, int32_t* shift, uint64_t* pairmask,
                   int32_t* part);
 int nbi_measure_fp32_peak(nb_ctx* c, double* fma_per_s);   // nb_force.cu
+int nbi_measure_fp32_pipe(nb_ctx* c, double* cycles);       // nb_force.cu
 int nbi_count_pairs(nb_ctx* c, int64_t* n_interacting, int64_t* n_excluded);   // nb_force.cu
 int nbi_count_slots(nb_ctx* c, int64_t* slots);            // nb_force.cu
 int nbi_inner_dump(nb_ctx* c, int64_t* n, int32_t* ci, int32_t* entry, int32_t* shift, int32_t* kind, int32_t* part);   // nb_force.cu

@@ -109,8 +109,9 @@ __global__ void __launch_bounds__(32) k_prune(PruneArgs A)
     const int wb = A.wb;
     const int32_t* __restrict__ olu = A.olu + sd.x;
     const int2* __restrict__ olm = A.olm + sd.y;
-    int32_t* il = A.il[wb] + sd.x;
-    int2* ilm = A.ilm[wb] + sd.y;
+    // (selected, not indexed: a run-time index into the kernel parameters makes ptxas copy them to local memory)
+    int32_t* il = (wb ? A.il[1] : A.il[0]) + sd.x;
+    int2* ilm = (wb ? A.ilm[1] : A.ilm[0]) + sd.y;
     const int ns = (n.x + 3) >> 2;
     int ea = ci, eb = ci, ea2 = ci, eb2 = ci;
     if (ns > 0) {
@@ -156,7 +157,7 @@ __global__ void __launch_bounds__(32) k_prune(PruneArgs A)
         if (s < ns) prune_step_unmasked(xi, yi, zi, A.rl2, ea, xa, 4 * s + g < n.x, lane, il, nu);
     }
     __syncwarp();
-    nb_ilist_finish(nu, nm, sd.x + ci, lane, A.cj_dummy, il, ilm, &A.seg_cnt[wb][t]);
+    nb_ilist_finish(nu, nm, sd.x + ci, lane, A.cj_dummy, il, ilm, (wb ? A.seg_cnt[1] : A.seg_cnt[0]) + t);
 }
 
 // Rolling part of every segment under `nparts`, looked up by the force kernel while some part lives in inner buffer 1.

@@ -24,7 +24,7 @@ NB_SHIFT_CENTER = 13
 EXPORTS = ["nb_init", "nb_put_atoms", "nb_put_atoms_host", "nb_search", "nb_prune", "nb_forces",
            "nb_forces_host", "nb_free", "nb_last_error", "nb_get_layout", "nb_get_slots", "nb_list_count",
            "nb_list_dump", "nb_get_stats", "nb_measure_fp32_peak", "nb_count_pairs", "nb_timing_enable",
-           "nb_timing_read", "nb_timing_stages", "nb_count_slots", "nb_inner_dump", "nb_prune_overlapped", "nb_forces_prune", "nb_step"]
+           "nb_timing_read", "nb_timing_stages", "nb_count_slots", "nb_inner_dump", "nb_prune_overlapped", "nb_forces_prune", "nb_step", "nb_measure_fp32_pipe"]
 NB_T_NAMES = ["put", "grid", "search", "masks", "prune", "force", "reduce", "force_energy"]
 
 
@@ -194,6 +194,11 @@ class Context:
         self._check(lib().nb_measure_fp32_peak(self._h, C.byref(v)))
         return v.value
 
+
+    def measure_fp32_pipe(self):
+        v = (C.c_double * 4)()
+        self._check(lib().nb_measure_fp32_pipe(self._h, v))
+        return {"ffma_3reg": v[0], "ffma2_3pairs": v[1], "ffma2_pair_pair_const": v[2], "fmul2_2pairs": v[3]}
 
     def count_pairs(self):
         """(interacting, excluded) atom pairs with r < rc over the inner list."""
