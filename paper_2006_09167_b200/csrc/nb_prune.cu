@@ -132,6 +132,14 @@ __global__ void __launch_bounds__(32) k_prune(PruneArgs A)
         zi[p] = make_float2(__fmaf_rn((float)sz, A.box[2], v0.z), __fmaf_rn((float)sz, A.box[2], v1.z));
     }
     int nu = 0, nm = 0;
+    // two alternating register sets (a: even steps, b: odd steps); j coordinates two steps ahead,
+    // list entries four steps ahead, indices clamped to the segment (as in the force kernel); the first two
+    // coordinate loads are in flight during the masked steps
+    float4 xa = make_float4(0.f, 0.f, 0.f, 0.f), xb = xa;
+    if (ns > 0) {
+        xa = A.xq[ea * 8 + k];
+        xb = A.xq[eb * 8 + k];
+    }
     // cluster pairs with a mask: few (about one step per zero-shift segment), no pipeline
     for (int s = 0; s < n.y; s += 4) {
         const bool valid = s + g < n.y;
@@ -140,9 +148,6 @@ __global__ void __launch_bounds__(32) k_prune(PruneArgs A)
         prune_step_masked(xi, yi, zi, A.rl2, e, x, valid, e.x == ci && sid == NB_SHIFT_CENTER, lane, ilm, nm);
     }
     if (ns > 0) {
-        // two alternating register sets (a: even steps, b: odd steps); j coordinates two steps ahead,
-        // list entries four steps ahead, indices clamped to the segment (as in the force kernel)
-        float4 xa = A.xq[ea * 8 + k], xb = A.xq[eb * 8 + k];
         int s = 0;
         for (; s + 1 < ns; s += 2) {
             prune_step_unmasked(xi, yi, zi, A.rl2, ea, xa, 4 * s + g < n.x, lane, il, nu);
