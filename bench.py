@@ -98,6 +98,8 @@ def parse_args():
     ap.add_argument("--inner-step", default="nb_step", choices=["nb_step", "calls"],
                     help="inner steps of the device leg through nb_step (one call, one CUDA graph launch) or through the three "
                          "calls nb_put_atoms / nb_prune / nb_forces; the e2e leg and the stage-timing passes always use the calls")
+    ap.add_argument("--e2e-prune", default="overlapped", choices=["overlapped", "plain"],
+                    help="e2e leg: nb_step_host (rolling prune hidden behind the host<->device copies) or put/prune/forces in sequence")
     ap.add_argument("--first-prune", default="separate", choices=["separate", "fused"],
                     help="first use of a fresh list: nb_prune(.., 0, 1) then nb_forces (separate), or the one-kernel nb_forces_prune "
                          "(fused, PAPER.md L189)")
@@ -205,6 +207,7 @@ class Replica:
         self.slots_at_frame = None
         self.overlapped = overlapped
         self.fused_first = fused_first
+        self.e2e_overlap = True
 
     def _rolling_prune(self, fr):
         w, c = self.w, self.ctx
@@ -240,17 +243,21 @@ class Replica:
             c.step(self.x_dev[fr], w.rlist_inner, fr % w.nparts, w.nparts, self.f_dev)
 
     def step_host(self, t):
-        """Host buffers in, host buffers out (the `e2e` leg): copies inside the timed region."""
+        """Host buffers in, host buffers out (the `e2e` leg): copies inside the timed region.  Inner steps go through
+        nb_step_host: the rolling prune of the NEXT step's part runs on this step's coordinates, on the library's second
+        stream, next to the device-to-host copy of the forces and the next host-to-device copy."""
         w, c = self.w, self.ctx
         fr = t % w.nstlist
-        c.put_atoms_host(self.x_host[fr].numpy(), self.q_host.numpy() if fr == 0 else None,
-                         self.t_host.numpy() if fr == 0 else None, w.box)
         if fr == 0:
+            c.put_atoms_host(self.x_host[fr].numpy(), self.q_host.numpy(), self.t_host.numpy(), w.box)
             c.search(w.rlist_outer)
             c.prune(w.rlist_inner, 0, 1)
             c.forces_host(self.f_host.numpy(), self.e_host.numpy(), self.v_host.numpy())
+        elif self.e2e_overlap and w.nparts <= 32:
+            c.step_host(self.x_host[fr].numpy(), self.f_host.numpy(), w.rlist_inner, (fr + 1) % w.nparts, w.nparts)
         else:
-            self._rolling_prune(fr)
+            c.put_atoms_host(self.x_host[fr].numpy(), None, None, w.box)
+            c.prune(w.rlist_inner, fr % w.nparts, w.nparts)
             c.forces_host(self.f_host.numpy(), None, None)
 
     def flush(self):
@@ -462,6 +469,7 @@ def run_b200(args):
     w = load_workload(args)
     rep = Replica(w, local_rank, flush=not args.no_flush, overlapped=args.prune == "overlapped" and w.nparts <= 32,
                   fused_first=args.first_prune == "fused")
+    rep.e2e_overlap = args.e2e_prune == "overlapped"
     ctx = rep.ctx
     fma_peak = ctx.measure_fp32_peak()          # lane-FMA/s of a register-resident FFMA chain, this GPU, now
     fp32_forms = ctx.measure_fp32_pipe()        # pipe occupancy of the FP32 / FP32x2 instruction forms, this GPU, now
@@ -529,6 +537,7 @@ def run_b200(args):
         e2e = {"value": sum_over_ranks(float(pairs_h)) / (ms_h_max * 1e-3), "unit": UNIT,
                "h2d_bytes_per_step": n * 12 + n * 8 / w.nstlist,        # x every step; q, type on search steps
                "d2h_bytes_per_step": n * 12 + 11 * 8 / w.nstlist,       # f every step; energies + virial on search steps
+               "prune": "nb_step_host: next step's part pruned next to the copies" if rep.e2e_overlap and w.nparts <= 32 else "plain",
                "ms_per_step": ms_h_max, "ms_search_step": pop_h["search"][0] / max(pop_h["search"][1], 1),
                "ms_inner_step": pop_h["inner"][0] / max(pop_h["inner"][1], 1)}
 

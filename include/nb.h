@@ -155,6 +155,16 @@ int nb_forces_prune(nb_ctx*, float rlist_inner, float* f, double* energies, doub
  * With stage timing on, an overlapped prune in flight or more than 32 parts it simply runs the three calls. */
 int nb_step(nb_ctx*, const float* x, float rlist_inner, int part, int nparts, float* f);
 
+/* One inner step with HOST buffers (the positions-in / forces-out exchange of PAPER.md L105), with the rolling prune
+ * hidden in the transfer gaps (L193: pruning "scheduled in chunks between force computations ... allows it to overlap
+ * other work"): x [host] natoms*3 is copied in (the copy runs next to a prune still in flight from the previous call),
+ * the forces over the current inner list are computed and copied to f [host] natoms*3, and the prune of `part` is
+ * started on the library's second stream right after the force kernel -- it overlaps the device-to-host copy, whatever
+ * the host does between two calls, and the next host-to-device copy.  Returns when f is complete (the prune may still
+ * be running).  As with nb_prune_overlapped the part pruned here, on THIS call's coordinates, is first used by the next
+ * call: pass the part the next step would have pruned, and choose rlist_inner - rc for nparts + 1 steps of motion. */
+int nb_step_host(nb_ctx*, const float* x, float* f, float rlist_inner, int part, int nparts);
+
 void nb_free(nb_ctx*);
 const char* nb_last_error(const nb_ctx*);
 

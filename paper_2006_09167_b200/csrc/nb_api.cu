@@ -156,12 +156,9 @@ static int put_atoms_common(nb_ctx* c, const float* x, const float* q, const int
         if (!finite_pos(box[k])) return nb_fail(c, NB_ERR_BOX, "box[%d] = %g is not positive", k, box[k]);
     cudaStream_t st = c->stream;
     const int n = c->natoms;
-    // an overlapped prune reads the coordinates this call overwrites: join it; its part flips to the new list here
-    int rcp = nbi_commit_pending(c);
-    if (rcp != NB_OK) return rcp;
     NbStageTimer tm(c, NB_T_PUT);
     bool device = kind == cudaMemcpyDeviceToDevice;
-    if (!device && !q && !type) {
+    if (!device && !q && !type && c->pending_part < 0) {
         // Positions only, from PINNED host memory (cudaHostAlloc / cudaHostRegister, as torch's pin_memory gives): the put
         // kernel reads them in place over PCIe, coalesced, and writes both the caller-order copy and the cluster-ordered
         // array -- one kernel instead of a staging copy followed by a refresh kernel.
@@ -174,10 +171,15 @@ static int put_atoms_common(nb_ctx* c, const float* x, const float* q, const int
         }
     }
     if (!device) {
+        // (enqueued BEFORE the join below: the staging copy does not touch what an overlapped prune reads, so the
+        // transfer and the prune run side by side)
         NB_CUDA(c, cudaMemcpyAsync(c->x.p, x, sizeof(float) * 3 * n, kind, st));
         if (q) NB_CUDA(c, cudaMemcpyAsync(c->q.p, q, sizeof(float) * n, kind, st));
         if (type) NB_CUDA(c, cudaMemcpyAsync(c->type.p, type, sizeof(int32_t) * n, kind, st));
     }
+    // an overlapped prune reads the cluster-ordered coordinates this call overwrites: join it; its part flips to the new list here
+    int rcp = nbi_commit_pending(c);
+    if (rcp != NB_OK) return rcp;
     for (int k = 0; k < 3; k++) c->box[k] = box[k];
     c->have_atoms = true;
     c->atoms_since_search = true;
@@ -414,6 +416,27 @@ extern "C" int nb_step(nb_ctx* c, const float* x, float rlist_inner, int part, i
     c->st.prune_count++;
     c->st.force_count++;
     c->st.kernel_launches += 4;
+    return NB_OK;
+}
+
+extern "C" int nb_step_host(nb_ctx* c, const float* x, float* f, float rlist_inner, int part, int nparts)
+{
+    if (!c) return NB_ERR_ARG;
+    DeviceGuard guard(c);
+    if (!x || !f) return nb_fail(c, NB_ERR_ARG, "nb_step_host: null argument");
+    if (!c->have_list || !c->have_grid) return nb_fail(c, NB_ERR_STATE, "nb_step_host without a valid list (call nb_search)");
+    if (nparts > 32) return nb_fail(c, NB_ERR_ARG, "nb_step_host: at most 32 rolling parts (got %d)", nparts);
+    int rc = prune_checks(c, rlist_inner, part, nparts);
+    if (rc != NB_OK) return rc;
+    const float box[3] = {c->box[0], c->box[1], c->box[2]};
+    if ((rc = put_atoms_common(c, x, nullptr, nullptr, box, cudaMemcpyHostToDevice)) != NB_OK) return rc;   // joins the previous prune
+    if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "nb_step_host: the box changed since the search");
+    cudaStream_t st = c->stream;
+    NB_CUDA(c, c->stage_f.ensure((size_t)3 * c->natoms, st));
+    if ((rc = nbi_forces(c, c->stage_f.p, nullptr, nullptr)) != NB_OK) return rc;
+    if ((rc = nbi_prune_overlapped(c, rlist_inner, part, nparts)) != NB_OK) return rc;   // forks here: after the force kernel and the gather
+    NB_CUDA(c, cudaMemcpyAsync(f, c->stage_f.p, sizeof(float) * 3 * c->natoms, cudaMemcpyDeviceToHost, st));
+    NB_CUDA(c, cudaStreamSynchronize(st));   // the forces are on the host; the prune may still be running
     return NB_OK;
 }
 

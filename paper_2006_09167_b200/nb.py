@@ -24,7 +24,7 @@ NB_SHIFT_CENTER = 13
 EXPORTS = ["nb_init", "nb_put_atoms", "nb_put_atoms_host", "nb_search", "nb_prune", "nb_forces",
            "nb_forces_host", "nb_free", "nb_last_error", "nb_get_layout", "nb_get_slots", "nb_list_count",
            "nb_list_dump", "nb_get_stats", "nb_measure_fp32_peak", "nb_count_pairs", "nb_timing_enable",
-           "nb_timing_read", "nb_timing_stages", "nb_count_slots", "nb_inner_dump", "nb_prune_overlapped", "nb_forces_prune", "nb_step", "nb_measure_fp32_pipe"]
+           "nb_timing_read", "nb_timing_stages", "nb_count_slots", "nb_inner_dump", "nb_prune_overlapped", "nb_forces_prune", "nb_step", "nb_measure_fp32_pipe", "nb_step_host"]
 NB_T_NAMES = ["put", "grid", "search", "masks", "prune", "force", "reduce", "force_energy"]
 
 
@@ -146,6 +146,9 @@ class Context:
 
     def step(self, x, rlist_inner, part, nparts, f):
         self._check(lib().nb_step(self._h, _dptr(x), C.c_float(rlist_inner), C.c_int(part), C.c_int(nparts), _dptr(f)))
+
+    def step_host(self, x, f, rlist_inner, part, nparts):
+        self._check(lib().nb_step_host(self._h, _hptr(x), _hptr(f), C.c_float(rlist_inner), C.c_int(part), C.c_int(nparts)))
 
     def forces_prune(self, rlist_inner, f, energies=None, virial=None):
         """The fused first prune: forces over the outer list + the whole inner list for rlist_inner in one kernel."""

@@ -555,6 +555,38 @@ def test_step_graph(which):
         b.ctx.step(b.x, w.rlist_inner, 0, k, b.f)
 
 
+def test_step_host(cfg1):
+    """nb_step_host: host positions in, host forces out, the prune of the next step's part started after the force
+    kernel on the second stream (overlapping the copies).  Forces within 1e-5 of the oracle at every step of a run
+    over two rolling parts; the part pruned by the last call equals the oracle's half-cluster list on the coordinates
+    that call saw; pinned and pageable buffers both work."""
+    import torch
+    w = cfg1
+    k = w.nparts
+    d = Driver(w)
+    d.put()
+    d.ctx.search(w.rlist_outer)
+    d.ctx.prune(w.rlist_inner)
+    d.forces()
+    f_pin = torch.zeros((w.natoms, 3), dtype=torch.float32).pin_memory()
+    x_pin = torch.zeros((w.natoms, 3), dtype=torch.float32).pin_memory()
+    f_pag = np.zeros((w.natoms, 3), dtype=np.float32)
+    for t in range(1, 9):
+        x = np.ascontiguousarray(w.positions_at(t), dtype=np.float32)
+        if t % 3:
+            x_pin.numpy()[:] = x
+            d.ctx.step_host(x_pin.numpy(), f_pin.numpy(), w.rlist_inner, (t + 1) % k, k)
+            f = f_pin.numpy().astype(np.float64)
+        else:
+            d.ctx.step_host(x, f_pag, w.rlist_inner, (t + 1) % k, k)
+            f = f_pag.astype(np.float64)
+        assert rel_rms(f, oracle_forces(w, x=x, method="cells").f) <= TOL_F
+    # the last call pruned part (8 + 1) % k on x_8: join it by putting x_8 again, then compare that part with the oracle
+    d.put(w.positions_at(8))
+    check_half_list(d, w, c_ranges=spread_ranges(d.ctx.get_layout()["nclusters"], 6, 24), part=9 % k)
+    assert rel_rms(d.forces(), oracle_forces(w, x=w.positions_at(8), method="cells").f) <= TOL_F
+
+
 @pytest.mark.parametrize("which", ["cfg0", "cfg1", "rect_rf", "lj"])
 def test_fused_first_prune(which):
     """nb_forces_prune -- one kernel walks the OUTER list of a fresh search,
