@@ -92,9 +92,10 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-flush", action="store_true", help="do not flush L2 between timed steps")
-    ap.add_argument("--prune", default="plain", choices=["plain", "overlapped"],
-                    help="rolling prune on the caller's stream before the force kernel (plain) or on the library's second "
-                         "stream next to it (overlapped, PAPER.md L193)")
+    ap.add_argument("--prune", default="auto", choices=["auto", "plain", "overlapped"],
+                    help="rolling prune on the caller's stream before the force kernel (plain), on the library's second "
+                         "stream next to it (overlapped, PAPER.md L193: the part pruned on this step's coordinates is first "
+                         "used by the next step), or whichever of the two is faster over a short untimed trial (auto)")
     ap.add_argument("--inner-step", default="nb_step", choices=["nb_step", "calls"],
                     help="inner steps of the device leg through nb_step (one call, one CUDA graph launch) or through the three "
                          "calls nb_put_atoms / nb_prune / nb_forces; the e2e leg and the stage-timing passes always use the calls")
@@ -489,6 +490,19 @@ def run_b200(args):
     # the force kernel timed, 13-26 % with every stage timed).  The force kernel (the roofline's kernel) is timed with
     # CUDA events in a second pass over the same schedule positions, the remaining stages in a third.
     ctx.timing_enable(False)
+    prune_trial = None
+    if args.prune == "auto" and w.nparts <= 32:
+        # untimed trial: 24 inner steps of each mode (after their own warm-up), the faster one is benched
+        trial_pos = [0] + list(range(1, 25))
+        prune_trial = {}
+        for mode in ("plain", "overlapped"):
+            rep.overlapped = mode == "overlapped"
+            fn = rep.step_device_graph if (args.inner_step == "nb_step" and not rep.overlapped) else rep.step_device
+            for t in trial_pos[:9]:
+                fn(t)
+            pop_t = rep.timed(fn, trial_pos)
+            prune_trial[mode] = pop_t["inner"][0] / pop_t["inner"][1]
+        rep.overlapped = prune_trial["overlapped"] < prune_trial["plain"]
     use_step = args.inner_step == "nb_step" and not rep.overlapped
     step_value = rep.step_device_graph if use_step else rep.step_device
     for i in range(W):
@@ -507,11 +521,13 @@ def run_b200(args):
     ctx.timing_stages(force_bit)
     ctx.timing_enable(True)
     ctx.timing_read(reset=True)
+    # (plain prune in both stage passes: the stage timer brackets launches on the caller's stream, and the force kernel
+    # is to be timed alone, not next to a prune on the second stream)
+    was_overlapped, rep.overlapped = rep.overlapped, False
     pop_f = rep.timed(rep.step_device, positions)
     stages = ctx.timing_read(reset=True)
-    # third pass, plain prune (the stage timer brackets launches on the caller's stream): the other stages
+    # third pass: the other stages
     ctx.timing_stages(0xFFFFFFFF & ~force_bit)
-    was_overlapped, rep.overlapped = rep.overlapped, False
     rep.timed(rep.step_device, positions)
     rep.overlapped = was_overlapped
     stages_other = ctx.timing_read(reset=True)
@@ -569,7 +585,8 @@ def run_b200(args):
                                   "~2.3-2.5, a scalar FFMA ~1; the kernel's step is 124 packed instructions, see DESIGN.md section 6",
                 "flop_per_slot": flop_slot, "slots_per_launch": slots_per_launch, "kernel_us": force_us,
                 "kernel_us_is": "mean of the F-only launches (the inner steps), CUDA events on the launching stream, in a second timed "
-                                "pass over the same schedule positions (ms_per_step of that pass: ms_per_step_with_force_events); "
+                                "pass over the same schedule positions with the plain prune, i.e. the kernel alone (ms_per_step of that "
+                                "pass: ms_per_step_with_force_events); "
                                 "the F+E+virial launches of the search steps are stage_us.force_energy",
                 "ms_per_step_with_force_events": ms_step_f}
 
@@ -610,7 +627,9 @@ def run_b200(args):
                 "ms_per_step": ms_step_max, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic",
                 "config": workload_config(w, args, {"l2": "flushed between timed steps (256 MiB fill)" if not args.no_flush
-                                                    else "not flushed", "prune": "overlapped" if rep.overlapped else "plain",
+                                                    else "not flushed", "prune": ("overlapped (second stream, next to the force kernel; the part pruned on this step's coordinates "
+                                                              "is first used by the next step)" if rep.overlapped else "plain (before the force kernel)"),
+                                                    "prune_trial_ms_inner_step": prune_trial,
                                                     "first_prune": args.first_prune,
                                                     "inner_step": "nb_step (CUDA graph)" if use_step else "three calls"}),
                 "schedule": {"timed_inner_steps": pop["inner"][1], "timed_search_steps": S, "ms_inner_step": ms_inner,
