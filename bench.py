@@ -9,7 +9,8 @@ One "step" is one MD step of the whole hot path on the synthetic water box, in t
 schedule: every step stages new coordinates
 (nb_put_atoms) and computes forces (nb_forces); every nstlist-th step first rebuilds the grid and
 the outer pair list (nb_search) and prunes it fully; every other step prunes one rolling part of
-the outer list (nb_prune) before the forces.  Whatever --steps is, BOTH kinds of step are timed in
+the outer list, before the forces (nb_prune) or next to them on a second stream (nb_prune_overlapped,
+PAPER.md L193; --prune auto benches the faster).  Whatever --steps is, BOTH kinds of step are timed in
 the same run: K inner steps and S = max(3, ceil(K/nstlist)) search steps (the schedule is restarted
 S times), and ms_per_step = (mean search step + (nstlist-1) * mean inner step) / nstlist is the cost
 of a step in the proportions the method prescribes -- every row of SURVEY 8(a) is inside it.
