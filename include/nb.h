@@ -17,8 +17,10 @@
  *    synchronising, except nb_search (one synchronisation at its end to read the list sizes
  *    back) and the introspection / _host calls.  Every call switches to the context's device
  *    and restores the caller's current device before returning.
- *  - Call order: nb_init -> nb_put_atoms -> nb_search -> { nb_put_atoms -> [nb_prune] ->
- *    nb_forces }* -> nb_put_atoms -> nb_search ...; violations return NB_ERR_STATE.
+ *  - Call order: nb_init -> nb_put_atoms -> nb_search -> { nb_put_atoms -> [nb_prune | nb_prune_overlapped]
+ *    -> nb_forces }* -> nb_put_atoms -> nb_search ...; violations return NB_ERR_STATE.  The first use of a
+ *    fresh list may be nb_forces_prune instead of nb_prune + nb_forces; nb_step / nb_step_host are one pass
+ *    of the braces in one call.
  *  - Units: nm, kJ/mol, e.  Rectangular periodic boxes only.  natoms, types, charges'
  *    layout and exclusions are fixed for the lifetime of a context (only
  *    positions change per step).
