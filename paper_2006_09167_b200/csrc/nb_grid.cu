@@ -154,7 +154,8 @@ __device__ __forceinline__ void slab_segment_sort(SlabScratch& s, const float4* 
 
 // One block per grid column: bitonic z-sort of the column in shared memory, then one warp per
 // 64-atom slab does the 2x2x2 sub-sorts and writes the cluster-ordered arrays and bounding boxes.
-__global__ void __launch_bounds__(256)
+#define NB_LAYOUT_WARPS 16   // warps per column block: one per 64-atom slab in flight (a column of config 2 holds 13 slabs)
+__global__ void __launch_bounds__(32 * NB_LAYOUT_WARPS)
 k_col_layout(int ncy, const int* __restrict__ col_atom_off, const int* __restrict__ col_sc_off,
              const int* __restrict__ col_atoms, const float4* __restrict__ xw_atom,
              const int* __restrict__ type, int pad_type, int np2_max, float4* __restrict__ xq,
@@ -163,7 +164,7 @@ k_col_layout(int ncy, const int* __restrict__ col_atom_off, const int* __restric
              float4* __restrict__ sbb_hi, float3 pad_base, float3 pad_step, NbTotals* __restrict__ tot)
 {
     extern __shared__ unsigned long long s_keys[];
-    __shared__ SlabScratch s_slab[8];
+    __shared__ SlabScratch s_slab[NB_LAYOUT_WARPS];
     int col = blockIdx.x;
     int a0 = col_atom_off[col], n = col_atom_off[col + 1] - a0;
     if (n == 0) return;
@@ -199,7 +200,7 @@ k_col_layout(int ncy, const int* __restrict__ col_atom_off, const int* __restric
     int nslab = (n + NB_SC_ATOMS - 1) / NB_SC_ATOMS;
     int sc0 = col_sc_off[col];
     SlabScratch& s = s_slab[warp];
-    for (int slab = warp; slab < nslab; slab += 8) {
+    for (int slab = warp; slab < nslab; slab += NB_LAYOUT_WARPS) {
 #pragma unroll
         for (int h = 0; h < 2; h++) {
             int e = lane + 32 * h, idx = slab * NB_SC_ATOMS + e;
@@ -421,7 +422,7 @@ int nbi_grid(nb_ctx* c)
         pd[k] = (float)(L[k] / (floor(L[k] / 3.0) + 0.5));   // L/d half-integer, d in (2, 6] nm (2L for L < 3)
         pb[k] = (float)(-(2.0 * L[k] + 8.0));
     }
-    k_col_layout<<<c->ncol, 256, smem, st>>>(c->ncy, c->col_atom_off.p, c->col_sc_off.p, c->col_atoms.p,
+    k_col_layout<<<c->ncol, 32 * NB_LAYOUT_WARPS, smem, st>>>(c->ncy, c->col_atom_off.p, c->col_sc_off.p, c->col_atoms.p,
                                              c->xw_atom.p, c->type.p, c->ntypes, np2, c->xq.p, c->type_slot.p,
                                              c->atom_of_slot.p, c->slot_of_atom.p, c->bb_lo.p, c->bb_hi.p,
                                              c->sbb_lo.p, c->sbb_hi.p, make_float3(pb[0], pb[1], pb[2]),
