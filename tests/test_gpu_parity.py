@@ -219,6 +219,33 @@ def test_lj_only_flavour():
     assert e[1] == 0.0 and abs(e[0] - ref.e_lj) / abs(ref.e_lj) <= TOL_E
 
 
+def test_many_atom_types():
+    """NB_MAX_TYPES - 1 = 95 LJ types (the paired LJ table of a block is then 6 KB of shared memory, the per-cluster rows
+    95 x 64 B): a charged LJ mixture without exclusions, every flavour's forces / energies against the all-pairs oracle."""
+    import dataclasses
+    base = W.lj_fluid(12, rc=0.9)
+    rng = np.random.Generator(np.random.PCG64(95))
+    nt = 95
+    sigma, eps = rng.uniform(0.25, 0.38, nt), rng.uniform(0.2, 1.0, nt)
+    q = rng.uniform(-0.5, 0.5, base.natoms).astype(np.float32)
+    q -= np.float32(q.mean())
+    w = dataclasses.replace(base, type=rng.integers(0, nt, base.natoms).astype(np.int32), q=q, ntypes=nt,
+                            lj_c6c12=W.lj_table(sigma, eps), coulomb="ewald")
+    for coulomb in ("ewald", "rf", "none"):
+        ww = dataclasses.replace(w, coulomb=coulomb)
+        d = Driver(ww)
+        d.put()
+        d.ctx.search(ww.rlist_outer)
+        d.ctx.prune(ww.rlist_inner)
+        ref = oracle_forces(ww)
+        f, e, vir = d.forces(energy=True, virial=True)
+        assert rel_rms(f, ref.f) <= TOL_F
+        assert abs(e.sum() - ref.energy) / abs(ref.energy) <= TOL_E
+        assert np.linalg.norm(vir - ref.virial) / np.linalg.norm(ref.virial) <= TOL_E
+        assert rel_rms(d.forces(), ref.f) <= TOL_F
+        d.ctx.close()
+
+
 def test_modifiers_none_and_finite_eps_rf(small_rect):
     w = small_rect
     from paper_2006_09167_b200 import nb
@@ -568,6 +595,17 @@ def test_step_graph(which):
                 assert inner_keys(a) == inner_keys(b)
     st = b.ctx.get_stats()
     assert st["force_count"] == a.ctx.get_stats()["force_count"] and st["prune_count"] == a.ctx.get_stats()["prune_count"]
+    # more keys than the cache holds (8): ten inner radii, three uses each (plain, capture, graph launch), evicting as it goes
+    x = w.positions_at(19)
+    xb = torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32)).to(b.dev)
+    fb_t = torch.empty((w.natoms, 3), dtype=torch.float32, device=b.dev)
+    ref = oracle_forces(w, x=x, method="cells" if which == "cfg1" else "allpairs").f
+    for i in range(10):
+        rl = w.rlist_inner + 1e-4 * i
+        for _ in range(3):
+            b.ctx.step(xb, rl, 1, k, fb_t)
+        torch.cuda.synchronize()
+        assert rel_rms(fb_t.cpu().numpy().astype(np.float64), ref) <= TOL_F
     bad_box = np.asarray(w.box, dtype=np.float32) * np.float32(1.01)
     b.ctx.put_atoms(b.x, b.q, b.t, bad_box)
     with pytest.raises(nb.NbError):
