@@ -521,33 +521,34 @@ long long oracle_lists(int nclusters, int C, const int32_t* atom_of_slot, const 
 }
 
 /*
- * The inner list at HALF j-cluster granularity (DESIGN.md section 5 "compact inner list"; the
- * paper's "splitting j-clusters" while pruning: the search's cluster pairs are "pruned
- * into" narrower ones).  This is the list the force kernel streams, so it gets its own definition:
+ * The inner list at SUB-cluster granularity on the j side (DESIGN.md section 5 "compact inner list", reading A22; the
+ * paper's "splitting j-clusters" while pruning: the search's cluster pairs are "pruned into" narrower ones).
+ * This is the list the force kernel streams, so it gets its own definition, for groups of G consecutive j atoms
+ * (G = C/2: half j-clusters, the paper's 8x4 shape; G = 1: single j atoms):
  *
  *   for every canonical triple (ci,cj,s) of S_outer (bb predicate, as in oracle_lists):
  *     - if its pair mask is NOT trivial (some pair of real atoms is excluded, or the triple is the
  *       zero-shift diagonal ci == cj): the WHOLE cluster pair is kept iff inner_test() holds
  *       -> one entry {ci, cj, s, kind 1};
- *     - else, for each half h in {0,1} of cj (atoms h*C/2 .. h*C/2 + C/2 - 1): the half is kept iff
- *       some real atom of the half is within fl32(rlist_inner^2) of some real atom of ci (A12 order)
- *       -> one entry {ci, 2*cj + h, s, kind 0}.
+ *     - else, for each group h in 0 .. C/G - 1 of cj (atoms h*G .. h*G + G - 1): the group is kept iff
+ *       some real atom of the group is within fl32(rlist_inner^2) of some real atom of ci (A12 order)
+ *       -> one entry {ci, (C/G)*cj + h, s, kind 0}     (G = 1: the entry is the j atom's slot).
  *
- * Same enumeration, sub-range rule, return value and output order (ci, cj, s, then kind-0 halves
+ * Same enumeration, sub-range rule, return value and output order (ci, cj, s, then kind-0 groups
  * in h order) as oracle_lists.  Pins: tests/test_oracle_lists.py (numpy recomputation on a layout
- * the test makes up, union-of-halves == inner flag of oracle_lists, completeness by k-d tree).
+ * the test makes up, union-of-groups == inner flag of oracle_lists, completeness by k-d tree).
  */
-long long oracle_half_lists(int nclusters, int C, const int32_t* atom_of_slot, const float* xq, const float* box,
-                            float rlist_outer, float rlist_inner, const int32_t* excl_off, const int32_t* excl_idx,
-                            int c_begin, int c_end, long long cap, int32_t* out_ci, int32_t* out_entry,
-                            int8_t* out_s /*[cap*3]*/, uint8_t* out_kind)
+static long long group_lists(int nclusters, int C, int G, const int32_t* atom_of_slot, const float* xq, const float* box,
+                             float rlist_outer, float rlist_inner, const int32_t* excl_off, const int32_t* excl_idx,
+                             int c_begin, int c_end, long long cap, int32_t* out_ci, int32_t* out_entry,
+                             int8_t* out_s /*[cap*3]*/, uint8_t* out_kind)
 {
     float* lo = (float*)malloc(sizeof(float) * 3 * (size_t)nclusters);
     float* hi = (float*)malloc(sizeof(float) * 3 * (size_t)nclusters);
     int32_t* nv = (int32_t*)malloc(sizeof(int32_t) * (size_t)nclusters);
     oracle_cluster_bb(nclusters, C, atom_of_slot, xq, lo, hi, nv);
     float ro2 = rlist_outer * rlist_outer, ri2 = rlist_inner * rlist_inner;   /* fl32(r*r) */
-    const int H = C / 2;
+    const int H = G, NG = C / G;   /* atoms per group, groups per j-cluster */
     long long total = 0;
     long long* cnt = (long long*)calloc((size_t)nclusters + 1, sizeof(long long));
     for (int pass = 0; pass < 2; pass++) {
@@ -581,7 +582,7 @@ long long oracle_half_lists(int nclusters, int C, const int32_t* atom_of_slot, c
                                 }
                                 continue;
                             }
-                            for (int h = 0; h < 2; h++) {
+                            for (int h = 0; h < NG; h++) {
                                 int keep = 0;
                                 for (int a = 0; a < C && !keep; a++) {
                                     if (atom_of_slot[ci * C + a] < 0) continue;
@@ -592,7 +593,7 @@ long long oracle_half_lists(int nclusters, int C, const int32_t* atom_of_slot, c
                                 }
                                 if (!keep) continue;
                                 if (pass && k < cap) {
-                                    out_ci[k] = ci; out_entry[k] = 2 * cj + h; out_kind[k] = 0;
+                                    out_ci[k] = ci; out_entry[k] = NG * cj + h; out_kind[k] = 0;
                                     out_s[3 * k] = (int8_t)sx; out_s[3 * k + 1] = (int8_t)sy; out_s[3 * k + 2] = (int8_t)sz;
                                 }
                                 k++;
@@ -608,4 +609,25 @@ long long oracle_half_lists(int nclusters, int C, const int32_t* atom_of_slot, c
     }
     free(lo); free(hi); free(nv); free(cnt);
     return total;
+}
+
+/* G = C/2: half j-clusters (entry = 2*cj + half). */
+long long oracle_half_lists(int nclusters, int C, const int32_t* atom_of_slot, const float* xq, const float* box,
+                            float rlist_outer, float rlist_inner, const int32_t* excl_off, const int32_t* excl_idx,
+                            int c_begin, int c_end, long long cap, int32_t* out_ci, int32_t* out_entry,
+                            int8_t* out_s /*[cap*3]*/, uint8_t* out_kind)
+{
+    return group_lists(nclusters, C, C / 2, atom_of_slot, xq, box, rlist_outer, rlist_inner, excl_off, excl_idx, c_begin, c_end, cap,
+                       out_ci, out_entry, out_s, out_kind);
+}
+
+/* G = 1: single j atoms (entry = the j atom's slot index cj*C + b): a j atom of an unmasked cluster pair is listed for
+ * the i-cluster iff it is within rlist_inner of one of its real atoms. */
+long long oracle_atom_lists(int nclusters, int C, const int32_t* atom_of_slot, const float* xq, const float* box,
+                            float rlist_outer, float rlist_inner, const int32_t* excl_off, const int32_t* excl_idx,
+                            int c_begin, int c_end, long long cap, int32_t* out_ci, int32_t* out_entry,
+                            int8_t* out_s /*[cap*3]*/, uint8_t* out_kind)
+{
+    return group_lists(nclusters, C, 1, atom_of_slot, xq, box, rlist_outer, rlist_inner, excl_off, excl_idx, c_begin, c_end, cap,
+                       out_ci, out_entry, out_s, out_kind);
 }

@@ -195,7 +195,7 @@ class HalfListResult:
 
 
 def half_lists(atom_of_slot, xq, box, rlist_outer, rlist_inner, excl_off, excl_idx, cluster_size=8,
-               c_begin=0, c_end=None) -> HalfListResult:
+               c_begin=0, c_end=None, fn="oracle_half_lists") -> HalfListResult:
     """The inner list at half-j-cluster granularity (oracle_half_lists) on the exported layout."""
     aos = np.ascontiguousarray(atom_of_slot, dtype=np.int32)
     xq32 = np.ascontiguousarray(xq, dtype=np.float32).reshape(-1, 4)
@@ -207,14 +207,14 @@ def half_lists(atom_of_slot, xq, box, rlist_outer, rlist_inner, excl_off, excl_i
     ncl = aos.shape[0] // cluster_size
     if c_end is None:
         c_end = ncl
-    lib().oracle_half_lists.restype = C.c_longlong
+    getattr(lib(), fn).restype = C.c_longlong
     cap = 0
     for _ in range(2):
         ci = np.zeros(max(cap, 1), dtype=np.int32)
         ent = np.zeros(max(cap, 1), dtype=np.int32)
         s = np.zeros((max(cap, 1), 3), dtype=np.int8)
         kind = np.zeros(max(cap, 1), dtype=np.uint8)
-        n = lib().oracle_half_lists(C.c_int(ncl), C.c_int(cluster_size), _ptr(aos), _ptr(xq32), _ptr(b32),
+        n = getattr(lib(), fn)(C.c_int(ncl), C.c_int(cluster_size), _ptr(aos), _ptr(xq32), _ptr(b32),
                                     C.c_float(rlist_outer), C.c_float(rlist_inner), _ptr(eo), _ptr(ei),
                                     C.c_int(c_begin), C.c_int(c_end), C.c_longlong(cap), _ptr(ci), _ptr(ent),
                                     _ptr(s), _ptr(kind))
@@ -222,3 +222,9 @@ def half_lists(atom_of_slot, xq, box, rlist_outer, rlist_inner, excl_off, excl_i
             return HalfListResult(ci[:n], ent[:n], s[:n], kind[:n])
         cap = int(n)
     raise RuntimeError("oracle_half_lists: count changed between passes")
+
+
+def atom_lists(atom_of_slot, xq, box, rlist_outer, rlist_inner, excl_off, excl_idx, cluster_size=8, c_begin=0, c_end=None):
+    """The inner list at single-j-ATOM granularity (oracle_atom_lists): kind-0 entries are j slot indices."""
+    return half_lists(atom_of_slot, xq, box, rlist_outer, rlist_inner, excl_off, excl_idx, cluster_size, c_begin, c_end,
+                      fn="oracle_atom_lists")

@@ -254,3 +254,68 @@ def test_half_lists_against_numpy(small):
     cj_full = np.where(hl.kind == 0, hl.entry // 2, hl.entry)
     sel = ((hl.ci >= 3) & (hl.ci < 6)) | ((cj_full >= 3) & (cj_full < 6))
     assert np.array_equal(np.sort(hl.keys()[sel]), np.sort(part.keys()))
+
+
+def test_atom_lists_against_numpy(small):
+    """oracle_atom_lists (reading A22, single-j-atom granularity) recomputed in numpy float32 on a test-made layout:
+    whole masked cluster pairs, and of the unmasked ones exactly the real j atoms that have a real i atom of the cluster
+    within fl32(rlist_inner^2), bit-exact as sets; consistent with oracle_lists (spanned cluster pairs = inner triples)
+    and with oracle_half_lists (a half is listed iff one of its atoms is); every atom pair within rlist_inner is covered
+    (k-d tree, fp64); no padding slot is ever listed; a sub-range is a selection of the full enumeration."""
+    w = small
+    aos, xq = _simple_layout(w)
+    res = O.lists(aos, xq, w.box, w.rlist_outer, w.rlist_inner, w.excl_off, w.excl_idx)
+    hl = O.half_lists(aos, xq, w.box, w.rlist_outer, w.rlist_inner, w.excl_off, w.excl_idx)
+    al = O.atom_lists(aos, xq, w.box, w.rlist_outer, w.rlist_inner, w.excl_off, w.excl_idx)
+    assert np.unique(al.keys()).size == al.keys().size
+    valid = (aos >= 0).reshape(-1, 8)
+    full = np.zeros(res.ci.size, dtype=np.uint64)
+    for a in range(8):
+        for b in range(8):
+            full |= (valid[res.ci, a] & valid[res.cj, b]).astype(np.uint64) << np.uint64(a * 8 + b)
+    masked = res.pairmask != full
+    diag = (res.ci == res.cj) & (res.s == 0).all(axis=1)
+    ri2 = np.float32(w.rlist_inner) * np.float32(w.rlist_inner)
+    si = res.ci[:, None] * 8 + np.arange(8)[None, :]
+    sj = res.cj[:, None] * 8 + np.arange(8)[None, :]
+    d2 = _atom_d2_np(xq, si, sj, res.s.astype(np.int64), w.box)       # [n, 8 (i atom), 8 (j atom)]
+    ok = valid[res.ci][:, :, None] & valid[res.cj][:, None, :]
+    close = (d2 < ri2) & ok
+    upper = np.triu(np.ones((8, 8), bool), 1)
+    close_m = np.where(diag[:, None, None], close & upper[None], close)
+    sid = LC.shift_id(res.s)
+    want = set()
+    for k in range(res.ci.size):
+        if masked[k]:
+            if close_m[k].any():
+                want.add((int(res.ci[k]), int(res.cj[k]), int(sid[k]), 1))
+        else:
+            for b in np.nonzero(close[k].any(axis=0))[0]:
+                want.add((int(res.ci[k]), 8 * int(res.cj[k]) + int(b), int(sid[k]), 0))
+    got = set(zip(al.ci.tolist(), al.entry.tolist(), LC.shift_id(al.s).tolist(), al.kind.tolist()))
+    assert got == want and sum(1 for g in got if g[3] == 0) > 1000
+    assert all(aos[e] >= 0 for _, e, _, kd in got if kd == 0)          # padding slots are never listed
+    # the cluster pairs spanned by the entries are exactly the inner triples of oracle_lists
+    spanned = {(c, e // 8 if kd == 0 else e, k) for c, e, k, kd in got}
+    inner = set(zip(res.ci[res.inner].tolist(), res.cj[res.inner].tolist(), sid[res.inner].tolist()))
+    assert spanned == inner
+    # a half j-cluster is listed iff one of its atoms is; masked entries are the same
+    half = set(zip(hl.ci.tolist(), hl.entry.tolist(), LC.shift_id(hl.s).tolist(), hl.kind.tolist()))
+    assert {(c, e // 4, k, 0) for c, e, k, kd in got if kd == 0} == {h for h in half if h[3] == 0}
+    assert {g for g in got if g[3] == 1} == {h for h in half if h[3] == 1}
+    # strictly finer than halves: fewer atom entries than 4 per listed half
+    n_atoms, n_halves = sum(1 for g in got if g[3] == 0), sum(1 for h in half if h[3] == 0)
+    assert 0.5 * 4 * n_halves < n_atoms < 0.95 * 4 * n_halves
+    # completeness in fp64, layout-independent (k-d tree): every atom pair closer than rlist_inner is covered, from either side
+    pi, pj, sp, _ = LC.close_atom_pairs(aos, xq, w.box, w.rlist_inner - 1e-6)
+    ka, kb = LC.shift_id(sp), LC.shift_id(-sp)
+    miss = 0
+    for a, b, k1, k2 in zip(pi.tolist(), pj.tolist(), ka.tolist(), kb.tolist()):
+        if not ((a // 8, b, k1, 0) in got or (b // 8, a, k2, 0) in got
+                or (a // 8, b // 8, k1, 1) in got or (b // 8, a // 8, k2, 1) in got):
+            miss += 1
+    assert miss == 0 and pi.size > 1000
+    part = O.atom_lists(aos, xq, w.box, w.rlist_outer, w.rlist_inner, w.excl_off, w.excl_idx, c_begin=3, c_end=6)
+    cj_full = np.where(al.kind == 0, al.entry // 8, al.entry)
+    sel = ((al.ci >= 3) & (al.ci < 6)) | ((cj_full >= 3) & (cj_full < 6))
+    assert np.array_equal(np.sort(al.keys()[sel]), np.sort(part.keys()))
