@@ -87,7 +87,7 @@ typedef struct {
     int64_t n_excl_masks;            /* joint entries carrying a non-trivial exclusion mask */
     int64_t n_work_units;            /* list chunks scheduled by the force/prune kernels (L199-L201) */
     int64_t slots_last_forces;       /* atom-pair slots the force kernel evaluates over the current inner list (= nb_count_slots):
-                                        32 per surviving half j-cluster, 64 per masked cluster pair; 0 before the first nb_forces */
+                                        8 per listed j atom (x 8 i atoms), 64 per masked cluster pair; 0 before the first nb_forces */
     int64_t kernel_launches;         /* kernels launched by this context so far */
     int64_t search_count, prune_count, force_count;
     int32_t list_grow_retries;       /* searches repeated because a list buffer sized from the previous search was too small */
@@ -186,8 +186,8 @@ int nb_list_dump(nb_ctx*, int which, int32_t* ci, int32_t* cj, int32_t* shift, u
                  int32_t* part);
 /* Dumps the COMPACT inner list the force kernel streams (for parity tests; slow, synchronises).
  * HOST arrays of *n entries, any may be NULL; call with all NULL to get *n.  Entry k: i-cluster ci[k],
- * shift[k] (as in nb_list_dump), kind[k] = 0: entry[k] is a half j-cluster index 2*cj + half (atoms
- * 4*entry .. 4*entry+3, a cluster pair without a mask, kept at half-cluster granularity);
+ * shift[k] (as in nb_list_dump), kind[k] = 0: entry[k] is the SLOT of one j atom (of a cluster pair without a
+ * mask: the list is kept at single-j-atom granularity, the atom is listed iff it is within rlist_inner of an atom of ci);
  * kind[k] = 1: entry[k] is a whole j-cluster cj whose pair with ci carries a mask; part[k]: rolling
  * part of the entry under the nparts of the last prune call.  Padding (dummy) entries are left out.
  * An overlapped prune still in flight is joined first. */
@@ -208,8 +208,8 @@ int nb_measure_fp32_pipe(nb_ctx*, double* cycles);
  * Host outputs; either may be NULL.  Synchronises. */
 int nb_count_pairs(nb_ctx*, int64_t* n_interacting, int64_t* n_excluded);
 /* Atom-pair slots the force kernel evaluates over the current inner list (the paper's "raw" pair
- * count, L167): the inner list is kept at half-j-cluster granularity (8 x 4 atoms = 32 slots per
- * entry; cluster pairs that carry an exclusion mask stay whole, 64 slots).  Host output.  Synchronises. */
+ * count, L167): 8 slots (the 8 i atoms) per listed j atom of the cluster pairs without a mask; cluster pairs that carry
+ * an exclusion mask stay whole, 64 slots.  Host output.  Synchronises. */
 int nb_count_slots(nb_ctx*, int64_t* slots);
 
 /* Per-stage device timing with CUDA events on the context's stream ("CUDA events

@@ -232,22 +232,20 @@ __global__ void __launch_bounds__(32, PRUNE ? 8 : 16) k_force(ForceArgs A)
     int32_t* il_w = PRUNE ? A.il_w + sd.x : nullptr;
     int2* ilm_w = PRUNE ? A.ilm_w + sd.y : nullptr;
     int nu_w = 0, nm_w = 0;
-    // unmasked steps: 8 half-clusters (4 atoms each) per step; PRUNE: 4 whole clusters per step
-    const int ns = PRUNE ? (cnt.x + 3) >> 2 : cnt.x >> 3;
-    const int g8 = PRUNE ? g : lane >> 2, k4 = PRUNE ? k : lane & 3;   // lane -> (entry of the step, atom in it)
-    constexpr int EPS = PRUNE ? 4 : 8, APE = PRUNE ? 8 : 4;          // entries per step, atoms per entry
-    // PRUNE: the last step may be partly filled; its spare lanes take a dummy cluster (far from everything:
-    // no force, no survivor; nb_grid.cu)
+    // unmasked steps: 32 listed j atoms per step, one per lane; PRUNE: the outer list, 4 whole clusters per step
+    const int ns = PRUNE ? (cnt.x + 3) >> 2 : cnt.x >> 5;
+    // this lane's j SLOT in step s.  PRUNE: the last step may be partly filled; its spare lanes take a dummy cluster
+    // (far from everything: no force, no survivor; nb_grid.cu)
     auto entry = [&](int s) {
-        if (!PRUNE) return il[EPS * s + g8];
-        const int idx = EPS * s + g8, v = il[min(idx, max(cnt.x - 1, 0))];
-        return idx < cnt.x ? v : A.cj_dummy;
+        if (!PRUNE) return il[32 * s + lane];
+        const int idx = 4 * s + g, v = il[min(idx, max(cnt.x - 1, 0))];
+        return (idx < cnt.x ? v : A.cj_dummy) * 8 + k;
     };
     // first list entries of both loops are requested before anything else is waited for
     int cj = 0, cj_n = 0;
     if (ns > 0) {
-        cj = entry(0) * APE + k4;              // unmasked path: cj* hold this lane's j SLOT
-        cj_n = entry(min(1, ns - 1)) * APE + k4;
+        cj = entry(0);                         // unmasked path: cj* hold this lane's j SLOT
+        cj_n = entry(min(1, ns - 1));
     }
     // ... and so is the first step of the masked loop (its loads chain entry -> atoms -> mask)
     int2 ce_next = g < cnt.y ? ilm[g] : make_int2(ci, 0);
@@ -308,26 +306,24 @@ __global__ void __launch_bounds__(32, PRUNE ? 8 : 16) k_force(ForceArgs A)
     float4 xj1 = xj;
     int tj1 = tj;
     if (ns > 0) {
-        cj2 = entry(min(2, ns - 1)) * APE + k4;
-        cj3 = entry(min(3, ns - 1)) * APE + k4;
+        cj2 = entry(min(2, ns - 1));
+        cj3 = entry(min(3, ns - 1));
         xj1 = A.xq[cj_n];
         tj1 = A.type_slot[cj_n];
     }
 #pragma unroll 2   // (unroll 3, the period of the rotation below, was measured slower)
     for (int s = 0; s < ns; s++) {
-        const int cj4 = entry(min(s + 4, ns - 1)) * APE + k4;
+        const int cj4 = entry(min(s + 4, ns - 1));
         const float4 x2 = A.xq[cj2];
         const int t2 = A.type_slot[cj2];
         float2 fjx, fjy, fjz;
         const bool found = pair_step<COUL, ENERGY, false, TWIN, PRUNE>(K, ljw + tj, nt1, I, fix, fiy, fiz, elj, ecoul, xj, 0xffu,
                                                                        0xffu, fjx, fjy, fjz, p3, A.rl2);
         red_add_v4(&A.f4[cj], -(fjx.x + fjx.y), -(fjy.x + fjy.y), -(fjz.x + fjz.y));
-        if (PRUNE) {
+        if (PRUNE) {   // the j atoms of the step that have a partner within rlist_inner keep their slot
             const unsigned gm = __ballot_sync(0xffffffffu, found);
-            unsigned hm = gm | (gm >> 1);
-            hm = (hm | (hm >> 2)) & 0x11111111u;   // bit 4h: half h of the step (lanes 4h..4h+3) has a survivor
-            if ((hm >> lane) & 1u) il_w[nu_w + __popc(hm & ((1u << lane) - 1u))] = (cj >> 2);   // slot/4 = 2*cj + half
-            nu_w += __popc(hm);
+            if (found) il_w[nu_w + __popc(gm & ((1u << lane) - 1u))] = cj;
+            nu_w += __popc(gm);
         }
         cj = cj_n; xj = xj1; tj = tj1;
         cj_n = cj2; xj1 = x2; tj1 = t2;
@@ -588,7 +584,7 @@ __global__ void __launch_bounds__(256) k_count_pairs(ForceArgs A, unsigned long 
 
 // Atom-pair slots of the inner list as the force kernel evaluates it: 32 per real (non-dummy) half-cluster
 // entry, 64 per masked cluster pair.  One thread per segment; statistics only.
-__global__ void k_count_slots(ForceArgs A, int nseg, int nhalf_real, unsigned long long* __restrict__ out)
+__global__ void k_count_slots(ForceArgs A, int nseg, int nslot_real, unsigned long long* __restrict__ out)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     unsigned long long n = 0;
@@ -596,7 +592,7 @@ __global__ void k_count_slots(ForceArgs A, int nseg, int nhalf_real, unsigned lo
         const int4 sd = A.segd[i];
         const int buf = nb_seg_buf(sd.w, A.bufmask, A.nparts, A.nunits);
         const int2 cnt = A.seg_cnt[buf][i];
-        for (int e = 0; e < cnt.x; e++) n += A.il[buf][sd.x + e] < nhalf_real ? 32u : 0u;
+        for (int e = 0; e < cnt.x; e++) n += A.il[buf][sd.x + e] < nslot_real ? 8u : 0u;   // 8 i atoms x one j atom
         n += 64ull * cnt.y;
     }
     for (int d = 16; d > 0; d >>= 1) n += __shfl_xor_sync(0xffffffffu, n, d);
@@ -810,7 +806,7 @@ int nbi_count_slots(nb_ctx* c, int64_t* slots)
     if (c->nseg_launch > 0) {
         ForceArgs A;
         fill_force_args(c, A);
-        k_count_slots<<<(c->nseg_launch + 127) / 128, 128, 0, st>>>(A, c->nseg_launch, 2 * c->nclusters_max,
+        k_count_slots<<<(c->nseg_launch + 127) / 128, 128, 0, st>>>(A, c->nseg_launch, 8 * c->nclusters_max,
                                                                    (unsigned long long*)c->counters.p);
         NB_LAUNCH_CHECK(c);
     }
@@ -851,8 +847,8 @@ int nbi_inner_dump(nb_ctx* c, int64_t* n, int32_t* ci, int32_t* entry, int32_t* 
         const int sci = sd.z & 0x3ffffff, sid = sd.z >> 26;
         const int prt = nb_part_of_unit(sd.w, std::max(c->last_nparts, 1), std::max(c->nunits, 1));
         for (int e = 0; e < cnt[b][s].x; e++) {
-            const int hc = il[b][sd.x + e];
-            if (hc >= 2 * c->nclusters_max) continue;   // dummy padding
+            const int hc = il[b][sd.x + e];             // slot of the listed j atom
+            if (hc >= 8 * c->nclusters_max) continue;   // dummy padding
             if (ci) ci[k] = sci;
             if (entry) entry[k] = hc;
             if (shift) shift[k] = sid;

@@ -177,10 +177,10 @@ struct nb_ctx {
     DevBuf<int32_t> seg_of_s0;                 // [nunits*8] s0 -> t
     DevBuf<int4> segd;                         // [nunits*8] by t: {il offset, ilm offset, i-cluster | shift id << 26, canonical unit}
     DevBuf<int2> ol_cnt;                       // [nunits*8] by t: OUTER {cluster pairs without a mask, with a mask}
-    DevBuf<int2> seg_cnt[2];                   // [nunits*8] by t: INNER {half-cluster entries (multiple of 8), masked cluster pairs}
+    DevBuf<int2> seg_cnt[2];                   // [nunits*8] by t: INNER {j-atom entries (multiple of 32), masked cluster pairs}
     DevBuf<int32_t> olu;                       // OUTER list, cluster pairs without a mask: cj, segment at il offset; written once per search
     DevBuf<int2> olm;                          // OUTER list, cluster pairs with a mask: {cj, mask ref}, segment at ilm offset
-    DevBuf<int32_t> il[2];                     // INNER list: surviving half j-clusters 2*cj + half (+ dummies up to a multiple of 8)
+    DevBuf<int32_t> il[2];                     // INNER list: slots of the surviving j atoms (+ dummies up to a multiple of 32)
     DevBuf<int2> ilm[2];                       // INNER list: surviving masked cluster pairs {cj, mask ref}
     // Two inner buffers: nb_prune_overlapped writes the part it prunes into the buffer the force kernel is
     // NOT reading and the part flips at the next nb_put_atoms.  Bit p of bufmask = buffer holding part p
@@ -276,21 +276,21 @@ __host__ __device__ inline void nb_shift_vec(int id, int& sx, int& sy, int& sz)
 int nb_fail(nb_ctx* c, int code, const char* fmt, ...);
 
 #ifdef __CUDACC__
-// The compact inner list is kept at HALF j-cluster granularity (4 atoms): an unmasked entry is the
-// half-cluster index hc = 2*cj + half, whose atoms are the slots 4*hc .. 4*hc+3.  The prune kernel
-// keeps a half iff one of its atoms is within rlist_inner of the i-cluster, which skips about a
-// tenth of the atom-pair slots a whole-cluster list evaluates (the cluster-pair "split" of the
-// paper's GPU lists).  Masked entries {cj, mask ref} stay whole clusters.
+// The compact inner list is kept at single-j-ATOM granularity (reading A22): an unmasked entry is the slot index of one
+// j atom, listed for the i-cluster iff it is within rlist_inner of one of the cluster's atoms.  Against whole j-clusters
+// that skips 35 % of the atom-pair slots on the water boxes (25 % against half j-clusters, the paper's 8x4 shape): the
+// lanes of the force kernel own one j atom each anyway, so the finer list costs nothing there; it is four times the
+// entries of a half-cluster list (4 B per listed j atom).  Cluster pairs that carry a mask stay whole: {cj, mask ref}.
 //
-// Closes a segment of nu unmasked half entries + nm masked entries (one warp): the unmasked count
-// is filled up to a multiple of 8 (one force-kernel step = 8 half-clusters) with dummy half-clusters.
+// Closes a segment of nu unmasked atom entries + nm masked cluster pairs (one warp): the unmasked count is filled up to
+// a multiple of 32 (one force-kernel step = 32 j atoms) with dummy atoms (far from everything, nb_grid.cu).
 __device__ __forceinline__ void nb_ilist_finish(int nu, int nm, int salt, int lane, int cj_dummy,
                                                 int32_t* __restrict__ il, int2* __restrict__ ilm, int2* __restrict__ cnt)
 {
-    const int rem = nu & 7;
+    const int rem = nu & 31;
     if (rem != 0) {
-        if (lane < 8 - rem) il[nu + lane] = 2 * cj_dummy + ((salt + lane) & (2 * NB_NDUMMY - 1));
-        nu += 8 - rem;
+        if (lane < 32 - rem) il[nu + lane] = 8 * cj_dummy + ((salt + lane) & (8 * NB_NDUMMY - 1));
+        nu += 32 - rem;
     }
     if (lane == 0) *cnt = make_int2(nu, nm);
 }

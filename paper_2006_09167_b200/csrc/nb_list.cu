@@ -500,7 +500,7 @@ __global__ void k_ilist_caps(const int4* __restrict__ units, int nseg_cap, const
             nm += __popc(eb);
         }
     }
-    capu[i] = (2 * nu + 7) & ~7;   // half-cluster entries, multiple of 8 (0 beyond the last segment: scanned as well)
+    capu[i] = (8 * nu + 31) & ~31;   // j-atom entries, multiple of 32 (0 beyond the last segment: scanned as well)
     capm[i] = nm;
     seg_len[i] = min(NB_SEG_MAXKEY - 1, ((2 * nu + 7) & ~7) + 2 * nm);
 }
@@ -580,7 +580,9 @@ __global__ void __launch_bounds__(256) k_ilist_build(BuildArgs A)
             if ((nb >> lane) & 1u) {
                 const int p = nu + __popc(nb & lt);
                 A.olu[o + p] = e.x;
-                *reinterpret_cast<int2*>(&A.il[o + 2 * p]) = make_int2(2 * e.x, 2 * e.x + 1);
+                int4* dst = reinterpret_cast<int4*>(&A.il[o + 8 * p]);   // all 8 atoms of the j-cluster
+                dst[0] = make_int4(8 * e.x, 8 * e.x + 1, 8 * e.x + 2, 8 * e.x + 3);
+                dst[1] = make_int4(8 * e.x + 4, 8 * e.x + 5, 8 * e.x + 6, 8 * e.x + 7);
             } else {
                 const int p = nm + __popc(eb & lt);
                 A.olm[om + p] = e;
@@ -592,7 +594,7 @@ __global__ void __launch_bounds__(256) k_ilist_build(BuildArgs A)
     }
     if (lane == 0) A.ol_cnt[t] = make_int2(nu, nm);
     __syncwarp();
-    nb_ilist_finish(2 * nu, nm, u.y * 8 + warp, lane, A.cj_dummy, A.il + o, A.ilm + om, &A.seg_cnt[t]);
+    nb_ilist_finish(8 * nu, nm, u.y * 8 + warp, lane, A.cj_dummy, A.il + o, A.ilm + om, &A.seg_cnt[t]);
 }
 
 // ---------------------------------------------------------------- introspection
@@ -634,7 +636,7 @@ __global__ void k_planes_from_il(int nseg, const int4* __restrict__ segd, const 
                                  const int32_t* __restrict__ il0, const int32_t* __restrict__ il1, const int2* __restrict__ ilm0,
                                  const int2* __restrict__ ilm1, const int4* __restrict__ units, const int* __restrict__ ent_count,
                                  const int* __restrict__ ent_jbegin, const int2* __restrict__ jl, unsigned bufmask, int nparts,
-                                 int nunits, int nhalf_real, uint32_t* __restrict__ plane_inner)
+                                 int nunits, int nslot_real, uint32_t* __restrict__ plane_inner)
 {
     const int t = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (t >= nseg) return;
@@ -649,9 +651,9 @@ __global__ void k_planes_from_il(int nseg, const int4* __restrict__ segd, const 
     for (int e = lane; e < cnt.x + cnt.y; e += 32) {
         int cj;
         if (e < cnt.x) {
-            const int hc = il[e];
-            if (hc >= nhalf_real) continue;   // dummy padding
-            cj = hc >> 1;
+            const int slot = il[e];
+            if (slot >= nslot_real) continue;   // dummy padding
+            cj = slot >> 3;
         } else {
             cj = ilm[e - cnt.x].x;
         }
@@ -1008,7 +1010,7 @@ int nbi_rebuild_inner_planes(nb_ctx* c)
         k_planes_from_il<<<(c->nseg_launch * 32 + 255) / 256, 256, 0, st>>>(
             c->nseg_launch, c->segd.p, c->seg_cnt[0].p, c->seg_cnt[1].p, c->il[0].p, c->il[1].p, c->ilm[0].p, c->ilm[1].p,
             c->units_canon.p, c->ent_count.p, c->ent_jbegin.p, c->jl.p, c->bufmask, c->buf_nparts, c->nunits,
-            2 * c->nclusters_max, c->plane_inner.p);
+            8 * c->nclusters_max, c->plane_inner.p);
         NB_LAUNCH_CHECK(c);
     }
     c->planes_dirty = false;

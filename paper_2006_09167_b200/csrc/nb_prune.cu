@@ -64,19 +64,16 @@ __device__ __forceinline__ bool prune_checks(const float2 (&xi)[4], const float2
     return found;
 }
 
-// One step over 4 cluster pairs WITHOUT a mask: a half j-cluster (4 atoms) survives iff one of its
-// atoms is within rlist_inner of an i atom; the survivors' half-cluster indices are appended to il.
+// One step over 4 cluster pairs WITHOUT a mask: a j atom survives iff it is within rlist_inner of an i atom; the
+// survivors' slot indices are appended to il in lane order (one ballot, one popc per lane).
 __device__ __forceinline__ void prune_step_unmasked(const float2 (&xi)[4], const float2 (&yi)[4], const float2 (&zi)[4],
                                                     const float rl2, const int cj, const float4 x, const bool valid,
                                                     const int lane, int32_t* __restrict__ il, int& nu)
 {
-    const bool found = prune_checks<false>(xi, yi, zi, x, rl2, false, 0);
-    const unsigned gm = __ballot_sync(0xffffffffu, found && valid);
-    unsigned hm = gm | (gm >> 1);
-    hm = (hm | (hm >> 2)) & 0x11111111u;          // bit 4h: half h of the step (lanes 4h..4h+3) has a survivor
-    if ((hm >> lane) & 1u)                        // its leader lane (lane % 4 == 0)
-        il[nu + __popc(hm & ((1u << lane) - 1u))] = 2 * cj + ((lane >> 2) & 1);
-    nu += __popc(hm);
+    const bool found = prune_checks<false>(xi, yi, zi, x, rl2, false, 0) && valid;
+    const unsigned gm = __ballot_sync(0xffffffffu, found);
+    if (found) il[nu + __popc(gm & ((1u << lane) - 1u))] = cj * 8 + (lane & 7);
+    nu += __popc(gm);
 }
 
 // One step over 4 cluster pairs WITH a mask (exclusions, or the zero-shift diagonal pair, which keeps

@@ -45,9 +45,12 @@ def efficiency_table(nside: int, rcs, buffers, device: int = 0):
             pruned = ctx.list_count(1)
             n_int2, n_exc2 = ctx.count_pairs()
             assert (n_int2, n_exc2) == (n_int, n_exc), "pruning at rlist >= rc must not lose a pair within rc"
+            slots = ctx.count_slots()
             rows.append({"rc": rc, "buffer": b, "pairs_within_rc": n_int + n_exc,
                          "cluster_pairs_searched": searched, "cluster_pairs_pruned": pruned,
+                         "slots_streamed": slots,
                          "eff_searched": (n_int + n_exc) / (64.0 * searched), "eff_pruned": (n_int + n_exc) / (64.0 * pruned),
+                         "eff_streamed": (n_int + n_exc) / float(slots),
                          "eff_1x1_ideal": (rc / rl) ** 3})
             ctx.close()
     return {"workload": w.name, "natoms": w.natoms, "cluster": "8x8", "rows": rows}
@@ -61,9 +64,9 @@ def main():
     a = ap.parse_args()
     tab = efficiency_table(a.nside, a.rc, a.buffers)
     print(json.dumps({k: v for k, v in tab.items() if k != "rows"}))
-    print("rc      buffer  eff(8x8 searched)  eff(8x8 pruned)  eff(1x1 ideal)")
+    print("rc      buffer  eff(8x8 searched)  eff(8x8 pruned)  eff(8x1 streamed)  eff(1x1 ideal)")
     for r in tab["rows"]:
-        print(f"{r['rc']:<7g} {r['buffer']:<7g} {r['eff_searched']:<18.4f} {r['eff_pruned']:<16.4f} {r['eff_1x1_ideal']:.4f}")
+        print(f"{r['rc']:<7g} {r['buffer']:<7g} {r['eff_searched']:<18.4f} {r['eff_pruned']:<16.4f} {r['eff_streamed']:<18.4f} {r['eff_1x1_ideal']:.4f}")
 
 
 if __name__ == "__main__":

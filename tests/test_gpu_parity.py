@@ -91,7 +91,8 @@ def spread_ranges(ncl, nranges, width):
 
 
 def check_half_list(d, w, c_ranges=None, part=None, before=None):
-    """The compact inner list the force kernel streams (nb_inner_dump) against oracle_half_lists on the
+    """The compact inner list the force kernel streams (nb_inner_dump: single j atoms of the cluster pairs without a
+    mask, whole cluster pairs with one) against oracle_atom_lists on the
     library's slot table at the CURRENT coordinates, bit-exact as sets (no guard band: both sides decide
     in fp32 with the A12 operation order); no duplicates, no dummy entries.
     c_ranges: compare only entries whose first or second cluster lies in one of the ranges (sampled check);
@@ -102,7 +103,7 @@ def check_half_list(d, w, c_ranges=None, part=None, before=None):
     ci, ent, s, kind, prt = d.inner_dump()
     keys = LC.half_entry_keys(ci, ent, s, kind)
     assert np.unique(keys).size == keys.size, "duplicate entry in the compact inner list"
-    cj = np.where(kind == 0, ent // 2, ent)
+    cj = np.where(kind == 0, ent // 8, ent)
     assert ent.size == 0 or (cj.max() < ncl and cj.min() >= 0 and ci.max() < ncl), "dummy or out-of-range entry leaked"
     if part is not None:
         # the oracle's entries of that part: the part of an entry is the part of its outer triple in the library's list
@@ -111,11 +112,11 @@ def check_half_list(d, w, c_ranges=None, part=None, before=None):
         order = np.argsort(okeys)
         okeys, opart = okeys[order], opart[order]
     for (c0, c1) in (c_ranges if c_ranges is not None else [(0, ncl)]):
-        ref = O.half_lists(aos, xq, w.box, w.rlist_outer, w.rlist_inner, w.excl_off, w.excl_idx, c_begin=c0, c_end=c1)
+        ref = O.atom_lists(aos, xq, w.box, w.rlist_outer, w.rlist_inner, w.excl_off, w.excl_idx, c_begin=c0, c_end=c1)
         rkeys = ref.keys()
         sel = ((ci >= c0) & (ci < c1)) | ((cj >= c0) & (cj < c1))
         if part is not None:
-            rcj = np.where(ref.kind == 0, ref.entry // 2, ref.entry)
+            rcj = np.where(ref.kind == 0, ref.entry // 8, ref.entry)
             tk = LC.triple_keys(ref.ci, rcj, ref.s)
             pos = np.searchsorted(okeys, tk)
             assert (pos < okeys.size).all() and np.array_equal(okeys[pos], tk), "oracle inner entry outside the library's outer list"
@@ -126,7 +127,7 @@ def check_half_list(d, w, c_ranges=None, part=None, before=None):
     if part is not None and before is not None:
         # label the earlier entries with TODAY's parts (through their outer triple) and compare the other parts
         bci, bent, bsid, bkind = before >> 38, (before >> 9) & ((1 << 29) - 1), (before >> 1) & 0xFF, before & 1
-        btk = (bci << 36) | (np.where(bkind == 0, bent // 2, bent) << 8) | bsid
+        btk = (bci << 36) | (np.where(bkind == 0, bent // 8, bent) << 8) | bsid
         bpart = opart[np.searchsorted(okeys, btk)]
         assert np.array_equal(np.sort(before[bpart != part]), np.sort(keys[prt != part])), "a prune changed another part"
     return keys
@@ -168,7 +169,7 @@ def test_config0_layout_lists_forces(cfg0):
     assert st["n_pairs_inner"] == ref_l.inner.sum() and st["n_pairs_outer"] == ref_l.inner.size
     assert st["slots_last_forces"] == d.ctx.count_slots() < 64 * st["n_pairs_inner"]
     hci, hent, _, hkind, _ = d.inner_dump()
-    assert st["slots_last_forces"] == 32 * int((hkind == 0).sum()) + 64 * int((hkind == 1).sum())
+    assert st["slots_last_forces"] == 8 * int((hkind == 0).sum()) + 64 * int((hkind == 1).sum())   # 8 i atoms x 1 j atom; whole masked pairs
     check_half_list(d, w)
     # mean number of set interaction-mask bits per joint entry: the paper's "approximately four of eight" (L135)
     assert 2.5 < st["n_pairs_outer"] / st["n_joint_outer"] < 6.5
@@ -465,8 +466,8 @@ def test_full_size_configs_in_bench_schedule(which):
 
 @pytest.mark.parametrize("which", ["cfg0", "rect_rf", "lj"])
 def test_half_cluster_inner_list(which):
-    """The compact inner list the force kernel streams is kept at half-j-cluster granularity (DESIGN.md
-    section 5).  Bit-exact against oracle_half_lists after a full prune and after rolling parts on moved
+    """The compact inner list the force kernel streams is kept at single-j-atom granularity (DESIGN.md
+    section 5, reading A22).  Bit-exact against oracle_atom_lists after a full prune and after rolling parts on moved
     coordinates; layout-independent fp64 check (k-d tree) that it is COMPLETE; the cluster pairs it spans
     are exactly the inner list of nb_list_dump (which is derived from it)."""
     w = {"cfg0": W.config0, "lj": lambda: W.lj_fluid(12, rc=0.9),
@@ -493,7 +494,7 @@ def test_half_cluster_inner_list(which):
     ka, kb = LC.shift_id(sp), LC.shift_id(-sp)
     missing = 0
     for a, b, k1, k2 in zip(si.tolist(), sj.tolist(), ka.tolist(), kb.tolist()):
-        if ((a // 8, b // 4, k1) in hkeys or (b // 8, a // 4, k2) in hkeys or (a // 8, b // 8, k1) in mkeys
+        if ((a // 8, b, k1) in hkeys or (b // 8, a, k2) in hkeys or (a // 8, b // 8, k1) in mkeys
                 or (b // 8, a // 8, k2) in mkeys):
             continue
         missing += 1
@@ -501,7 +502,7 @@ def test_half_cluster_inner_list(which):
     # same cluster pairs as the bit-plane inner list
     dci, dcj, dsv, _, _ = d.dump(1)
     planes = set(zip(dci.tolist(), dcj.tolist(), LC.shift_id(dsv).tolist()))
-    spanned = {(a, e // 2, k) for a, e, k in hkeys} | mkeys
+    spanned = {(a, e // 8, k) for a, e, k in hkeys} | mkeys
     assert spanned == planes
 
 
@@ -724,7 +725,7 @@ def test_work_efficiency_table_against_oracle():
         for r in rows:
             assert abs(r["pairs_within_rc"] - (ref.npairs + ref.npairs_excl)) <= 2
             assert r["cluster_pairs_pruned"] <= r["cluster_pairs_searched"]
-            assert r["eff_searched"] <= r["eff_pruned"] < r["eff_1x1_ideal"] <= 1.0
+            assert r["eff_searched"] <= r["eff_pruned"] < r["eff_streamed"] < r["eff_1x1_ideal"] <= 1.0   # finer list, fewer slots
         effs = [r["eff_searched"] for r in rows]
         assert effs[0] > effs[1] > effs[2]
 
