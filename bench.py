@@ -595,11 +595,11 @@ def run_b200(args):
     if rank == 0:
         st = st1
         # prune kernel (a6): one rolling part per inner step; arithmetic = 64 distance checks per outer cluster pair
-        n_outer, n_half = st["n_pairs_outer"], slots_step / 32.0
+        n_outer, n_listed = st["n_pairs_outer"], slots_step / 8.0   # listed j atoms ~ slots / 8
         p_us = per_stage_us["prune"]
         prune_launch_pairs = n_outer * (S + (pop["inner"][1]) / w.nparts) / max(S + pop["inner"][1], 1)   # mean over full + rolling launches
         prune_flop = prune_launch_pairs * 64 * PRUNE_FLOP_PER_CHECK
-        prune_bytes = prune_launch_pairs * 4 + st["nslots"] * 16 + (prune_launch_pairs / max(n_outer, 1)) * n_half * 4
+        prune_bytes = prune_launch_pairs * 4 + st["nslots"] * 16 + (prune_launch_pairs / max(n_outer, 1)) * n_listed * 4
         ptraffic, ptraffic_src = ncu_traffic("prune", args.config, w.coulomb) if workload_is_config else (None, "not a BASELINE config")
         roofline_prune = None
         if p_us:
@@ -611,7 +611,7 @@ def run_b200(args):
                               "hbm": {"achieved": prune_bytes / (p_us * 1e-6) / 1e9, "peak": hbm_gbs, "unit": "GB/s",
                                       "frac": prune_bytes / (p_us * 1e-6) / 1e9 / hbm_gbs, "peak_source": hbm_src,
                                       "algorithmic_bytes_per_launch": prune_bytes,
-                                      "bytes_are": "4 B per outer cluster pair read + xq once (16 B/slot) + 4 B per surviving half entry written",
+                                      "bytes_are": "4 B per outer cluster pair read + xq once (16 B/slot) + 4 B per surviving j-atom entry written",
                                       "traffic": ptraffic, "traffic_source": ptraffic_src}}
         # gridding (a2): HBM-side algorithmic bytes, and what the launch count alone costs
         g_us = per_stage_us["grid"]

@@ -9,7 +9,7 @@
 // Thread mapping (differs from the paper's 8x4-per-warp tiles): one thread
 // block = one warp = one i-cluster working through one segment of the compact inner list that the
 // prune kernel wrote for it.  The 8 i atoms sit in registers of every lane as 4 packed pairs.
-// Lanes own j atoms: an unmasked step takes the next 8 half j-clusters (4 atoms each, 32 j atoms),
+// Lanes own j atoms: an unmasked step takes the next 32 listed j atoms (the inner list is kept per j atom),
 // a masked step 4 whole j-clusters with their exclusion masks; every lane evaluates its j atom
 // against the 8 i atoms, two at a time with packed FP32x2 instructions.  Consequences: no shuffle
 // in the inner loop (the j force is private to its lane and leaves with ONE vector atomic per j
@@ -203,7 +203,7 @@ __device__ __forceinline__ bool pair_step(const NbConst& K, const float4* __rest
     return found;
 }
 
-// PRUNE = false: the inner list (half j-clusters, 8 per step; masked cluster pairs, 4 per step).
+// PRUNE = false: the inner list (listed j atoms, 32 per step; masked cluster pairs, 4 per step).
 // PRUNE = true: the fused first prune of a freshly searched list: the same kernel walks
 // the OUTER list (whole j-clusters, 4 per step), evaluates the forces, and writes the inner list from
 // the r^2 values it has anyway -- one ballot per step, as in nb_prune.cu's kernel.
@@ -220,7 +220,7 @@ __global__ void __launch_bounds__(32, PRUNE ? 8 : 16) k_force(ForceArgs A)
     const int4 sd = A.segd[blockIdx.x];
     // (the part comes from a table written when nparts changes: deriving it from the unit index costs a 64-bit division)
     const int buf = PRUNE || !A.bufmask ? 0 : (int)((A.bufmask >> A.seg_part[blockIdx.x]) & 1u);
-    // PRUNE: outer counts {cluster pairs without a mask, with a mask}; else inner {half entries, masked pairs}
+    // PRUNE: outer counts {cluster pairs without a mask, with a mask}; else inner {j-atom entries, masked pairs}
     const int2 cnt = PRUNE ? A.ol_cnt[blockIdx.x] : A.seg_cnt[buf][blockIdx.x];
     const int ci = sd.z & 0x3ffffff, sid = sd.z >> 26, warp = ci & 7;
     const int nt1 = K.ntypes1;
@@ -298,7 +298,7 @@ __global__ void __launch_bounds__(32, PRUNE ? 8 : 16) k_force(ForceArgs A)
         }
     }
 
-    // Cluster pairs without a mask: always full steps of 8 half-clusters (PRUNE: 4 clusters, the last step
+    // Cluster pairs without a mask: always full steps of 32 listed j atoms (PRUNE: 4 clusters, the last step
     // possibly partly filled).  ptxas schedules memory operations whose consumer is an iteration away at the
     // END of a step, so the j data is requested TWO steps ahead into registers (xj: this step, xj1: next
     // step, x2: the one after) and the list entries four steps ahead, indices clamped to the segment.
@@ -582,7 +582,7 @@ __global__ void __launch_bounds__(256) k_count_pairs(ForceArgs A, unsigned long 
     }
 }
 
-// Atom-pair slots of the inner list as the force kernel evaluates it: 32 per real (non-dummy) half-cluster
+// Atom-pair slots of the inner list as the force kernel evaluates it: 8 per real (non-dummy) j-atom
 // entry, 64 per masked cluster pair.  One thread per segment; statistics only.
 __global__ void k_count_slots(ForceArgs A, int nseg, int nslot_real, unsigned long long* __restrict__ out)
 {

@@ -438,7 +438,7 @@ int nbi_grid(nb_ctx* c)
         // (rewritten only when the box or their place in the arrays has changed)
         // Dummy j-clusters (index nclusters_max .. nclusters_max + NB_NDUMMY - 1): padding-like atoms beyond the
         // padding lattice that interact with nothing.  The prune kernel may fill an inner list
-        // segment up to a multiple of 8 half-clusters with them; the (zero) forces the force kernel adds to their
+        // segment up to a multiple of 32 atoms with them; the (zero) forces the force kernel adds to their
         // slots are never read, and spreading them over NB_NDUMMY clusters avoids atomic hot spots.
         std::vector<float4> hx((size_t)NB_C * NB_NDUMMY);
         std::vector<int32_t> ht((size_t)NB_C * NB_NDUMMY, c->ntypes);

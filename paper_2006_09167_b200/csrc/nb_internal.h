@@ -36,7 +36,7 @@ struct NbTotals {
     int pad[6];
 };
 enum { NB_OVF_COL = 1, NB_OVF_JOINT = 2, NB_OVF_UNITS = 4, NB_OVF_MASKS = 8, NB_OVF_IL = 16, NB_OVF_ILM = 32 };
-#define NB_SEG_MAXKEY 2080              // segment length key (half entries + 2 x masked) is below this
+#define NB_SEG_MAXKEY 2080              // segment length key (see k_ilist_caps) is below this
 #define NB_MAX_SORT_PARTS 16            // rolling parts whose prune order is sorted longest first (more: canonical order)
 
 // One growable device array.

@@ -482,7 +482,7 @@ __global__ void k_excl_planes(const int2* __restrict__ jl, const unsigned long l
 
 // ---------------------------------------------------------------- compact lists (nb_internal.h)
 // Segment capacities per (work unit, i-cluster): every outer cluster pair can survive a prune.
-// seg_len is the sort key of the launch orders (half entries + 2 x masked pairs ~ force kernel work).
+// seg_len is the sort key of the launch orders (twice the unmasked cluster pairs, rounded up to 8, + 2 x masked pairs ~ force kernel work).
 __global__ void k_ilist_caps(const int4* __restrict__ units, int nseg_cap, const uint32_t* __restrict__ plane_outer,
                              const uint32_t* __restrict__ plane_excl, NbTotals* __restrict__ tot, Caps caps,
                              int* __restrict__ capu, int* __restrict__ capm, int* __restrict__ seg_len)
@@ -630,7 +630,7 @@ __global__ void k_count_nonempty(const int* __restrict__ ent_count, int nent, lo
 }
 
 // plane_inner (the inner list at cluster-pair granularity, which only the dumps and the pair counting
-// read) from the compact inner list the force kernel streams: one warp per segment; a listed half or
+// read) from the compact inner list the force kernel streams: one warp per segment; a listed j atom or
 // masked cluster pair sets the bit of its joint entry, found by bisection in the unit's slice of jl.
 __global__ void k_planes_from_il(int nseg, const int4* __restrict__ segd, const int2* __restrict__ cnt0, const int2* __restrict__ cnt1,
                                  const int32_t* __restrict__ il0, const int32_t* __restrict__ il1, const int2* __restrict__ ilm0,

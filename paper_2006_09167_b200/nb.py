@@ -217,7 +217,7 @@ class Context:
 
     def inner_dump(self):
         """The compact inner list the force kernel streams: numpy arrays ci, entry, shift id, kind
-        (0: entry = half j-cluster index 2*cj + half; 1: entry = whole j-cluster with a mask), part."""
+        (0: entry = slot of a listed j atom; 1: entry = whole j-cluster with a mask), part."""
         n = C.c_int64()
         null = C.c_void_p(0)
         self._check(lib().nb_inner_dump(self._h, C.byref(n), null, null, null, null, null))
