@@ -462,6 +462,17 @@ def test_full_size_configs_in_bench_schedule(which):
             torch.cuda.synchronize()
             assert rel_rms(ft.cpu().numpy().astype(np.float64), oracle_forces(w, x=x, method="cells").f) <= TOL_F
     check_half_list(d, w, c_ranges=sample, part=(t1 - 1) % k)
+    # ... and the other order bench.py --prune auto may pick: the rolling prune on the second stream next to the force
+    # kernel (nb_prune_overlapped; the part pruned on step t's coordinates is first used at step t + 1)
+    for t in range(t1, t1 + 2 * k + 1):
+        x = w.positions_at(t)
+        d.put(x)                                          # joins the prune of step t - 1: its part flips here
+        d.ctx.prune_overlapped(w.rlist_inner, t % k, k)
+        f = d.forces()
+    assert rel_rms(f, oracle_forces(w, x=x, method="cells").f) <= TOL_F   # (every part has been through the second buffer by now)
+    d.put(x)                                              # same coordinates again: the last prune is joined, nothing moved
+    if which != "cfg3":
+        check_half_list(d, w, c_ranges=sample, part=(t1 + 2 * k) % k)
 
 
 @pytest.mark.parametrize("which", ["cfg0", "rect_rf", "lj"])
