@@ -167,10 +167,15 @@ class ClockSampler(threading.Thread):
                         self.reasons.add(name)
             except Exception:
                 pass
-            time.sleep(0.02)
+            time.sleep(0.002)
 
     def result(self):
         self.stop_flag = True
+        if self.nv is not None and not self.samples:   # (a region shorter than the thread's start-up: one reading now)
+            try:
+                self.samples.append(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM))
+            except Exception:
+                pass
         if self.nv is None or not self.samples:
             return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": []}
         s = sorted(self.samples)
@@ -514,7 +519,6 @@ def run_b200(args):
     sampler.start()
     pop = rep.timed(step_value, positions)
     barrier()
-    clocks = sampler.result()
     st1 = ctx.get_stats()
     launches = st1["kernel_launches"] - launches0 - 3   # get_stats itself launches three counting kernels
     # second pass: the same steps with an event pair around the force kernel only
@@ -532,6 +536,7 @@ def run_b200(args):
     rep.timed(rep.step_device, positions)
     rep.overlapped = was_overlapped
     stages_other = ctx.timing_read(reset=True)
+    clocks = sampler.result()   # sampled every 2 ms over the three timed passes (the value pass alone lasts a few ms at --steps 20)
     stages = {k: (stages[k] if k in ("force", "force_energy") else stages_other[k]) for k in stages}
     ctx.timing_stages(0xFFFFFFFF)
     ctx.timing_enable(False)
