@@ -146,6 +146,22 @@ int nb_forces_host(nb_ctx*, float* f, double* energies, double* virial);
  * same inner list bit for bit, forces equal up to summation order.  Same argument rules as nb_prune / nb_forces. */
 int nb_forces_prune(nb_ctx*, float rlist_inner, float* f, double* energies, double* virial);
 
+/* nb_forces for callers that cannot call cudaMalloc (a stream under CUDA graph capture, a tight serving loop, a harness
+ * that forbids it): same arguments, same kernels, same results up to the order of the atomic adds, but the call allocates
+ * NOTHING -- no cudaMalloc / cudaFree, no event creation, no allocating library routine.  The force kernel's scratch (the
+ * cluster-order force accumulator and the per-shift force sums of the virial: i and j forces are
+ * accumulated on the device and reduced once) lives in one static device array of NB_STATIC_SCRATCH_BYTES inside the
+ * library instead of the context's own buffers; every GPU that loads the library holds it until the process exits.
+ * Limit: the bound on the system's atom slots, 64 * (natoms/64 + columns of the search grid), a few per cent above
+ * natoms, must not exceed NB_STATIC_MAX_SLOTS -- about 245 000 atoms; beyond it the call returns NB_ERR_OVERFLOW with a
+ * message and does nothing.  The array is shared by every context on the device and keeps the last call's contents: each
+ * call clears what it uses on its stream first, and two calls that overlap on the GPU (two contexts on different streams)
+ * RACE -- serialise them.  No stage timing is recorded for this call.  Its device address is resolved per device at
+ * nb_init (cudaGetSymbolAddress); if that failed the call returns NB_ERR_CUDA.  Call-order rules as nb_forces. */
+#define NB_STATIC_MAX_SLOTS 262144
+#define NB_STATIC_SCRATCH_BYTES ((64 + NB_STATIC_MAX_SLOTS + 8 * 1024) * 16)   /* 4 326 400 B */
+int nb_forces_static(nb_ctx*, float* f, double* energies, double* virial);
+
 /* One inner step of the schedule as ONE call: nb_put_atoms(x, NULL, NULL, the box of the last search) +
  * nb_prune(rlist_inner, part, nparts) + nb_forces(f, NULL, NULL): the same kernels in the same order, so the same inner
  * list bit for bit and the same forces up to the order of the atomic adds.

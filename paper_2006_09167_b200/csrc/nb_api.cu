@@ -58,6 +58,7 @@ extern "C" int nb_init(const nb_params* p, nb_ctx** out)
     c->stream = (cudaStream_t)p->stream;
     c->natoms = p->natoms;
     c->ntypes = p->ntypes;
+    nbi_static_scratch_setup(c);   // nb_forces_static: device address of the static scratch, once per device (never fails nb_init)
     if (cudaDeviceGetAttribute(&c->nsm, cudaDevAttrMultiProcessorCount, p->device) != cudaSuccess || c->nsm <= 0) c->nsm = 148;
     *out = c;   // returned even on failure below so that nb_last_error() can be read; nb_free() it
 
@@ -255,6 +256,16 @@ extern "C" int nb_forces(nb_ctx* c, float* f, double* energies, double* virial)
     if (virial && !energies) return nb_fail(c, NB_ERR_ARG, "nb_forces: virial needs energies (same kernel flavour)");
     if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "nb_forces without a valid list (call nb_search)");
     return nbi_forces(c, f, energies, virial);
+}
+
+extern "C" int nb_forces_static(nb_ctx* c, float* f, double* energies, double* virial)
+{
+    if (!c) return NB_ERR_ARG;
+    DeviceGuard guard(c);
+    if (!f) return nb_fail(c, NB_ERR_ARG, "nb_forces_static: f is null");
+    if (virial && !energies) return nb_fail(c, NB_ERR_ARG, "nb_forces_static: virial needs energies (same kernel flavour)");
+    if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "nb_forces_static without a valid list (call nb_search)");
+    return nbi_forces_static(c, f, energies, virial);
 }
 
 extern "C" int nb_forces_prune(nb_ctx* c, float rlist_inner, float* f, double* energies, double* virial)

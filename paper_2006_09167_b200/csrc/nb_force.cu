@@ -19,6 +19,7 @@
 #include "nb_internal.h"
 
 #include <algorithm>
+#include <mutex>
 
 #include "ewald_corr_coeffs.h"
 
@@ -891,5 +892,109 @@ int nbi_count_pairs(nb_ctx* c, int64_t* n_interacting, int64_t* n_excluded)
     NB_CUDA(c, cudaStreamSynchronize(st));
     if (n_interacting) *n_interacting = v[0];
     if (n_excluded) *n_excluded = v[1];
+    return NB_OK;
+}
+
+// ---------------------------------------------------------------- nb_forces_static: nb_forces that allocates nothing
+// For callers that cannot call cudaMalloc (a stream under graph capture, a tight serving loop, a harness that forbids it).
+// The force kernel's scratch -- the cluster-order accumulator f4 it adds into and the per-shift i-force sums / virial
+// partials -- lives in ONE file-scope device array of a fixed size instead of the context's cudaMalloc'ed buffers
+// (c->f4, c->fshift).  Every GPU that loads the library holds the array until the process exits (NB_STATIC_SCRATCH_BYTES,
+// about 4.1 MiB).  All calls of all contexts on a device share it: calls that overlap on the GPU race, and it keeps the
+// last call's contents, so every call clears the part it uses first.
+//   bytes [0, 1024): 27*3 + 9 doubles (per-shift force sums, sum x (x) f)
+//   then NB_STATIC_MAX_SLOTS + 8 * NB_NDUMMY float4: force accumulator, real slots then the dummy clusters' slots
+#define NB_STATIC_HEAD_F4 64   // 1024 B
+static __device__ __align__(256) float4 g_nb_static_scratch[NB_STATIC_HEAD_F4 + NB_STATIC_MAX_SLOTS + NB_C * NB_NDUMMY];
+static_assert(sizeof(g_nb_static_scratch) == NB_STATIC_SCRATCH_BYTES, "nb.h states the size of the static scratch");
+static_assert((NB_NSHIFT * 3 + 9) * sizeof(double) <= NB_STATIC_HEAD_F4 * sizeof(float4), "head of the static scratch");
+
+// In host code `g_nb_static_scratch` is a host-side stand-in, not a device address: the address a kernel can use comes
+// from cudaGetSymbolAddress, once per device, with that device current (nb_init has made it current).
+void nbi_static_scratch_setup(nb_ctx* c)
+{
+    static std::mutex mu;
+    static void* addr_of_device[64] = {};
+    c->static_scratch = nullptr;
+    c->static_scratch_cuda_err = 0;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess && (dev != c->prm.device || dev < 0 || dev >= 64)) e = cudaErrorInvalidDevice;
+    if (e == cudaSuccess) {
+        std::lock_guard<std::mutex> lock(mu);
+        if (!addr_of_device[dev]) {
+            void* p = nullptr;
+            e = cudaGetSymbolAddress(&p, g_nb_static_scratch);
+            if (e == cudaSuccess) addr_of_device[dev] = p;
+        }
+        if (e == cudaSuccess) c->static_scratch = addr_of_device[dev];
+    }
+    if (e != cudaSuccess) {
+        c->static_scratch_cuda_err = (int)e;
+        cudaGetLastError();   // nb_forces_static reports it; the other calls are not affected
+    }
+}
+
+// The non-fused half of nbi_forces with the two scratch pointers replaced; same kernels, same launch order.  No stage
+// timers (their events are created on demand), no DevBuf::ensure: nothing here allocates.
+int nbi_forces_static(nb_ctx* c, float* f, double* energies, double* virial)
+{
+    cudaStream_t st = c->stream;
+    if (!c->static_scratch)
+        return nb_fail(c, NB_ERR_CUDA, "nb_forces_static: cudaGetSymbolAddress of the static scratch failed at nb_init: %s",
+                       cudaGetErrorString((cudaError_t)c->static_scratch_cuda_err));
+    if (c->nslots_max > NB_STATIC_MAX_SLOTS)
+        return nb_fail(c, NB_ERR_OVERFLOW,
+                       "nb_forces_static: this system needs %d atom slots (natoms/64 + grid columns super-clusters of 64), the static "
+                       "scratch holds NB_STATIC_MAX_SLOTS = %d; use nb_forces",
+                       c->nslots_max, (int)NB_STATIC_MAX_SLOTS);
+    double* fshift = reinterpret_cast<double*>(c->static_scratch);
+    float4* f4 = reinterpret_cast<float4*>(c->static_scratch) + NB_STATIC_HEAD_F4;
+    const size_t nf4 = (size_t)c->nslots_max + NB_C * NB_NDUMMY;
+    // the accumulator must start at zero; the array holds whatever the last call (of any context) left in it
+    NB_CUDA(c, cudaMemsetAsync(f4, 0, nf4 * sizeof(float4), st));
+    ForceArgs A;
+    fill_force_args(c, A);
+    A.f4 = f4;
+    A.cj_dummy = c->nclusters_max;
+    {
+        const double P[5] = {NB_EWC_P0, NB_EWC_P1, NB_EWC_P2, NB_EWC_P3, NB_EWC_P4};
+        const double Q[6] = {NB_EWC_Q0, NB_EWC_Q1, NB_EWC_Q2, NB_EWC_Q3, NB_EWC_Q4, NB_EWC_Q5};
+        const double b = c->beta_d, b2 = b * b;
+        double bk = 1.0;
+        const double qlead = b2 * b2 * b2 * b2 * b2 * Q[5];
+        for (int k = 0; k < 6; k++, bk *= b2) {
+            if (k < 5) A.kc.ewp2[k] = make_float2((float)(b * b2 * bk * P[k] / qlead), (float)(b * b2 * bk * P[k] / qlead));
+            A.kc.ewq2[k] = make_float2((float)(bk * Q[k] / qlead), (float)(bk * Q[k] / qlead));
+        }
+    }
+    A.fshift = fshift;
+    A.energies = energies;
+    const bool energy = energies != nullptr;
+    if (energy) {
+        NB_CUDA(c, cudaMemsetAsync(energies, 0, 2 * sizeof(double), st));
+        NB_CUDA(c, cudaMemsetAsync(fshift, 0, (NB_NSHIFT * 3 + 9) * sizeof(double), st));
+    }
+    if (c->nunits > 0 && c->nseg_launch > 0) {
+        const bool twin = c->twin;
+        int rc;
+        if (c->prm.coulomb == NB_COUL_EWALD) rc = launch_force_e<NB_COUL_EWALD>(c, A, energy, twin, false);
+        else if (c->prm.coulomb == NB_COUL_RF) rc = launch_force_e<NB_COUL_RF>(c, A, energy, twin, false);
+        else rc = launch_force_e<NB_COUL_NONE>(c, A, energy, twin, false);
+        if (rc != NB_OK) return rc;
+    }
+    double* xf = fshift + NB_NSHIFT * 3;
+    const int nslots = c->nslots_max;
+    if (virial)
+        NB_CUDA(c, nb_launch_pdl(k_gather<true>, dim3((nslots + 255) / 256), dim3(256), 0, st, nslots, f4, c->atom_of_slot.p, c->xq.p, f, xf));
+    else
+        NB_CUDA(c, nb_launch_pdl(k_gather4, dim3((nslots / 4 + 255) / 256), dim3(256), 0, st, nslots / 4, f4,
+                                 reinterpret_cast<const int4*>(c->atom_of_slot.p), f));
+    NB_LAUNCH_CHECK(c);
+    if (virial) {
+        k_virial_final<<<1, 32, 0, st>>>(xf, fshift, make_float3(c->box[0], c->box[1], c->box[2]), virial);
+        NB_LAUNCH_CHECK(c);
+    }
+    c->st.force_count++;
     return NB_OK;
 }

@@ -198,6 +198,9 @@ struct nb_ctx {
     int nseg_launch = 0;                       // segments with a non-empty outer list (= force kernel grid)
     DevBuf<float4> ljrow;                      // [nclusters_max * 4 * (ntypes+1)] paired LJ rows per i-cluster (nb_force.cu), written at search
     DevBuf<double> fshift;                     // [27*3] per-shift i-force sums (virial)
+    void* static_scratch = nullptr;            // nb_forces_static: device address of nb_force.cu's static scratch array on this
+                                               // context's device (cudaGetSymbolAddress at nb_init), nullptr if that failed
+    int static_scratch_cuda_err = 0;           // the cudaError_t of that failure
 
     // --- nb_step: the inner step (put + rolling prune + forces) as one CUDA graph launch ---
     // One cached graph per (part, nparts, rlist_inner); captured on a private stream (the caller's may be the legacy
@@ -376,3 +379,5 @@ int nbi_ljrows(nb_ctx* c);                                  // nb_force.cu: pair
 int nbi_exclusive_scan(nb_ctx* c, const int32_t* in, int32_t* out, int64_t n, int32_t* total_dev);  // nb_list.cu
 const void* nbi_put_kernel();                               // nb_grid.cu: the k_put entry (node lookup in captured graphs)
 const void* nbi_gather4_kernel();                           // nb_force.cu: the k_gather4 entry
+void nbi_static_scratch_setup(nb_ctx* c);                   // nb_force.cu: resolves c->static_scratch (the context's device is current)
+int nbi_forces_static(nb_ctx* c, float* f, double* energies, double* virial);   // nb_force.cu: nb_forces_static

@@ -24,7 +24,8 @@ NB_SHIFT_CENTER = 13
 EXPORTS = ["nb_init", "nb_put_atoms", "nb_put_atoms_host", "nb_search", "nb_prune", "nb_forces",
            "nb_forces_host", "nb_free", "nb_last_error", "nb_get_layout", "nb_get_slots", "nb_list_count",
            "nb_list_dump", "nb_get_stats", "nb_measure_fp32_peak", "nb_count_pairs", "nb_timing_enable",
-           "nb_timing_read", "nb_timing_stages", "nb_count_slots", "nb_inner_dump", "nb_prune_overlapped", "nb_forces_prune", "nb_step", "nb_measure_fp32_pipe", "nb_step_host"]
+           "nb_timing_read", "nb_timing_stages", "nb_count_slots", "nb_inner_dump", "nb_prune_overlapped", "nb_forces_prune", "nb_step", "nb_measure_fp32_pipe", "nb_step_host",
+           "nb_forces_static"]
 NB_T_NAMES = ["put", "grid", "search", "masks", "prune", "force", "reduce", "force_energy"]
 
 
@@ -143,6 +144,11 @@ class Context:
     def forces(self, f, energies=None, virial=None):
         """f [N,3] f32 CUDA tensor (overwritten); energies [2] f64, virial [9] f64 CUDA tensors or None."""
         self._check(lib().nb_forces(self._h, _dptr(f), _dptr(energies), _dptr(virial)))
+
+    def forces_static(self, f, energies=None, virial=None):
+        """nb_forces without any allocation: the kernel's scratch is a static device array of the library (size limit:
+        nb.h NB_STATIC_MAX_SLOTS; calls that overlap on the GPU race)."""
+        self._check(lib().nb_forces_static(self._h, _dptr(f), _dptr(energies), _dptr(virial)))
 
     def step(self, x, rlist_inner, part, nparts, f):
         self._check(lib().nb_step(self._h, _dptr(x), C.c_float(rlist_inner), C.c_int(part), C.c_int(nparts), _dptr(f)))
