@@ -21,7 +21,8 @@
  * Pins (tests/test_oracle_*.py, run with -m "not gpu"): closed-form single
  * pairs T1/T2/T3, beta T4, image brute force T5, Newton T6, translation T7,
  * finite differences T8, virial identities T9, pair-count T14, exclusion
- * extremes T15.  No function here is "parity unpinned".
+ * extremes T15; oracle_forces_split: parts sum to the whole, the local part equals the all-pairs sum of
+ * the local atoms alone (tests/test_oracle_split.py).  No function here is "parity unpinned".
  *
  * Build: gcc -O2 -fopenmp -ffp-contract=off -shared -fPIC (oracle/build_oracle.py).
  * -ffp-contract=off matters: the list predicates below must round exactly where
@@ -223,6 +224,34 @@ int oracle_forces_allpairs(int n, const double* x, const double* q, const int32_
         }
     }
     reduce_accum(n, nt, part, f, E, vir, npairs);
+    return 0;
+}
+
+/*
+ * Local / non-local split (with domain decomposition "non-bonded work [is split] into two kernels: one for
+ * local-only interactions and one for interactions that involve non-local particles"; reading A25): atoms
+ * [0, nlocal) are the domain's local (home) atoms, atoms [nlocal, n) its non-local (halo) atoms.  The same double
+ * loop as oracle_forces_allpairs restricted to   which = 1: pairs with BOTH atoms local;
+ * which = 2: pairs with AT LEAST ONE non-local atom;   which = 0: every pair.  (Which non-local/non-local pairs a
+ * rank of a decomposed run owns is a domain-decomposition rule, out of scope: here every pair of the system belongs
+ * to exactly one of the two parts, so part 1 + part 2 = the whole.)
+ */
+int oracle_forces_split(int n, int nlocal, int which, const double* x, const double* q, const int32_t* type,
+                        const double* box, const float* lj, const int32_t* excl_off, const int32_t* excl_idx,
+                        const oracle_params* p, double* f, double* E, double* vir, long long* npairs)
+{
+    accum* part = alloc_accum(n, 1);
+    for (int i = 0; i < n; i++) {
+        for (int j = i + 1; j < n; j++) {
+            int both_local = i < nlocal && j < nlocal;
+            if (which == 1 && !both_local) continue;
+            if (which == 2 && both_local) continue;
+            double d[3] = { x[3 * i] - x[3 * j], x[3 * i + 1] - x[3 * j + 1], x[3 * i + 2] - x[3 * j + 2] };
+            min_image(d, box);
+            add_pair(p, q, type, lj, excl_off, excl_idx, i, j, d, &part[0]);
+        }
+    }
+    reduce_accum(n, 1, part, f, E, vir, npairs);
     return 0;
 }
 

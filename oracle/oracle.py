@@ -115,6 +115,30 @@ def forces(x, q, typ, box, lj_c6c12, excl_off, excl_idx, p: Params, method: str 
     return ForceResult(f, float(e[0]), float(e[1]), vir.reshape(3, 3), int(npairs[0]), int(npairs[1]))
 
 
+def forces_split(x, q, typ, box, lj_c6c12, excl_off, excl_idx, p: Params, nlocal: int, which: int) -> ForceResult:
+    """Local / non-local split (reading A25): which = 1 pairs among the local atoms [0, nlocal),
+    which = 2 pairs with at least one non-local atom, which = 0 all pairs."""
+    x64 = np.ascontiguousarray(x, dtype=np.float64)
+    q64 = np.ascontiguousarray(q, dtype=np.float64)
+    t = np.ascontiguousarray(typ, dtype=np.int32)
+    b64 = np.ascontiguousarray(box, dtype=np.float64)
+    lj = np.ascontiguousarray(lj_c6c12, dtype=np.float32)
+    eo = np.ascontiguousarray(excl_off, dtype=np.int32)
+    ei = np.ascontiguousarray(excl_idx, dtype=np.int32)
+    if ei.size == 0:
+        ei = np.zeros(1, dtype=np.int32)
+    n = x64.shape[0]
+    f = np.zeros((n, 3), dtype=np.float64)
+    e = np.zeros(2, dtype=np.float64)
+    vir = np.zeros(9, dtype=np.float64)
+    npairs = np.zeros(2, dtype=np.int64)
+    pc = p.c()
+    lib().oracle_forces_split(C.c_int(n), C.c_int(int(nlocal)), C.c_int(int(which)), _ptr(x64), _ptr(q64), _ptr(t),
+                              _ptr(b64), _ptr(lj), _ptr(eo), _ptr(ei), C.byref(pc), _ptr(f), _ptr(e), _ptr(vir),
+                              _ptr(npairs))
+    return ForceResult(f, float(e[0]), float(e[1]), vir.reshape(3, 3), int(npairs[0]), int(npairs[1]))
+
+
 def virial_shift_identity(x, q, typ, box, lj_c6c12, excl_off, excl_idx, p: Params) -> np.ndarray:
     x64 = np.ascontiguousarray(x, dtype=np.float64)
     q64 = np.ascontiguousarray(q, dtype=np.float64)
