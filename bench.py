@@ -105,6 +105,9 @@ def parse_args():
     ap.add_argument("--first-prune", default="separate", choices=["separate", "fused"],
                     help="first use of a fresh list: nb_prune(.., 0, 1) then nb_forces (separate), or the one-kernel nb_forces_prune "
                          "(fused, PAPER.md L189)")
+    ap.add_argument("--split-frac", type=float, default=0.0,
+                    help="side measurement of the local / non-local kernel pair (SURVEY 8.1 f4, PAPER.md L101): the molecules with "
+                         "x < frac * Lx are local, the rest non-local; prints its own JSON line instead of the bench line")
     return ap.parse_args()
 
 
@@ -661,10 +664,78 @@ def run_b200(args):
     return 0
 
 
+def run_split(args):
+    """Inner steps with the force work as the paper's two kernels: put + rolling prune, then
+    nb_forces_nonlocal (high-priority stream) and nb_forces_local.  Reports when the halo forces are complete (host clock
+    at the return of nb_sync_nonlocal) and when everything is, next to the same steps through nb_forces.  One GPU; not
+    the bench line."""
+    import time
+
+    import numpy as np
+    import torch
+    from paper_2006_09167_b200 import nb, workloads
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the non-bonded path has no CPU fallback")
+    w0 = load_workload(args)
+    w, nlocal = workloads.local_first(w0, lambda x: x[:, 0] < args.split_frac * w0.box[0])
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    ctx = nb.context_for(w, device=0)
+    ctx.set_local(nlocal)
+    frames = torch.from_numpy(np.stack([w.positions_at(t) for t in range(w.nstlist)])).to(dev)
+    q, typ = torch.from_numpy(w.q).to(dev), torch.from_numpy(w.type).to(dev)
+    f = torch.zeros((w.natoms, 3), dtype=torch.float32, device=dev)
+    flush = None if args.no_flush else torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    ctx.put_atoms(frames[0], q, typ, w.box)
+    ctx.search(w.rlist_outer)
+    ctx.prune(w.rlist_inner, 0, 1)
+    info = ctx.split_info()
+
+    def step(fr, split):
+        ctx.put_atoms(frames[fr], None, None, w.box)
+        ctx.prune(w.rlist_inner, fr % w.nparts, w.nparts)
+        if split:
+            ctx.forces_nonlocal(f)
+            ctx.forces_local(f)
+        else:
+            ctx.forces(f, None, None)
+
+    out = {}
+    for split in (False, True):
+        t_halo, t_all = [], []
+        for k in range(args.warmup + args.steps):
+            fr = 1 + k % (w.nstlist - 1)
+            if flush is not None:
+                flush.fill_(1)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            step(fr, split)
+            if split:
+                ctx.sync_nonlocal()
+                t1 = time.perf_counter()
+            torch.cuda.synchronize()
+            t2 = time.perf_counter()
+            if k >= args.warmup:
+                t_all.append(t2 - t0)
+                if split:
+                    t_halo.append(t1 - t0)
+        out["split" if split else "union"] = {"us_all_forces": 1e6 * float(np.median(t_all)),
+                                              **({"us_halo_forces": 1e6 * float(np.median(t_halo))} if split else {})}
+    print(json.dumps({"measurement": "local / non-local kernel pair (SURVEY 8.1 f4, PAPER.md L101), inner step = put + rolling "
+                                     "prune + forces, host clock from the first call to completion, median",
+                      "config": workload_config(w, args, {"nlocal": nlocal, "split_frac": args.split_frac,
+                                                          "segments_local": info["nseg_local"],
+                                                          "segments_nonlocal": info["nseg"] - info["nseg_local"]}),
+                      "steps": args.steps, "warmup": args.warmup, **out}))
+    return 0
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.split_frac > 0:
+        return run_split(args)
     return run_b200(args)
 
 

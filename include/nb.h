@@ -146,6 +146,37 @@ int nb_forces_host(nb_ctx*, float* f, double* energies, double* virial);
  * same inner list bit for bit, forces equal up to summation order.  Same argument rules as nb_prune / nb_forces. */
 int nb_forces_prune(nb_ctx*, float rlist_inner, float* f, double* energies, double* virial);
 
+/* Local / non-local split of the non-bonded work (with domain decomposition "interactions with particles
+ * not local to the domain depend on halo exchange.  This is handled by splitting non-bonded work into two kernels: one for
+ * local-only interactions and one for interactions that involve non-local particles. ... launch non-local work in a high
+ * priority stream to preempt the local kernel and return remote forces early, while the local kernel execution can overlap
+ * with communication").  This library is the kernel side of that design on ONE GPU; the halo exchange itself (which atoms
+ * a rank receives, the transfers) is the caller's.
+ *   nb_set_local(nlocal): atoms [0, nlocal) of the caller's order are the domain's LOCAL (home) atoms, atoms
+ *     [nlocal, natoms) its NON-LOCAL (halo) atoms.  Takes effect at the next nb_search (required: the current list is
+ *     dropped), which grids the two classes separately so that every cluster is purely local or non-local; lists, prune,
+ *     nb_forces, nb_step work as before on the union.  nlocal = natoms (the default) switches the split off.
+ *   nb_forces_nonlocal(f): enqueues, on the library's HIGH-PRIORITY stream (ordered after everything enqueued on the
+ *     context's stream so far), the force kernel over the pairs of the inner list that involve at least one non-local
+ *     atom, then writes the finished forces of the non-local atoms to f[nlocal .. natoms) ([dev] natoms*3 as in nb_forces;
+ *     rows of local atoms are not touched by this call).  Every atom pair of the system is in exactly one of the two
+ *     kernels (which non-local/non-local pairs a rank owns is a decomposition rule the caller applies by what it puts in).
+ *   nb_sync_nonlocal(): blocks the host until those non-local forces are complete (the point where a caller sends them
+ *     back to their home ranks while the local kernel still runs).
+ *   nb_forces_local(f): enqueues the local-local kernel on the context's stream -- it runs next to the non-local one -- and,
+ *     after both kernels, writes the forces of the local atoms (local-local + their share of the non-local pairs) to
+ *     f[0 .. nlocal).  Must follow nb_forces_nonlocal (NB_ERR_STATE otherwise); after it f equals what nb_forces(f, NULL,
+ *     NULL) gives, up to the order of the atomic adds.  Force-only flavour (energies / virial: nb_forces).  Not available
+ *     while stage timing is on. */
+int nb_set_local(nb_ctx*, int32_t nlocal);
+int nb_forces_nonlocal(nb_ctx*, float* f);
+int nb_forces_local(nb_ctx*, float* f);
+int nb_sync_nonlocal(nb_ctx*);
+/* Introspection of the split after nb_search: clusters [0, nclusters_local) hold local atoms only, the others non-local
+ * atoms only; the force kernel's segment order (the order nb_inner_dump walks) has the nseg_local local-local segments
+ * first, then the nseg - nseg_local segments that involve a non-local cluster. */
+int nb_split_info(nb_ctx*, int32_t* nlocal, int32_t* nclusters_local, int32_t* nseg_local, int32_t* nseg);
+
 /* nb_forces for callers that cannot call cudaMalloc (a stream under CUDA graph capture, a tight serving loop, a harness
  * that forbids it): same arguments, same kernels, same results up to the order of the atomic adds, but the call allocates
  * NOTHING -- no cudaMalloc / cudaFree, no event creation, no allocating library routine.  The force kernel's scratch (the

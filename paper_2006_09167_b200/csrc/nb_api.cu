@@ -58,6 +58,7 @@ extern "C" int nb_init(const nb_params* p, nb_ctx** out)
     c->stream = (cudaStream_t)p->stream;
     c->natoms = p->natoms;
     c->ntypes = p->ntypes;
+    c->nlocal = p->natoms;         // no local / non-local split until nb_set_local
     nbi_static_scratch_setup(c);   // nb_forces_static: device address of the static scratch, once per device (never fails nb_init)
     if (cudaDeviceGetAttribute(&c->nsm, cudaDevAttrMultiProcessorCount, p->device) != cudaSuccess || c->nsm <= 0) c->nsm = 148;
     *out = c;   // returned even on failure below so that nb_last_error() can be read; nb_free() it
@@ -256,6 +257,63 @@ extern "C" int nb_forces(nb_ctx* c, float* f, double* energies, double* virial)
     if (virial && !energies) return nb_fail(c, NB_ERR_ARG, "nb_forces: virial needs energies (same kernel flavour)");
     if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "nb_forces without a valid list (call nb_search)");
     return nbi_forces(c, f, energies, virial);
+}
+
+// ---- local / non-local split ----
+extern "C" int nb_set_local(nb_ctx* c, int32_t nlocal)
+{
+    if (!c) return NB_ERR_ARG;
+    DeviceGuard guard(c);
+    if (nlocal < 1 || nlocal > c->natoms) return nb_fail(c, NB_ERR_ARG, "nb_set_local: nlocal = %d outside [1, %d]", nlocal, c->natoms);
+    if (c->nl_pending) return nb_fail(c, NB_ERR_STATE, "nb_set_local between nb_forces_nonlocal and nb_forces_local");
+    int rc = nbi_commit_pending(c);
+    if (rc != NB_OK) return rc;
+    if (nlocal != c->nlocal) {
+        c->nlocal = nlocal;
+        c->have_list = false;   // the grid changes: a new search is needed
+        c->have_grid = false;
+        c->cold = true;         // and its buffers are sized afresh
+    }
+    return nlocal < c->natoms ? nbi_split_setup(c) : NB_OK;
+}
+
+extern "C" int nb_forces_nonlocal(nb_ctx* c, float* f)
+{
+    if (!c) return NB_ERR_ARG;
+    DeviceGuard guard(c);
+    if (!f) return nb_fail(c, NB_ERR_ARG, "nb_forces_nonlocal: f is null");
+    if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "nb_forces_nonlocal without a valid list (call nb_search)");
+    if (c->nl_pending) return nb_fail(c, NB_ERR_STATE, "nb_forces_nonlocal twice without nb_forces_local");
+    if (c->timing) return nb_fail(c, NB_ERR_STATE, "nb_forces_nonlocal: stage timing is not available for the split kernels");
+    int rc = nbi_commit_pending(c);
+    return rc != NB_OK ? rc : nbi_forces_nonlocal(c, f);
+}
+
+extern "C" int nb_forces_local(nb_ctx* c, float* f)
+{
+    if (!c) return NB_ERR_ARG;
+    DeviceGuard guard(c);
+    if (!f) return nb_fail(c, NB_ERR_ARG, "nb_forces_local: f is null");
+    if (!c->nl_pending) return nb_fail(c, NB_ERR_STATE, "nb_forces_local without a preceding nb_forces_nonlocal");
+    return nbi_forces_local(c, f);
+}
+
+extern "C" int nb_sync_nonlocal(nb_ctx* c)
+{
+    if (!c) return NB_ERR_ARG;
+    DeviceGuard guard(c);
+    return nbi_sync_nonlocal(c);
+}
+
+extern "C" int nb_split_info(nb_ctx* c, int32_t* nlocal, int32_t* nclusters_local, int32_t* nseg_local, int32_t* nseg)
+{
+    if (!c) return NB_ERR_ARG;
+    if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "nb_split_info without a valid list (call nb_search)");
+    if (nlocal) *nlocal = c->nlocal;
+    if (nclusters_local) *nclusters_local = c->nsc_local * NB_SUPER_SIZE;
+    if (nseg_local) *nseg_local = c->nseg_local;
+    if (nseg) *nseg = c->nseg_launch;
+    return NB_OK;
 }
 
 extern "C" int nb_forces_static(nb_ctx* c, float* f, double* energies, double* virial)
@@ -474,6 +532,8 @@ extern "C" void nb_free(nb_ctx* c)
     DeviceGuard guard(c);
     if (c->side_stream) cudaStreamSynchronize(c->side_stream);
     cudaStreamSynchronize(c->stream);
+    if (c->stream_hp) cudaStreamSynchronize(c->stream_hp);
+    nbi_split_free(c);
     if (c->side_stream) cudaStreamDestroy(c->side_stream);
     for (auto& g : c->step_graphs) step_graph_release(g);
     if (c->capture_stream) cudaStreamDestroy(c->capture_stream);

@@ -49,6 +49,9 @@ struct ForceArgs {
     int2* seg_cnt_w;
     float rl2;                  // fl32(rlist_inner^2), reading A12
     int cj_dummy;
+    cudaStream_t launch_stream;   // nullptr: the context's stream
+    int seg_base, seg_count;    // launch over the segments [seg_base, seg_base + seg_count) of the force order (count 0: all
+                                // of them): the local / non-local kernels of nb_forces_local / nb_forces_nonlocal
     float4* f4;
     double* fshift;     // [27*3]
     double* energies;   // [2]
@@ -218,11 +221,12 @@ __global__ void __launch_bounds__(32, PRUNE ? 8 : 16) k_force(ForceArgs A)
     nb_pdl_trigger();
     const NbConst& K = A.kc;
     const int lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7;
-    const int4 sd = A.segd[blockIdx.x];
+    const int seg = blockIdx.x + A.seg_base;
+    const int4 sd = A.segd[seg];
     // (the part comes from a table written when nparts changes: deriving it from the unit index costs a 64-bit division)
-    const int buf = PRUNE || !A.bufmask ? 0 : (int)((A.bufmask >> A.seg_part[blockIdx.x]) & 1u);
+    const int buf = PRUNE || !A.bufmask ? 0 : (int)((A.bufmask >> A.seg_part[seg]) & 1u);
     // PRUNE: outer counts {cluster pairs without a mask, with a mask}; else inner {j-atom entries, masked pairs}
-    const int2 cnt = PRUNE ? A.ol_cnt[blockIdx.x] : A.seg_cnt[buf][blockIdx.x];
+    const int2 cnt = PRUNE ? A.ol_cnt[seg] : A.seg_cnt[buf][seg];
     const int ci = sd.z & 0x3ffffff, sid = sd.z >> 26, warp = ci & 7;
     const int nt1 = K.ntypes1;
     float4* ljw = s_ljp;
@@ -336,7 +340,7 @@ __global__ void __launch_bounds__(32, PRUNE ? 8 : 16) k_force(ForceArgs A)
     }
     if (PRUNE) {
         __syncwarp();
-        nb_ilist_finish(nu_w, nm_w, sd.x + ci, lane, A.cj_dummy, il_w, ilm_w, &A.seg_cnt_w[blockIdx.x]);
+        nb_ilist_finish(nu_w, nm_w, sd.x + ci, lane, A.cj_dummy, il_w, ilm_w, &A.seg_cnt_w[seg]);
     }
 
     float fi[24];
@@ -538,7 +542,7 @@ __global__ void __launch_bounds__(256) k_count_pairs(ForceArgs A, unsigned long 
 {
     const int4 u = A.units[blockIdx.x];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 3, k = lane & 7;
-    const int sci = u.w, h = u.x - sci * NB_NHALF, ci = sci * 8 + warp;
+    const int sci = u.w, h = (u.x - sci * NB_NENT) % NB_NHALF, ci = sci * 8 + warp;
     int sx, sy, sz;
     nb_shift_vec(nb_half_shift_id(h), sx, sy, sz);
     float xi[8], yi[8], zi[8];
@@ -610,7 +614,8 @@ int launch_force(nb_ctx* c, const ForceArgs& A)
     const size_t smem = sizeof(float4) * 4 * (size_t)c->kc.ntypes1;   // paired LJ table of one i-cluster, 64 B per type
     if (smem > 48 * 1024)
         NB_CUDA(c, cudaFuncSetAttribute(k_force<COUL, ENERGY, TWIN, PRUNE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    NB_CUDA(c, nb_launch_pdl(k_force<COUL, ENERGY, TWIN, PRUNE>, dim3(c->nseg_launch), dim3(32), smem, c->stream, A));
+    NB_CUDA(c, nb_launch_pdl(k_force<COUL, ENERGY, TWIN, PRUNE>, dim3(A.seg_count > 0 ? A.seg_count : c->nseg_launch), dim3(32), smem,
+                             A.launch_stream ? A.launch_stream : c->stream, A));
     NB_LAUNCH_CHECK(c);
     return NB_OK;
 }
@@ -996,5 +1001,114 @@ int nbi_forces_static(nb_ctx* c, float* f, double* energies, double* virial)
         NB_LAUNCH_CHECK(c);
     }
     c->st.force_count++;
+    return NB_OK;
+}
+
+// ---------------------------------------------------------------- local / non-local split
+// "splitting non-bonded work into two kernels: one for local-only interactions and one for interactions that involve
+// non-local particles ... launch non-local work in a high priority stream to preempt the local kernel and return remote
+// forces early, while the local kernel execution can overlap with communication."
+// nb_set_local makes the search grid local and non-local atoms separately, so every segment of the inner list is
+// local-local or involves a non-local cluster, and the force order lists the local segments first: the two kernels are
+// the SAME k_force over the two ranges of that order.  Both add into the one accumulator f4 (atomics); the non-local
+// atoms' slots, which only the non-local kernel touches, are the tail [64 * nsc_local, nslots_max) of the cluster order.
+static void force_args_inner(nb_ctx* c, ForceArgs& A)
+{
+    fill_force_args(c, A);
+    A.cj_dummy = c->nclusters_max;
+    const double P[5] = {NB_EWC_P0, NB_EWC_P1, NB_EWC_P2, NB_EWC_P3, NB_EWC_P4};
+    const double Q[6] = {NB_EWC_Q0, NB_EWC_Q1, NB_EWC_Q2, NB_EWC_Q3, NB_EWC_Q4, NB_EWC_Q5};
+    const double b = c->beta_d, b2 = b * b;
+    double bk = 1.0;
+    const double qlead = b2 * b2 * b2 * b2 * b2 * Q[5];
+    for (int k = 0; k < 6; k++, bk *= b2) {
+        if (k < 5) A.kc.ewp2[k] = make_float2((float)(b * b2 * bk * P[k] / qlead), (float)(b * b2 * bk * P[k] / qlead));
+        A.kc.ewq2[k] = make_float2((float)(bk * Q[k] / qlead), (float)(bk * Q[k] / qlead));
+    }
+}
+
+static int launch_force_range(nb_ctx* c, ForceArgs& A, int base, int count, cudaStream_t st)
+{
+    if (count <= 0) return NB_OK;
+    A.seg_base = base;
+    A.seg_count = count;
+    A.launch_stream = st;
+    const bool twin = c->twin;
+    if (c->prm.coulomb == NB_COUL_EWALD) return launch_force_e<NB_COUL_EWALD>(c, A, false, twin, false);
+    if (c->prm.coulomb == NB_COUL_RF) return launch_force_e<NB_COUL_RF>(c, A, false, twin, false);
+    return launch_force_e<NB_COUL_NONE>(c, A, false, twin, false);
+}
+
+// gather of the slots [slot0, slot1) (multiples of 64) to the caller's atom order
+static int gather_range(nb_ctx* c, int slot0, int slot1, float* f, cudaStream_t st)
+{
+    const int nq = (slot1 - slot0) / 4;
+    if (nq <= 0) return NB_OK;
+    NB_CUDA(c, nb_launch_pdl(k_gather4, dim3((nq + 255) / 256), dim3(256), 0, st, nq, c->f4.p + slot0,
+                             reinterpret_cast<const int4*>(c->atom_of_slot.p + slot0), f));
+    NB_LAUNCH_CHECK(c);
+    return NB_OK;
+}
+
+int nbi_split_setup(nb_ctx* c)
+{
+    if (c->stream_hp) return NB_OK;
+    int lo = 0, hi = 0;
+    NB_CUDA(c, cudaDeviceGetStreamPriorityRange(&lo, &hi));   // hi = the numerically lowest value = the highest priority
+    NB_CUDA(c, cudaStreamCreateWithPriority(&c->stream_hp, cudaStreamNonBlocking, hi));
+    NB_CUDA(c, cudaEventCreateWithFlags(&c->ev_nl_in, cudaEventDisableTiming));
+    NB_CUDA(c, cudaEventCreateWithFlags(&c->ev_nl_kernel, cudaEventDisableTiming));
+    NB_CUDA(c, cudaEventCreateWithFlags(&c->ev_nl_done, cudaEventDisableTiming));
+    return NB_OK;
+}
+
+void nbi_split_free(nb_ctx* c)
+{
+    if (c->ev_nl_in) cudaEventDestroy(c->ev_nl_in);
+    if (c->ev_nl_kernel) cudaEventDestroy(c->ev_nl_kernel);
+    if (c->ev_nl_done) cudaEventDestroy(c->ev_nl_done);
+    if (c->stream_hp) cudaStreamDestroy(c->stream_hp);
+    c->ev_nl_in = c->ev_nl_kernel = c->ev_nl_done = nullptr;
+    c->stream_hp = nullptr;
+}
+
+// The non-local kernel and the gather of the non-local atoms' forces, on the high-priority stream, ordered after
+// everything enqueued on the context's stream so far (coordinates, prune).
+int nbi_forces_nonlocal(nb_ctx* c, float* f)
+{
+    int rc = nbi_split_setup(c);
+    if (rc != NB_OK) return rc;
+    NB_CUDA(c, cudaEventRecord(c->ev_nl_in, c->stream));
+    NB_CUDA(c, cudaStreamWaitEvent(c->stream_hp, c->ev_nl_in, 0));
+    ForceArgs A;
+    force_args_inner(c, A);
+    if ((rc = launch_force_range(c, A, c->nseg_local, c->nseg_launch - c->nseg_local, c->stream_hp)) != NB_OK) return rc;
+    NB_CUDA(c, cudaEventRecord(c->ev_nl_kernel, c->stream_hp));
+    if ((rc = gather_range(c, c->nsc_local * NB_SC_ATOMS, c->nslots_max, f, c->stream_hp)) != NB_OK) return rc;
+    NB_CUDA(c, cudaEventRecord(c->ev_nl_done, c->stream_hp));
+    c->nl_pending = true;
+    c->st.force_count++;
+    return NB_OK;
+}
+
+// The local kernel on the context's stream (it runs next to the non-local one), then, once the non-local kernel has
+// added its share to the local atoms as well, the gather of the local atoms' forces.
+int nbi_forces_local(nb_ctx* c, float* f)
+{
+    ForceArgs A;
+    force_args_inner(c, A);
+    int rc = launch_force_range(c, A, 0, c->nseg_local, c->stream);
+    if (rc != NB_OK) return rc;
+    NB_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_nl_kernel, 0));
+    if ((rc = gather_range(c, 0, c->nsc_local * NB_SC_ATOMS, f, c->stream)) != NB_OK) return rc;
+    // later work on the context's stream (the next put / prune / search) must not overtake the non-local gather
+    NB_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_nl_done, 0));
+    c->nl_pending = false;
+    return NB_OK;
+}
+
+int nbi_sync_nonlocal(nb_ctx* c)
+{
+    if (c->ev_nl_done) NB_CUDA(c, cudaEventSynchronize(c->ev_nl_done));
     return NB_OK;
 }

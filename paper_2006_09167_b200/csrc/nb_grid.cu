@@ -24,7 +24,7 @@ __device__ __forceinline__ uint32_t float_orderable(float v)
 // The column counters are few (a hundred for 100k atoms) and consecutive atoms mostly share a column,
 // so the lanes of a warp that hit the same column send ONE atomic (match_any + popc ranks).
 __global__ void k_bin(int n, const float* __restrict__ x, const float* __restrict__ q, const int* __restrict__ type,
-                      int ntypes, float3 box, int ncx, int ncy, float inv_cx, float inv_cy, char4* __restrict__ image,
+                      int ntypes, float3 box, int ncx, int ncy, float inv_cx, float inv_cy, int nlocal, char4* __restrict__ image,
                       float4* __restrict__ xw_atom, int* __restrict__ atom_col, int* __restrict__ atom_rank,
                       int* __restrict__ col_count, NbTotals* __restrict__ tot)
 {
@@ -48,7 +48,7 @@ __global__ void k_bin(int n, const float* __restrict__ x, const float* __restric
         }
         int cx = min(ncx - 1, max(0, (int)floorf(w[0] * inv_cx)));
         int cy = min(ncy - 1, max(0, (int)floorf(w[1] * inv_cy)));
-        col = cx * ncy + cy;
+        col = cx * ncy + cy + (i >= nlocal ? ncx * ncy : 0);   // non-local atoms: the second column set (nb_set_local)
         image[i] = make_char4((signed char)img[0], (signed char)img[1], (signed char)img[2], 0);
         xw_atom[i] = make_float4(w[0], w[1], w[2], q[i]);
         atom_col[i] = col;
@@ -66,7 +66,7 @@ __global__ void k_bin(int n, const float* __restrict__ x, const float* __restric
 }
 
 // Single block: exclusive scans over columns of the atom count and of the super-cluster count.
-__global__ void k_col_scan(int ncol, const int* __restrict__ col_count, int* __restrict__ col_atom_off,
+__global__ void k_col_scan(int ncol, int ncol_local, const int* __restrict__ col_count, int* __restrict__ col_atom_off,
                            int* __restrict__ col_sc_off, NbTotals* __restrict__ totals)
 {
     __shared__ int s_a[1024], s_s[1024];
@@ -92,6 +92,7 @@ __global__ void k_col_scan(int ncol, const int* __restrict__ col_count, int* __r
         if (c < ncol) {
             col_atom_off[c] = carry_a + s_a[t] - cnt;
             col_sc_off[c] = carry_s + s_s[t] - nsc;
+            if (c == ncol_local) totals->nsc_local = carry_s + s_s[t] - nsc;   // first super-cluster of the non-local columns
         }
         __syncthreads();
         if (t == 1023) { carry_a += s_a[t]; carry_s += s_s[t]; }
@@ -101,6 +102,7 @@ __global__ void k_col_scan(int ncol, const int* __restrict__ col_count, int* __r
         col_atom_off[ncol] = carry_a;
         col_sc_off[ncol] = carry_s;
         totals->nsc = carry_s;
+        if (ncol_local >= ncol) totals->nsc_local = carry_s;
         totals->max_col = maxc;
     }
 }
@@ -156,7 +158,7 @@ __device__ __forceinline__ void slab_segment_sort(SlabScratch& s, const float4* 
 // 64-atom slab does the 2x2x2 sub-sorts and writes the cluster-ordered arrays and bounding boxes.
 #define NB_LAYOUT_WARPS 16   // warps per column block: one per 64-atom slab in flight (a column of config 2 holds 13 slabs)
 __global__ void __launch_bounds__(32 * NB_LAYOUT_WARPS)
-k_col_layout(int ncy, const int* __restrict__ col_atom_off, const int* __restrict__ col_sc_off,
+k_col_layout(int ncy, int ncol_local, const int* __restrict__ col_atom_off, const int* __restrict__ col_sc_off,
              const int* __restrict__ col_atoms, const float4* __restrict__ xw_atom,
              const int* __restrict__ type, int pad_type, int np2_max, float4* __restrict__ xq,
              int* __restrict__ type_slot, int* __restrict__ atom_of_slot, int* __restrict__ slot_of_atom,
@@ -228,8 +230,10 @@ k_col_layout(int ncy, const int* __restrict__ col_atom_off, const int* __restric
                 // with a spacing d_k chosen so that L_k / d_k is a half-integer: two padding atoms
                 // never coincide under any shift, and all distances stay small enough (< ~1e3 nm)
                 // for the force kernel's arithmetic to remain finite without a clamp.
-                int cx = col / ncy, cy = col % ncy;
-                v = make_float4(pad_base.x - pad_step.x * (float)e, pad_base.y - pad_step.y * (float)(cy & 63),
+                // (the padding of a non-local column, which lies on top of its local twin, sits 128 lattice steps further out)
+                const int cls = col >= ncol_local ? 1 : 0, colm = col - cls * ncol_local;
+                int cx = colm / ncy, cy = colm % ncy;
+                v = make_float4(pad_base.x - pad_step.x * (float)(e + 128 * cls), pad_base.y - pad_step.y * (float)(cy & 63),
                                 pad_base.z - pad_step.z * (float)(cx & 63), 0.f);
             }
             xq[slot] = v;
@@ -370,13 +374,16 @@ int nbi_grid(nb_ctx* c)
     c->ncol = c->ncx * c->ncy;
     c->inv_cx = (float)(c->ncx / (double)L[0]);
     c->inv_cy = (float)(c->ncy / (double)L[1]);
+    // local / non-local split (nb_set_local): the non-local atoms get a column set of their own behind the local one
+    c->nclass = c->nlocal < n ? 2 : 1;
+    c->ncol_tot = c->ncol * c->nclass;
     // sum over columns of ceil(count/64) <= natoms/64 + columns: everything below is sized by this bound
-    c->nsc_max = n / NB_SC_ATOMS + c->ncol;
+    c->nsc_max = n / NB_SC_ATOMS + c->ncol_tot;
     c->nclusters_max = c->nsc_max * NB_SUPER_SIZE;
     c->nslots_max = c->nsc_max * NB_SC_ATOMS;
-    NB_CUDA(c, c->col_count.ensure(c->ncol + 1, st));
-    NB_CUDA(c, c->col_atom_off.ensure(c->ncol + 1, st));
-    NB_CUDA(c, c->col_sc_off.ensure(c->ncol + 1, st));
+    NB_CUDA(c, c->col_count.ensure(c->ncol_tot + 1, st));
+    NB_CUDA(c, c->col_atom_off.ensure(c->ncol_tot + 1, st));
+    NB_CUDA(c, c->col_sc_off.ensure(c->ncol_tot + 1, st));
     NB_CUDA(c, c->atom_col.ensure(n, st));
     NB_CUDA(c, c->atom_rank.ensure(n, st));
     NB_CUDA(c, c->col_atoms.ensure(n, st));
@@ -392,12 +399,12 @@ int nbi_grid(nb_ctx* c)
     NB_CUDA(c, c->sbb_hi.ensure(c->nsc_max, st));
     NB_CUDA(c, c->f4.ensure(c->nslots_max + NB_C * NB_NDUMMY, st));
     NB_CUDA(c, cudaMemsetAsync(c->f4.p, 0, sizeof(float4) * (c->nslots_max + NB_C * NB_NDUMMY), st));
-    NB_CUDA(c, cudaMemsetAsync(c->col_count.p, 0, sizeof(int) * (c->ncol + 1), st));
+    NB_CUDA(c, cudaMemsetAsync(c->col_count.p, 0, sizeof(int) * (c->ncol_tot + 1), st));
     float3 box = make_float3(L[0], L[1], L[2]);
     k_bin<<<(n + 255) / 256, 256, 0, st>>>(n, c->x.p, c->q.p, c->type.p, c->ntypes, box, c->ncx, c->ncy, c->inv_cx, c->inv_cy,
-                                           c->image.p, c->xw_atom.p, c->atom_col.p, c->atom_rank.p, c->col_count.p, c->tot_dev);
+                                           c->nlocal, c->image.p, c->xw_atom.p, c->atom_col.p, c->atom_rank.p, c->col_count.p, c->tot_dev);
     NB_LAUNCH_CHECK(c);
-    k_col_scan<<<1, 1024, 0, st>>>(c->ncol, c->col_count.p, c->col_atom_off.p, c->col_sc_off.p, c->tot_dev);
+    k_col_scan<<<1, 1024, 0, st>>>(c->ncol_tot, c->ncol, c->col_count.p, c->col_atom_off.p, c->col_sc_off.p, c->tot_dev);
     NB_LAUNCH_CHECK(c);
     k_col_scatter<<<(n + 255) / 256, 256, 0, st>>>(n, c->atom_col.p, c->atom_rank.p, c->col_atom_off.p,
                                                    c->col_atoms.p);
@@ -422,13 +429,13 @@ int nbi_grid(nb_ctx* c)
         pd[k] = (float)(L[k] / (floor(L[k] / 3.0) + 0.5));   // L/d half-integer, d in (2, 6] nm (2L for L < 3)
         pb[k] = (float)(-(2.0 * L[k] + 8.0));
     }
-    k_col_layout<<<c->ncol, 32 * NB_LAYOUT_WARPS, smem, st>>>(c->ncy, c->col_atom_off.p, c->col_sc_off.p, c->col_atoms.p,
+    k_col_layout<<<c->ncol_tot, 32 * NB_LAYOUT_WARPS, smem, st>>>(c->ncy, c->ncol, c->col_atom_off.p, c->col_sc_off.p, c->col_atoms.p,
                                              c->xw_atom.p, c->type.p, c->ntypes, np2, c->xq.p, c->type_slot.p,
                                              c->atom_of_slot.p, c->slot_of_atom.p, c->bb_lo.p, c->bb_hi.p,
                                              c->sbb_lo.p, c->sbb_hi.p, make_float3(pb[0], pb[1], pb[2]),
                                              make_float3(pd[0], pd[1], pd[2]), c->tot_dev);
     NB_LAUNCH_CHECK(c);
-    k_grid_tail<<<(c->ncol * NB_SC_ATOMS + 255) / 256, 256, 0, st>>>(c->nsc_max, c->tot_dev, c->ntypes, c->xq.p, c->type_slot.p,
+    k_grid_tail<<<(c->ncol_tot * NB_SC_ATOMS + 255) / 256, 256, 0, st>>>(c->nsc_max, c->tot_dev, c->ntypes, c->xq.p, c->type_slot.p,
                                                                    c->atom_of_slot.p, c->bb_lo.p, c->bb_hi.p, c->sbb_lo.p,
                                                                    c->sbb_hi.p, make_float3(pb[0], pb[1], pb[2]),
                                                                    make_float3(pd[0], pd[1], pd[2]));

@@ -15,6 +15,10 @@
 #define NB_C NB_CLUSTER_SIZE          // atoms per cluster
 #define NB_SC_ATOMS 64                // atoms per super-cluster (8 clusters x 8 atoms)
 #define NB_NHALF 14                   // zero shift + 13 shifts with s >lex 0
+#define NB_NENT (2 * NB_NHALF)        // list elements per super-cluster: (j class, shift); element e of super-cluster sci
+                                      // is sci * NB_NENT + jcls * NB_NHALF + h.  j class 1 = non-local j clusters
+                                      // (nb_set_local; empty otherwise), so every element, work unit and segment is
+                                      // purely local or non-local
 #define NB_BATCH 32                   // joint j entries per mask word (one ballot)
 #define NB_MAX_UNIT_BATCHES 16        // a work unit spans at most this many batches of one list element
 #define NB_NDUMMY 1024                // dummy j-clusters behind the real ones (spread the never-read force adds)
@@ -33,7 +37,9 @@ struct NbTotals {
     int nseg_launch;           // segments with a non-empty outer list
     int overflow;              // NB_OVF_* bits: a stage found its buffer too small and did nothing
     int bad_type;              // an atom type outside [0, ntypes)
-    int pad[6];
+    int nsc_local;             // (a2) super-clusters of local atoms: they come first (nb_set_local; = nsc otherwise)
+    int nseg_local;            // non-empty segments whose pairs are local-local: first in the force kernel's order
+    int pad[4];
 };
 enum { NB_OVF_COL = 1, NB_OVF_JOINT = 2, NB_OVF_UNITS = 4, NB_OVF_MASKS = 8, NB_OVF_IL = 16, NB_OVF_ILM = 32 };
 #define NB_SEG_MAXKEY 2080              // segment length key (see k_ilist_caps) is below this
@@ -118,6 +124,14 @@ struct nb_ctx {
 
     // --- grid (a2) ---
     int ncx = 0, ncy = 0, ncol = 0;
+    // local / non-local split (nb_set_local): atoms [0, nlocal) are local, the rest non-local (halo).
+    // The two classes are gridded into separate column sets (ncol_tot = nclass * ncol columns, class 1 after class 0),
+    // so that clusters, super-clusters, list elements and segments are pure; nlocal = natoms: one class, nothing changes.
+    int nlocal = 0, nclass = 1, ncol_tot = 0;
+    int nsc_local = 0, nseg_local = 0;         // known after the end-of-search synchronisation
+    cudaStream_t stream_hp = nullptr;          // high-priority stream of the non-local kernel
+    cudaEvent_t ev_nl_in = nullptr, ev_nl_kernel = nullptr, ev_nl_done = nullptr;
+    bool nl_pending = false;                   // nb_forces_nonlocal enqueued, nb_forces_local not yet
     float inv_cx = 0.f, inv_cy = 0.f;          // columns per nm
     DevBuf<int32_t> col_count, col_atom_off, col_sc_off, atom_col, atom_rank, col_atoms;
     DevBuf<char4> image;                       // periodic image fixed at the last search
@@ -131,7 +145,7 @@ struct nb_ctx {
     DevBuf<float4> f4;                         // [nslots] force accumulator (x,y,z,unused), kept zero between calls
 
     // --- pair list (a3, a4) ---
-    int nent = 0;                              // nsc * NB_NHALF (super-cluster, shift) slots, some empty
+    int nent = 0;                              // nsc * NB_NENT (super-cluster, j class, shift) slots, some empty
     DevBuf<int32_t> ent_count;                 // [nent] joint entries per slot
     DevBuf<int32_t> ent_jbegin;                // [nent+1] first j slot (multiple of NB_BATCH)
     int64_t njslots = 0, nbatch = 0;
@@ -379,5 +393,10 @@ int nbi_ljrows(nb_ctx* c);                                  // nb_force.cu: pair
 int nbi_exclusive_scan(nb_ctx* c, const int32_t* in, int32_t* out, int64_t n, int32_t* total_dev);  // nb_list.cu
 const void* nbi_put_kernel();                               // nb_grid.cu: the k_put entry (node lookup in captured graphs)
 const void* nbi_gather4_kernel();                           // nb_force.cu: the k_gather4 entry
+int nbi_split_setup(nb_ctx* c);                             // nb_force.cu: high-priority stream and events of the local / non-local split
+void nbi_split_free(nb_ctx* c);
+int nbi_forces_nonlocal(nb_ctx* c, float* f);               // nb_force.cu: non-local kernel + gather of the non-local atoms
+int nbi_forces_local(nb_ctx* c, float* f);                  // nb_force.cu: local kernel + gather of the local atoms
+int nbi_sync_nonlocal(nb_ctx* c);
 void nbi_static_scratch_setup(nb_ctx* c);                   // nb_force.cu: resolves c->static_scratch (the context's device is current)
 int nbi_forces_static(nb_ctx* c, float* f, double* energies, double* virial);   // nb_force.cu: nb_forces_static

@@ -177,6 +177,7 @@ int exclusive_scan(nb_ctx* c, F f, int32_t* out, int64_t n, int32_t* total_dev)
 // ---------------------------------------------------------------- search
 struct SearchArgs {
     int nsc_max, ncx, ncy;
+    int nclass;     // 2 with a local / non-local split (nb_set_local): the j side is searched per class, one list element each
     float inv_cx, inv_cy;
     float box[3];
     float rl2;      // fl32(rlist*rlist): the exact predicate's threshold (reading A12)
@@ -211,14 +212,16 @@ __global__ void __launch_bounds__(128) k_search(SearchArgs A)
     const int sci = blockIdx.x * 4 + warp;
     if (sci >= A.nsc_max) return;
     if (sci >= A.tot->nsc) {   // between the actual count and the host's bound: empty list elements
-        if (!FILL && lane < NB_NHALF) A.ent_count[sci * NB_NHALF + lane] = 0;
+        if (!FILL && lane < NB_NENT) A.ent_count[sci * NB_NENT + lane] = 0;
         return;
     }
     if (FILL && stage_overflow(A.tot, A.caps)) return;
     const int g = lane >> 3, k = lane & 7;
     const float4 ilo = A.bb_lo[sci * 8 + k], ihi = A.bb_hi[sci * 8 + k];
     const float4 slo = A.sbb_lo[sci], shi = A.sbb_hi[sci];
-    for (int h = 0; h < NB_NHALF; h++) {
+    if (!FILL && A.nclass == 1 && lane < NB_NHALF) A.ent_count[sci * NB_NENT + NB_NHALF + lane] = 0;   // no non-local j class
+    for (int hh = 0; hh < NB_NHALF * A.nclass; hh++) {
+        const int h = hh % NB_NHALF, jcls = hh / NB_NHALF;
         int sx, sy, sz;
         nb_shift_vec(nb_half_shift_id(h), sx, sy, sz);
         const float fx = (float)sx, fy = (float)sy, fz = (float)sz;
@@ -237,7 +240,7 @@ __global__ void __launch_bounds__(128) k_search(SearchArgs A)
                               __fmaf_rn(fz, A.box[2], slo.z)};
         const float thi[3] = {__fmaf_rn(fx, A.box[0], shi.x), __fmaf_rn(fy, A.box[1], shi.y),
                               __fmaf_rn(fz, A.box[2], shi.z)};
-        const int ent = sci * NB_NHALF + h;
+        const int ent = sci * NB_NENT + hh;
         int count = 0;
         const int base = FILL ? A.ent_jbegin[ent] : 0;
         // candidate columns: those that can hold an atom within rm of the shifted i super-box
@@ -249,7 +252,7 @@ __global__ void __launch_bounds__(128) k_search(SearchArgs A)
             const int cy0 = max(0, (int)floorf(ylo * A.inv_cy)), cy1 = min(A.ncy - 1, (int)floorf(yhi * A.inv_cy));
             for (int cx = cx0; cx <= cx1; cx++) {
                 for (int cy = cy0; cy <= cy1; cy++) {
-                    const int col = cx * A.ncy + cy;
+                    const int col = cx * A.ncy + cy + jcls * A.ncx * A.ncy;
                     int s0 = A.col_sc_off[col];
                     const int s1 = A.col_sc_off[col + 1];
                     if (h == 0) s0 = max(s0, sci);   // zero shift: only cj >= ci (half list, reading A14)
@@ -286,7 +289,9 @@ __global__ void __launch_bounds__(128) k_search(SearchArgs A)
                             const unsigned lm = __ballot_sync(0xffffffffu, listed);
                             if (FILL && listed) {
                                 const int pos = base + count + __popc(lm & ((1u << lane) - 1u));
-                                A.jl[pos] = make_int2(cj, (h == 0 && scj == sci) ? 1 : 0);
+                                // own super-cluster: the diagonal cluster pair needs a mask (zero shift: b > a only; under
+                                // a shift, in boxes of a few cluster lengths: an atom never pairs with its own image)
+                                A.jl[pos] = make_int2(cj, scj == sci ? 1 : 0);
                                 A.imask[pos] = (uint8_t)imask;
                             }
                             count += __popc(lm);
@@ -357,7 +362,7 @@ __global__ void k_unit_fill(int nent, const int* __restrict__ ent_count, const i
     const int b0 = ent_jbegin[e] / NB_BATCH, u0 = unit_off[e];
     for (int k = 0; k < nsplit; k++) {
         const int b = (int)((long long)nb * k / nsplit), bend = (int)((long long)nb * (k + 1) / nsplit);
-        units[u0 + k] = make_int4(e, b0 + b, b0 + bend, e / NB_NHALF);
+        units[u0 + k] = make_int4(e, b0 + b, b0 + bend, e / NB_NENT);
         for (int bb = b; bb < bend; bb++) {
             batch_ent[b0 + bb] = e;
             batch_unit[b0 + bb] = u0 + k;
@@ -377,6 +382,9 @@ struct ExclArgs {
     NbTotals* tot;
     Caps caps;
 };
+
+// j class of a cluster: non-local clusters come after the local ones (nb_set_local)
+__device__ __forceinline__ int cluster_class(const NbTotals* tot, int cluster) { return (cluster >> 3) >= tot->nsc_local ? 1 : 0; }
 
 // One thread per atom; each unordered excluded pair is handled once (from its lower index; nb_init
 // checks that the CSR is symmetric), in both orientations and under every shift the cluster pair is
@@ -409,7 +417,7 @@ __global__ void k_excl(ExclArgs A)
                                      __fmaf_rn((float)sz, A.box[2], lo[o].z), __fmaf_rn((float)sx, A.box[0], hi[o].x),
                                      __fmaf_rn((float)sy, A.box[1], hi[o].y), __fmaf_rn((float)sz, A.box[2], hi[o].z)};
                 if (!(bb_dist2_exact(ib, lo[1 - o], hi[1 - o]) < A.rl2)) continue;
-                int ent = scp * NB_NHALF + h;
+                int ent = scp * NB_NENT + cluster_class(A.tot, cq) * NB_NHALF + h;
                 int cnt = A.ent_count[ent];
                 if (cnt == 0) continue;
                 int lo_ = A.ent_jbegin[ent], hi_ = lo_ + cnt;
@@ -443,14 +451,16 @@ __global__ void k_excl_assign(int2* __restrict__ jl, const int* __restrict__ pre
     int ref = prefix[i] + 1;
     jl[i].y = ref;
     int ent = batch_ent[i >> 5];
-    int sci = ent / NB_NHALF, h = ent % NB_NHALF;
+    int sci = ent / NB_NENT, h = (ent % NB_NENT) % NB_NHALF;
     unsigned long long upper = 0;   // bit b*8+a set iff b > a
     for (int b = 0; b < 8; b++)
         for (int a = 0; a < b; a++) upper |= 1ull << (b * 8 + a);
+    const unsigned long long not_self = ~0x8040201008040201ull;   // bit b*8+a with b == a cleared
     for (int w = 0; w < 8; w++) {
-        bool diag = h == 0 && e.x == sci * 8 + w;
-        masks[((size_t)ref * 8 + w) * 2] = diag ? upper : ~0ull;       // interact
-        masks[((size_t)ref * 8 + w) * 2 + 1] = diag ? upper : ~0ull;   // counted at all
+        const bool same = e.x == sci * 8 + w, diag = h == 0 && same;
+        const unsigned long long m = diag ? upper : (same ? not_self : ~0ull);   // (same cluster under a shift: all but a == b)
+        masks[((size_t)ref * 8 + w) * 2] = m;       // interact
+        masks[((size_t)ref * 8 + w) * 2 + 1] = m;   // counted at all
     }
 }
 
@@ -509,16 +519,27 @@ __global__ void k_ilist_caps(const int4* __restrict__ units, int nseg_cap, const
 // lists being scheduled late").  Key = part * NB_SEG_MAXKEY + (NB_SEG_MAXKEY - 1 - length); nparts = 1
 // gives the force kernel's launch order.  The order among equal keys is whatever the atomics make it:
 // only scheduling depends on it.
+// The force kernel's order (units != nullptr, nparts = 1) is keyed by locality first (a local and a
+// non-local kernel): non-empty local-local segments [0, nseg_local), longest first, then the non-empty segments that
+// involve a non-local cluster [nseg_local, nseg_launch), longest first, then the empty ones.  Without nb_set_local
+// every segment is local and the order is the plain longest-first one.
+__device__ __forceinline__ int sort_bucket(int s0, int len, int nparts, int nunits, const int4* units, const NbTotals* tot)
+{
+    if (!units) return nb_part_of_unit(s0 >> 3, nparts, nunits) * NB_SEG_MAXKEY + NB_SEG_MAXKEY - 1 - len;
+    if (len == 0) return 2 * NB_SEG_MAXKEY - 1;
+    const int4 u = units[s0 >> 3];
+    const int cls = (u.w >= tot->nsc_local || (u.x - u.w * NB_NENT) >= NB_NHALF) ? 1 : 0;
+    return cls * NB_SEG_MAXKEY + NB_SEG_MAXKEY - 1 - len;
+}
 __global__ void k_sort_hist(const int* __restrict__ seg_len, const NbTotals* __restrict__ tot, int units_cap, int nparts,
-                            int* __restrict__ hist)
+                            const int4* __restrict__ units, int* __restrict__ hist)
 {
     const int s0 = blockIdx.x * blockDim.x + threadIdx.x;
     const int nunits = tot->nunits;
     if (nunits > units_cap || s0 >= nunits * 8) return;
-    const int part = nb_part_of_unit(s0 >> 3, nparts, nunits);
-    atomicAdd(&hist[part * NB_SEG_MAXKEY + NB_SEG_MAXKEY - 1 - seg_len[s0]], 1);
+    atomicAdd(&hist[sort_bucket(s0, seg_len[s0], nparts, nunits, units, tot)], 1);
 }
-__global__ void __launch_bounds__(1024) k_sort_scan(int* __restrict__ hist, int nbuckets, NbTotals* __restrict__ tot, int nparts)
+__global__ void __launch_bounds__(1024) k_sort_scan(int* __restrict__ hist, int nbuckets, NbTotals* __restrict__ tot, bool force_order)
 {
     __shared__ int s_warp[33];
     int carry = 0;
@@ -528,18 +549,19 @@ __global__ void __launch_bounds__(1024) k_sort_scan(int* __restrict__ hist, int 
         int bt;
         const int e = block_excl_scan_1024(v, s_warp, bt);
         if (i < nbuckets) hist[i] = carry + e;
-        if (nparts == 1 && i == NB_SEG_MAXKEY - 1) tot->nseg_launch = carry + e;   // everything before the length-0 bucket
+        if (force_order && i == NB_SEG_MAXKEY) tot->nseg_local = carry + e;            // everything before the non-local buckets
+        if (force_order && i == 2 * NB_SEG_MAXKEY - 1) tot->nseg_launch = carry + e;   // everything before the length-0 bucket
         carry += bt;
     }
 }
 __global__ void k_sort_scatter(const int* __restrict__ seg_len, const NbTotals* __restrict__ tot, int units_cap, int nparts,
-                               int* __restrict__ hist, int* __restrict__ seg_of_s0, int* __restrict__ table)
+                               const int4* __restrict__ units, int* __restrict__ hist, int* __restrict__ seg_of_s0,
+                               int* __restrict__ table)
 {
     const int s0 = blockIdx.x * blockDim.x + threadIdx.x;
     const int nunits = tot->nunits;
     if (nunits > units_cap || s0 >= nunits * 8) return;
-    const int part = nb_part_of_unit(s0 >> 3, nparts, nunits);
-    const int pos = atomicAdd(&hist[part * NB_SEG_MAXKEY + NB_SEG_MAXKEY - 1 - seg_len[s0]], 1);
+    const int pos = atomicAdd(&hist[sort_bucket(s0, seg_len[s0], nparts, nunits, units, tot)], 1);
     if (table) table[pos] = seg_of_s0[s0];   // a prune order: segment ids of each part, longest first
     else seg_of_s0[s0] = pos;                // the force kernel's order: this IS the segment id
 }
@@ -570,7 +592,7 @@ __global__ void __launch_bounds__(256) k_ilist_build(BuildArgs A)
     const int o = A.il_off[s0], om = A.ilm_off[s0];
     const int t = A.seg_of_s0[s0];
     if (lane == 0)
-        A.segd[t] = make_int4(o, om, (u.w * 8 + warp) | (nb_half_shift_id(u.x - u.w * NB_NHALF) << 26), blockIdx.x);
+        A.segd[t] = make_int4(o, om, (u.w * 8 + warp) | (nb_half_shift_id((u.x - u.w * NB_NENT) % NB_NHALF) << 26), blockIdx.x);
     const unsigned lt = (1u << lane) - 1u;
     int nu = 0, nm = 0;
     for (int b = u.y; b < u.z; b++) {
@@ -700,7 +722,7 @@ __global__ void k_dump_fill(DumpArgs A)
     if (!bits) return;
     int2 je = A.jl[e];
     int ent = A.batch_ent[e >> 5];
-    int sci = ent / NB_NHALF, h = ent % NB_NHALF;
+    int sci = ent / NB_NENT, h = (ent % NB_NENT) % NB_NHALF;
     const int part = nb_part_of_unit(A.batch_unit[e >> 5], A.nparts, A.nunits);
     unsigned jvalid = 0;
     for (int b = 0; b < 8; b++) jvalid |= (A.atom_of_slot[je.x * 8 + b] >= 0 ? 1u : 0u) << b;
@@ -800,14 +822,16 @@ const int NB_RETRY = 1;
 int sort_segments(nb_ctx* c, int nparts, int nseg_cap, const int* seg_len, int* table)
 {
     cudaStream_t st = c->stream;
-    const int nbuckets = nparts * NB_SEG_MAXKEY;
+    const bool force_order = table == nullptr;   // (then nparts = 1): keyed by locality, then length
+    const int4* units = force_order ? c->units_canon.p : nullptr;
+    const int nbuckets = force_order ? 2 * NB_SEG_MAXKEY : nparts * NB_SEG_MAXKEY;
     NB_CUDA(c, c->sort_hist.ensure(nbuckets, st));
     NB_CUDA(c, cudaMemsetAsync(c->sort_hist.p, 0, sizeof(int) * nbuckets, st));
-    k_sort_hist<<<(nseg_cap + 255) / 256, 256, 0, st>>>(seg_len, c->tot_dev, (int)c->cap_units, nparts, c->sort_hist.p);
+    k_sort_hist<<<(nseg_cap + 255) / 256, 256, 0, st>>>(seg_len, c->tot_dev, (int)c->cap_units, nparts, units, c->sort_hist.p);
     NB_LAUNCH_CHECK(c);
-    k_sort_scan<<<1, 1024, 0, st>>>(c->sort_hist.p, nbuckets, c->tot_dev, nparts);
+    k_sort_scan<<<1, 1024, 0, st>>>(c->sort_hist.p, nbuckets, c->tot_dev, force_order);
     NB_LAUNCH_CHECK(c);
-    k_sort_scatter<<<(nseg_cap + 255) / 256, 256, 0, st>>>(seg_len, c->tot_dev, (int)c->cap_units, nparts, c->sort_hist.p,
+    k_sort_scatter<<<(nseg_cap + 255) / 256, 256, 0, st>>>(seg_len, c->tot_dev, (int)c->cap_units, nparts, units, c->sort_hist.p,
                                                            c->seg_of_s0.p, table);
     NB_LAUNCH_CHECK(c);
     return NB_OK;
@@ -825,7 +849,7 @@ int search_attempt(nb_ctx* c, float rlist)
     NbStageTimer* tm = new NbStageTimer(c, NB_T_SEARCH);
     struct TmGuard { NbStageTimer*& t; ~TmGuard() { delete t; } } tm_guard{tm};
     const int nsc_max = c->nsc_max;
-    c->nent = nsc_max * NB_NHALF;
+    c->nent = nsc_max * NB_NENT;
     const int nent = c->nent;
     NB_CUDA(c, c->ent_count.ensure(nent + 1, st));
     NB_CUDA(c, c->ent_jbegin.ensure(nent + 1, st));
@@ -836,6 +860,7 @@ int search_attempt(nb_ctx* c, float rlist)
     const int target_units = 6 * nsm;   // about 6 prune work units per SM (measured best on configs 1-3)
 
     SearchArgs A;
+    A.nclass = c->nclass;
     A.nsc_max = nsc_max; A.ncx = c->ncx; A.ncy = c->ncy; A.inv_cx = c->inv_cx; A.inv_cy = c->inv_cy;
     for (int k = 0; k < 3; k++) A.box[k] = c->box[k];
     A.rl2 = rlist * rlist;
@@ -970,6 +995,8 @@ int search_attempt(nb_ctx* c, float rlist)
     c->il_total = T.il_total;
     c->ilm_total = T.ilm_total;
     c->nseg_launch = T.nseg_launch;
+    c->nseg_local = T.nseg_local;
+    c->nsc_local = T.nsc_local;
     c->st.nsuper = c->nsc;
     c->st.nclusters = c->nclusters;
     c->st.nslots = c->nslots;

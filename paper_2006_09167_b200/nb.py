@@ -25,7 +25,7 @@ EXPORTS = ["nb_init", "nb_put_atoms", "nb_put_atoms_host", "nb_search", "nb_prun
            "nb_forces_host", "nb_free", "nb_last_error", "nb_get_layout", "nb_get_slots", "nb_list_count",
            "nb_list_dump", "nb_get_stats", "nb_measure_fp32_peak", "nb_count_pairs", "nb_timing_enable",
            "nb_timing_read", "nb_timing_stages", "nb_count_slots", "nb_inner_dump", "nb_prune_overlapped", "nb_forces_prune", "nb_step", "nb_measure_fp32_pipe", "nb_step_host",
-           "nb_forces_static"]
+           "nb_forces_static", "nb_set_local", "nb_forces_nonlocal", "nb_forces_local", "nb_sync_nonlocal", "nb_split_info"]
 NB_T_NAMES = ["put", "grid", "search", "masks", "prune", "force", "reduce", "force_energy"]
 
 
@@ -144,6 +144,24 @@ class Context:
     def forces(self, f, energies=None, virial=None):
         """f [N,3] f32 CUDA tensor (overwritten); energies [2] f64, virial [9] f64 CUDA tensors or None."""
         self._check(lib().nb_forces(self._h, _dptr(f), _dptr(energies), _dptr(virial)))
+
+    def set_local(self, nlocal):
+        """Atoms [0, nlocal) are local, the rest non-local (halo); takes effect at the next search."""
+        self._check(lib().nb_set_local(self._h, C.c_int32(int(nlocal))))
+
+    def forces_nonlocal(self, f):
+        self._check(lib().nb_forces_nonlocal(self._h, _dptr(f)))
+
+    def forces_local(self, f):
+        self._check(lib().nb_forces_local(self._h, _dptr(f)))
+
+    def sync_nonlocal(self):
+        self._check(lib().nb_sync_nonlocal(self._h))
+
+    def split_info(self):
+        v = [C.c_int32() for _ in range(4)]
+        self._check(lib().nb_split_info(self._h, *[C.byref(a) for a in v]))
+        return dict(nlocal=v[0].value, nclusters_local=v[1].value, nseg_local=v[2].value, nseg=v[3].value)
 
     def forces_static(self, f, energies=None, virial=None):
         """nb_forces without any allocation: the kernel's scratch is a static device array of the library (size limit:

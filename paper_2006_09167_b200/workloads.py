@@ -321,5 +321,41 @@ def water_box(nside: int) -> Workload:
                           rlist_inner=1.03, nstlist=100, nparts=2)
 
 
+def local_first(w: Workload, is_local_atom):
+    """Stand-in for the atom order of a decomposed run (local atoms and the non-local atoms received
+    in the halo exchange): returns (the workload with the molecules whose FIRST atom satisfies is_local_atom(x) moved to
+    the front, nlocal).  Pure index bookkeeping: molecules stay contiguous and whole, exclusions are remapped.
+    is_local_atom maps the [N,3] coordinates to a boolean per atom."""
+    n = w.natoms
+    mol = w.mol_of_atom
+    nmol = int(mol.max()) + 1
+    first = np.full(nmol, n, dtype=np.int64)
+    np.minimum.at(first, mol, np.arange(n))
+    flag_mol = np.asarray(is_local_atom(w.x))[first]
+    key = np.where(flag_mol[mol], 0, 1)
+    perm = np.argsort(key, kind="stable")          # new position k holds old atom perm[k]
+    inv = np.empty(n, dtype=np.int64)
+    inv[perm] = np.arange(n)
+    nlocal = int((key == 0).sum())
+    counts = (w.excl_off[1:] - w.excl_off[:-1])[perm]
+    off = np.concatenate([[0], np.cumsum(counts)]).astype(np.int32)
+    idx = np.empty(int(off[-1]), dtype=np.int32)
+    for k in range(n):                               # rows are short (intramolecular): a plain loop
+        o = perm[k]
+        idx[off[k]:off[k + 1]] = np.sort(inv[w.excl_idx[w.excl_off[o]:w.excl_off[o + 1]]])
+    mol_old = mol[perm]
+    _, first_pos, mol_new = np.unique(mol_old, return_index=True, return_inverse=True)
+    order = np.argsort(first_pos, kind="stable")    # new molecule ids in order of first appearance
+    rank = np.empty_like(order)
+    rank[order] = np.arange(order.size)
+    mol_new = rank[mol_new].astype(np.int32)
+    old_of_new_mol = np.unique(mol_old)[order]
+    w2 = dataclasses.replace(
+        w, name=w.name + "_localfirst", x=np.ascontiguousarray(w.x[perm]), q=np.ascontiguousarray(w.q[perm]),
+        type=np.ascontiguousarray(w.type[perm]), excl_off=off, excl_idx=idx, mol_of_atom=mol_new,
+        unit_dir=np.ascontiguousarray(w.unit_dir[old_of_new_mol]))
+    return w2, nlocal
+
+
 def by_index(k: int, **kw) -> Workload:
     return [config0, config1, config2, config3, config4][k](**kw)
