@@ -20,7 +20,8 @@
  *  - Call order: nb_init -> nb_put_atoms -> nb_search -> { nb_put_atoms -> [nb_prune | nb_prune_overlapped]
  *    -> nb_forces }* -> nb_put_atoms -> nb_search ...; violations return NB_ERR_STATE.  The first use of a
  *    fresh list may be nb_forces_prune instead of nb_prune + nb_forces; nb_step / nb_step_host are one pass
- *    of the braces in one call.
+ *    of the braces in one call; nb_forces_nonlocal + nb_forces_local (after nb_set_local and a search) or
+ *    nb_forces_static stand where nb_forces does.
  *  - Units: nm, kJ/mol, e.  Rectangular periodic boxes only.  natoms, types, charges'
  *    layout and exclusions are fixed for the lifetime of a context (only
  *    positions change per step).
