@@ -113,6 +113,9 @@ def test_split_config1_rolling_and_step(cfg1):
             d.ctx.step(xt, w.rlist_inner, part, w.nparts, fx)       # the one-call inner step on the split grid
             d.torch.cuda.synchronize()
             d.x = xt
+        elif t == 2:
+            d.put(x)
+            d.ctx.prune_overlapped(w.rlist_inner, part, w.nparts)   # second stream; joined by the split calls / the dump
         else:
             d.put(x)
             d.ctx.prune(w.rlist_inner, part, w.nparts)
