@@ -142,6 +142,39 @@ def test_split_config1_rolling_and_step(cfg1):
     assert rel_rms(d.forces(), oracle_forces(w, method="cells").f) <= TOL_F
 
 
+def test_split_config4_heterogeneous_full_size():
+    """The slab / vapour system with five atom types and random charges at full size (150k atoms): half of the dense slab
+    is local, the other half and the vapour non-local; sampled list ranges on both sides of the class boundary."""
+    import dataclasses
+    from tests.test_gpu_parity import spread_ranges
+    w0 = W.config4()
+    w, nlocal = local_first(w0, lambda x: x[:, 0] < 9.0)
+    assert 0.2 * w.natoms < nlocal < 0.6 * w.natoms
+    d = Driver(w)
+    d.ctx.set_local(nlocal)
+    d.put()
+    d.ctx.search(w.rlist_outer)
+    d.ctx.prune(w.rlist_inner, 0, 1)
+    info = check_partition(d, nlocal)
+    ncl = d.ctx.get_layout()["nclusters"]
+    ncl_loc = info["nclusters_local"]
+    ranges = [(max(ncl_loc - 12, 0), min(ncl_loc + 12, ncl))] + spread_ranges(ncl, 4, 16)   # the first straddles the class boundary
+    for r in ranges:
+        check_lists(d, w, w.rlist_outer, w.rlist_inner, c_range=r)
+    check_half_list(d, w, c_ranges=ranges)
+    whole = oracle_forces(w, method="cells")
+    f_nl, f = split_forces(d, nlocal)
+    assert rel_rms(f_nl[nlocal:], whole.f[nlocal:]) <= TOL_F and np.isnan(f_nl[:nlocal]).all()
+    assert rel_rms(f, whole.f) <= TOL_F
+    # a moved frame after a rolling prune
+    x = w.positions_at(3)
+    d.put(x)
+    d.ctx.prune(w.rlist_inner, 3 % w.nparts, w.nparts)
+    whole = oracle_forces(dataclasses.replace(w, x=x), method="cells")
+    f_nl, f = split_forces(d, nlocal)
+    assert rel_rms(f_nl[nlocal:], whole.f[nlocal:]) <= TOL_F and rel_rms(f, whole.f) <= TOL_F
+
+
 def test_split_call_order_and_arguments(cfg0):
     from paper_2006_09167_b200 import nb
     w, nlocal = halo_workload(cfg0, 0.5)
