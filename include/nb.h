@@ -166,7 +166,8 @@ int nb_forces_prune(nb_ctx*, float rlist_inner, float* f, double* energies, doub
  *     back to their home ranks while the local kernel still runs).
  *   nb_forces_local(f): enqueues the local-local kernel on the context's stream -- it runs next to the non-local one -- and,
  *     after both kernels, writes the forces of the local atoms (local-local + their share of the non-local pairs) to
- *     f[0 .. nlocal).  Must follow nb_forces_nonlocal (NB_ERR_STATE otherwise); after it f equals what nb_forces(f, NULL,
+ *     f[0 .. nlocal).  Must follow nb_forces_nonlocal (NB_ERR_STATE otherwise; so do nb_put_atoms, nb_search, nb_prune and
+ *     nb_forces between the two calls: nothing may overtake the non-local kernel); after it f equals what nb_forces(f, NULL,
  *     NULL) gives, up to the order of the atomic adds.  Force-only flavour (energies / virial: nb_forces).  Not available
  *     while stage timing is on. */
 int nb_set_local(nb_ctx*, int32_t nlocal);

@@ -152,6 +152,7 @@ static int put_atoms_common(nb_ctx* c, const float* x, const float* q, const int
     if (!c) return NB_ERR_ARG;
     DeviceGuard guard(c);
     if (!x || !box) return nb_fail(c, NB_ERR_ARG, "nb_put_atoms: null argument");
+    if (c->nl_pending) return nb_fail(c, NB_ERR_STATE, "nb_put_atoms between nb_forces_nonlocal and nb_forces_local (the non-local kernel may still read the coordinates)");
     if ((!q || !type) && !c->have_atoms)
         return nb_fail(c, NB_ERR_ARG, "nb_put_atoms: q and type may be NULL only after a call that passed them");
     for (int k = 0; k < 3; k++)
@@ -215,6 +216,7 @@ extern "C" int nb_search(nb_ctx* c, float rlist_outer)
     if (!c) return NB_ERR_ARG;
     DeviceGuard guard(c);
     if (!c->have_atoms) return nb_fail(c, NB_ERR_STATE, "nb_search before nb_put_atoms");
+    if (c->nl_pending) return nb_fail(c, NB_ERR_STATE, "nb_search between nb_forces_nonlocal and nb_forces_local");
     const float minL = fminf(c->box[0], fminf(c->box[1], c->box[2]));
     if (!(rlist_outer >= c->prm.rc) || !(rlist_outer <= 0.5f * minL))
         return nb_fail(c, NB_ERR_CUTOFF, "rlist_outer = %g must satisfy rc = %g <= rlist_outer <= min(L)/2 = %g", rlist_outer, c->prm.rc, 0.5f * minL);
@@ -227,6 +229,7 @@ extern "C" int nb_search(nb_ctx* c, float rlist_outer)
 static int prune_checks(nb_ctx* c, float rlist_inner, int part, int nparts)
 {
     if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "nb_prune without a valid list (call nb_search)");
+    if (c->nl_pending) return nb_fail(c, NB_ERR_STATE, "nb_prune between nb_forces_nonlocal and nb_forces_local (the non-local kernel may still read the list)");
     if (nparts < 1 || part < 0 || part >= nparts) return nb_fail(c, NB_ERR_ARG, "nb_prune: part %d of %d", part, nparts);
     if (!(rlist_inner >= c->prm.rc) || !(rlist_inner <= c->rlist_outer))
         return nb_fail(c, NB_ERR_CUTOFF, "rlist_inner = %g must satisfy rc = %g <= rlist_inner <= rlist_outer = %g", rlist_inner, c->prm.rc, c->rlist_outer);
@@ -256,6 +259,7 @@ extern "C" int nb_forces(nb_ctx* c, float* f, double* energies, double* virial)
     if (!f) return nb_fail(c, NB_ERR_ARG, "nb_forces: f is null");
     if (virial && !energies) return nb_fail(c, NB_ERR_ARG, "nb_forces: virial needs energies (same kernel flavour)");
     if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "nb_forces without a valid list (call nb_search)");
+    if (c->nl_pending) return nb_fail(c, NB_ERR_STATE, "nb_forces between nb_forces_nonlocal and nb_forces_local");
     return nbi_forces(c, f, energies, virial);
 }
 

@@ -199,6 +199,11 @@ def test_split_call_order_and_arguments(cfg0):
     with pytest.raises(nb.NbError) as ei:
         d.ctx.set_local(nlocal - 3)             # in the middle of a split step
     assert ei.value.code == -2
+    for call in (lambda: d.put(), lambda: d.ctx.search(w.rlist_outer), lambda: d.ctx.prune(w.rlist_inner, 0, 1),
+                 lambda: d.ctx.forces(d.f)):    # nothing may overtake the non-local kernel: these wait for nb_forces_local
+        with pytest.raises(nb.NbError) as ei:
+            call()
+        assert ei.value.code == -2
     d.ctx.forces_local(d.f)
     d.torch.cuda.synchronize()
     assert rel_rms(d.f.cpu().numpy().astype(np.float64), oracle_forces(w).f) <= TOL_F
