@@ -327,6 +327,7 @@ extern "C" int nb_forces_static(nb_ctx* c, float* f, double* energies, double* v
     if (!f) return nb_fail(c, NB_ERR_ARG, "nb_forces_static: f is null");
     if (virial && !energies) return nb_fail(c, NB_ERR_ARG, "nb_forces_static: virial needs energies (same kernel flavour)");
     if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "nb_forces_static without a valid list (call nb_search)");
+    if (c->nl_pending) return nb_fail(c, NB_ERR_STATE, "nb_forces_static between nb_forces_nonlocal and nb_forces_local");
     return nbi_forces_static(c, f, energies, virial);
 }
 
