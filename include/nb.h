@@ -157,7 +157,7 @@ int nb_forces_prune(nb_ctx*, float rlist_inner, float* f, double* energies, doub
  *     [nlocal, natoms) its NON-LOCAL (halo) atoms.  Takes effect at the next nb_search (required: the current list is
  *     dropped), which grids the two classes separately so that every cluster is purely local or non-local; lists, prune,
  *     nb_forces, nb_step work as before on the union.  nlocal = natoms (the default) switches the split off.
- *   nb_forces_nonlocal(f): enqueues, on the library's HIGH-PRIORITY stream (ordered after everything enqueued on the
+ *   nb_forces_nonlocal(f, energies, virial): enqueues, on the library's HIGH-PRIORITY stream (ordered after everything enqueued on the
  *     context's stream so far), the force kernel over the pairs of the inner list that involve at least one non-local
  *     atom, then writes the finished forces of the non-local atoms to f[nlocal .. natoms) ([dev] natoms*3 as in nb_forces;
  *     rows of local atoms are not touched by this call).  Every atom pair of the system is in exactly one of the two
@@ -168,10 +168,11 @@ int nb_forces_prune(nb_ctx*, float rlist_inner, float* f, double* energies, doub
  *     after both kernels, writes the forces of the local atoms (local-local + their share of the non-local pairs) to
  *     f[0 .. nlocal).  Must follow nb_forces_nonlocal (NB_ERR_STATE otherwise; so do nb_put_atoms, nb_search, nb_prune and
  *     nb_forces between the two calls: nothing may overtake the non-local kernel); after it f equals what nb_forces(f, NULL,
- *     NULL) gives, up to the order of the atomic adds.  Force-only flavour (energies / virial: nb_forces).  Not available
- *     while stage timing is on. */
+ *     NULL) gives, up to the order of the atomic adds.  energies / virial as in nb_forces ([dev]; NULL: the force-only
+ *     kernel flavour): both kernels add into them, they are complete after nb_forces_local.  Not available while stage
+ *     timing is on. */
 int nb_set_local(nb_ctx*, int32_t nlocal);
-int nb_forces_nonlocal(nb_ctx*, float* f);
+int nb_forces_nonlocal(nb_ctx*, float* f, double* energies, double* virial);
 int nb_forces_local(nb_ctx*, float* f);
 int nb_sync_nonlocal(nb_ctx*);
 /* Introspection of the split after nb_search: clusters [0, nclusters_local) hold local atoms only, the others non-local

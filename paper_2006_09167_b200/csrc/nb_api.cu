@@ -281,16 +281,17 @@ extern "C" int nb_set_local(nb_ctx* c, int32_t nlocal)
     return nlocal < c->natoms ? nbi_split_setup(c) : NB_OK;
 }
 
-extern "C" int nb_forces_nonlocal(nb_ctx* c, float* f)
+extern "C" int nb_forces_nonlocal(nb_ctx* c, float* f, double* energies, double* virial)
 {
     if (!c) return NB_ERR_ARG;
     DeviceGuard guard(c);
     if (!f) return nb_fail(c, NB_ERR_ARG, "nb_forces_nonlocal: f is null");
+    if (virial && !energies) return nb_fail(c, NB_ERR_ARG, "nb_forces_nonlocal: virial needs energies (same kernel flavour)");
     if (!c->have_list) return nb_fail(c, NB_ERR_STATE, "nb_forces_nonlocal without a valid list (call nb_search)");
     if (c->nl_pending) return nb_fail(c, NB_ERR_STATE, "nb_forces_nonlocal twice without nb_forces_local");
     if (c->timing) return nb_fail(c, NB_ERR_STATE, "nb_forces_nonlocal: stage timing is not available for the split kernels");
     int rc = nbi_commit_pending(c);
-    return rc != NB_OK ? rc : nbi_forces_nonlocal(c, f);
+    return rc != NB_OK ? rc : nbi_forces_nonlocal(c, f, energies, virial);
 }
 
 extern "C" int nb_forces_local(nb_ctx* c, float* f)

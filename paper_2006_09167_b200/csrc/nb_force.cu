@@ -1027,25 +1027,30 @@ static void force_args_inner(nb_ctx* c, ForceArgs& A)
     }
 }
 
-static int launch_force_range(nb_ctx* c, ForceArgs& A, int base, int count, cudaStream_t st)
+static int launch_force_range(nb_ctx* c, ForceArgs& A, int base, int count, bool energy, cudaStream_t st)
 {
     if (count <= 0) return NB_OK;
     A.seg_base = base;
     A.seg_count = count;
     A.launch_stream = st;
     const bool twin = c->twin;
-    if (c->prm.coulomb == NB_COUL_EWALD) return launch_force_e<NB_COUL_EWALD>(c, A, false, twin, false);
-    if (c->prm.coulomb == NB_COUL_RF) return launch_force_e<NB_COUL_RF>(c, A, false, twin, false);
-    return launch_force_e<NB_COUL_NONE>(c, A, false, twin, false);
+    if (c->prm.coulomb == NB_COUL_EWALD) return launch_force_e<NB_COUL_EWALD>(c, A, energy, twin, false);
+    if (c->prm.coulomb == NB_COUL_RF) return launch_force_e<NB_COUL_RF>(c, A, energy, twin, false);
+    return launch_force_e<NB_COUL_NONE>(c, A, energy, twin, false);
 }
 
-// gather of the slots [slot0, slot1) (multiples of 64) to the caller's atom order
-static int gather_range(nb_ctx* c, int slot0, int slot1, float* f, cudaStream_t st)
+// gather of the slots [slot0, slot1) (multiples of 64) to the caller's atom order; with_virial: also sum x (x) f into xf
+static int gather_range(nb_ctx* c, int slot0, int slot1, float* f, bool with_virial, cudaStream_t st)
 {
-    const int nq = (slot1 - slot0) / 4;
-    if (nq <= 0) return NB_OK;
-    NB_CUDA(c, nb_launch_pdl(k_gather4, dim3((nq + 255) / 256), dim3(256), 0, st, nq, c->f4.p + slot0,
-                             reinterpret_cast<const int4*>(c->atom_of_slot.p + slot0), f));
+    const int ns = slot1 - slot0;
+    if (ns <= 0) return NB_OK;
+    if (with_virial)
+        NB_CUDA(c, nb_launch_pdl(k_gather<true>, dim3((ns + 255) / 256), dim3(256), 0, st, ns, c->f4.p + slot0,
+                                 (const int*)(c->atom_of_slot.p + slot0), (const float4*)(c->xq.p + slot0), f,
+                                 c->fshift.p + NB_NSHIFT * 3));
+    else
+        NB_CUDA(c, nb_launch_pdl(k_gather4, dim3((ns / 4 + 255) / 256), dim3(256), 0, st, ns / 4, c->f4.p + slot0,
+                                 reinterpret_cast<const int4*>(c->atom_of_slot.p + slot0), f));
     NB_LAUNCH_CHECK(c);
     return NB_OK;
 }
@@ -1074,17 +1079,28 @@ void nbi_split_free(nb_ctx* c)
 
 // The non-local kernel and the gather of the non-local atoms' forces, on the high-priority stream, ordered after
 // everything enqueued on the context's stream so far (coordinates, prune).
-int nbi_forces_nonlocal(nb_ctx* c, float* f)
+// energies / virial (as in nb_forces): both kernels add into them; they are complete after nb_forces_local.
+int nbi_forces_nonlocal(nb_ctx* c, float* f, double* energies, double* virial)
 {
     int rc = nbi_split_setup(c);
     if (rc != NB_OK) return rc;
+    const bool energy = energies != nullptr;
+    if (energy) {   // cleared on the context's stream, before either kernel can start
+        NB_CUDA(c, c->fshift.ensure(NB_NSHIFT * 3 + 9, c->stream));
+        NB_CUDA(c, cudaMemsetAsync(energies, 0, 2 * sizeof(double), c->stream));
+        NB_CUDA(c, cudaMemsetAsync(c->fshift.p, 0, (NB_NSHIFT * 3 + 9) * sizeof(double), c->stream));
+    }
+    c->nl_energies = energies;
+    c->nl_virial = virial;
     NB_CUDA(c, cudaEventRecord(c->ev_nl_in, c->stream));
     NB_CUDA(c, cudaStreamWaitEvent(c->stream_hp, c->ev_nl_in, 0));
     ForceArgs A;
     force_args_inner(c, A);
-    if ((rc = launch_force_range(c, A, c->nseg_local, c->nseg_launch - c->nseg_local, c->stream_hp)) != NB_OK) return rc;
+    A.fshift = c->fshift.p;
+    A.energies = energies;
+    if ((rc = launch_force_range(c, A, c->nseg_local, c->nseg_launch - c->nseg_local, energy, c->stream_hp)) != NB_OK) return rc;
     NB_CUDA(c, cudaEventRecord(c->ev_nl_kernel, c->stream_hp));
-    if ((rc = gather_range(c, c->nsc_local * NB_SC_ATOMS, c->nslots_max, f, c->stream_hp)) != NB_OK) return rc;
+    if ((rc = gather_range(c, c->nsc_local * NB_SC_ATOMS, c->nslots_max, f, virial != nullptr, c->stream_hp)) != NB_OK) return rc;
     NB_CUDA(c, cudaEventRecord(c->ev_nl_done, c->stream_hp));
     c->nl_pending = true;
     c->st.force_count++;
@@ -1097,12 +1113,19 @@ int nbi_forces_local(nb_ctx* c, float* f)
 {
     ForceArgs A;
     force_args_inner(c, A);
-    int rc = launch_force_range(c, A, 0, c->nseg_local, c->stream);
+    A.fshift = c->fshift.p;
+    A.energies = c->nl_energies;
+    int rc = launch_force_range(c, A, 0, c->nseg_local, c->nl_energies != nullptr, c->stream);
     if (rc != NB_OK) return rc;
     NB_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_nl_kernel, 0));
-    if ((rc = gather_range(c, 0, c->nsc_local * NB_SC_ATOMS, f, c->stream)) != NB_OK) return rc;
+    if ((rc = gather_range(c, 0, c->nsc_local * NB_SC_ATOMS, f, c->nl_virial != nullptr, c->stream)) != NB_OK) return rc;
     // later work on the context's stream (the next put / prune / search) must not overtake the non-local gather
     NB_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_nl_done, 0));
+    if (c->nl_virial) {   // both gathers have added their sum x (x) f, both kernels their per-shift force sums
+        k_virial_final<<<1, 32, 0, c->stream>>>(c->fshift.p + NB_NSHIFT * 3, c->fshift.p, make_float3(c->box[0], c->box[1], c->box[2]),
+                                                c->nl_virial);
+        NB_LAUNCH_CHECK(c);
+    }
     c->nl_pending = false;
     return NB_OK;
 }

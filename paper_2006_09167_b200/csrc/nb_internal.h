@@ -132,6 +132,7 @@ struct nb_ctx {
     cudaStream_t stream_hp = nullptr;          // high-priority stream of the non-local kernel
     cudaEvent_t ev_nl_in = nullptr, ev_nl_kernel = nullptr, ev_nl_done = nullptr;
     bool nl_pending = false;                   // nb_forces_nonlocal enqueued, nb_forces_local not yet
+    double *nl_energies = nullptr, *nl_virial = nullptr;   // the caller's outputs of that pending pair of calls
     float inv_cx = 0.f, inv_cy = 0.f;          // columns per nm
     DevBuf<int32_t> col_count, col_atom_off, col_sc_off, atom_col, atom_rank, col_atoms;
     DevBuf<char4> image;                       // periodic image fixed at the last search
@@ -395,7 +396,7 @@ const void* nbi_put_kernel();                               // nb_grid.cu: the k
 const void* nbi_gather4_kernel();                           // nb_force.cu: the k_gather4 entry
 int nbi_split_setup(nb_ctx* c);                             // nb_force.cu: high-priority stream and events of the local / non-local split
 void nbi_split_free(nb_ctx* c);
-int nbi_forces_nonlocal(nb_ctx* c, float* f);               // nb_force.cu: non-local kernel + gather of the non-local atoms
+int nbi_forces_nonlocal(nb_ctx* c, float* f, double* energies, double* virial);               // nb_force.cu: non-local kernel + gather of the non-local atoms
 int nbi_forces_local(nb_ctx* c, float* f);                  // nb_force.cu: local kernel + gather of the local atoms
 int nbi_sync_nonlocal(nb_ctx* c);
 void nbi_static_scratch_setup(nb_ctx* c);                   // nb_force.cu: resolves c->static_scratch (the context's device is current)

@@ -149,8 +149,8 @@ class Context:
         """Atoms [0, nlocal) are local, the rest non-local (halo); takes effect at the next search."""
         self._check(lib().nb_set_local(self._h, C.c_int32(int(nlocal))))
 
-    def forces_nonlocal(self, f):
-        self._check(lib().nb_forces_nonlocal(self._h, _dptr(f)))
+    def forces_nonlocal(self, f, energies=None, virial=None):
+        self._check(lib().nb_forces_nonlocal(self._h, _dptr(f), _dptr(energies), _dptr(virial)))
 
     def forces_local(self, f):
         self._check(lib().nb_forces_local(self._h, _dptr(f)))

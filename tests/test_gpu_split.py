@@ -88,6 +88,23 @@ def test_split_small_systems(which):
     _, f2 = split_forces(d, nlocal)
     assert rel_rms(f2, whole.f) <= TOL_F
     assert rel_rms(d.forces(), whole.f) <= TOL_F
+    # the F + E + virial flavour of the pair: both kernels add into the energies and the per-shift sums, both gathers into
+    # sum x (x) f; complete after nb_forces_local
+    d.f.fill_(float("nan"))
+    d.e.fill_(float("nan"))
+    d.v.fill_(float("nan"))
+    d.ctx.forces_nonlocal(d.f, d.e, d.v)
+    d.ctx.sync_nonlocal()
+    d.ctx.forces_local(d.f)
+    d.torch.cuda.synchronize()
+    fe, ee, ve = d.f.cpu().numpy().astype(np.float64), d.e.cpu().numpy(), d.v.cpu().numpy().reshape(3, 3)
+    assert rel_rms(fe, whole.f) <= TOL_F
+    assert abs(ee[0] - whole.e_lj) <= 1e-5 * abs(whole.energy) and abs(ee[1] - whole.e_coul) <= 1e-5 * abs(whole.energy)
+    assert np.linalg.norm(ve - whole.virial) <= 1e-5 * np.linalg.norm(whole.virial)
+    assert np.allclose(ee, e, rtol=1e-9, atol=1e-9 * abs(whole.energy)) and np.linalg.norm(ve - v) <= 1e-5 * np.linalg.norm(v)
+    with pytest.raises(Exception):
+        d.ctx.forces_nonlocal(d.f, None, d.v)      # virial needs energies
+    assert rel_rms(d.forces(), whole.f) <= TOL_F   # (the rejected call left no split step pending)
     # the local kernel alone = the local atoms alone (oracle part 1): non-local forces on the local atoms are the difference
     loc = split_oracle(w, nlocal, 1)
     assert rel_rms(f[:nlocal] - nl.f[:nlocal], loc.f[:nlocal]) <= 1e-4   # (difference of two fp32 results)
